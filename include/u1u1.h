@@ -1,0 +1,179 @@
+/*
+ * u1u1.h -- C ABI of the B200-native U(1)xU(1) lattice field evolution library (libu1u1.so).
+ *
+ * The library evolves Saffin's dual-U(1) model (two complex scalars phi, psi with conjugate momenta
+ * Pi, Psi; two gauge fields A, B stored as link phases theta = dx*A with electric fields E, H;
+ * 20 fp32 words per site) on a periodic N^3 comoving lattice, as discretised in Correia & Martins,
+ * arXiv:2208.01525 (cited below as PAPER.md:<line>), and computes the paper's in-loop diagnostics.
+ * Every step of that path runs in hand-written sm_100a CUDA kernels; there is no CPU fallback.
+ *
+ * Conventions
+ *   - Plain C types only.  Pointers are marked HOST or DEVICE.  The library never allocates or
+ *     frees device memory: the caller owns `state_dev` and `scratch_dev` for the life of the context.
+ *   - All work is enqueued on the CUDA stream given to u1u1_create (a cudaStream_t passed as void*;
+ *     NULL = the legacy default stream).  Calls that fill HOST output synchronise that stream.
+ *   - Every int-returning call returns 0 on success or a negative U1U1_E* code; no exception crosses
+ *     the ABI.  u1u1_last_error(ctx) returns a human-readable message for the last failure.
+ *   - Canonical state layout (export/import): float32 [20][N][N][N], x fastest, components
+ *       0 phi_re 1 phi_im 2 Pi_re 3 Pi_im 4 psi_re 5 psi_im 6 Psi_re 7 Psi_im
+ *       8..10 thetaA_xyz  11..13 E_xyz  14..16 thetaB_xyz  17..19 H_xyz
+ *     theta_i = dx*A_i is NON-compact (never reduced mod 2 pi; the paper's gauge action is the
+ *     non-compact one); E_i = dA_i/dtau.  The internal layout differs.
+ *   - Time levels: positions (phi, psi, theta) at tau, momenta (Pi, Psi, E, H) at tau - dtau/2.
+ */
+#ifndef U1U1_H
+#define U1U1_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define U1U1_OK 0
+#define U1U1_EINVAL (-1)   /* bad argument, NULL pointer, struct_size mismatch                   */
+#define U1U1_ESIZE (-2)    /* N unsupported, or a caller buffer is too small                     */
+#define U1U1_EPARAM (-3)   /* couplings outside 0 <= kappa < sqrt(lambda1 lambda2)/2 */
+#define U1U1_ESTATE (-4)   /* call out of order (e.g. step before init_fields / configure)        */
+#define U1U1_ECUDA (-5)    /* a CUDA runtime call or kernel launch failed                         */
+#define U1U1_EUNSTABLE (-6)/* dtau^2 (12/dx^2 + (lambda+2kappa) sigma^2 a^{2s}) >= 4: leapfrog unstable */
+
+#define U1U1_DIAG_LEN 48   /* doubles written by u1u1_diagnostics  */
+#define U1U1_GAUSS_LEN 8   /* doubles written by u1u1_gauss_violation */
+
+typedef struct u1u1_ctx u1u1_ctx;
+
+/* Model and run parameters.  Couplings are the a=1 values of PAPER.md:89 Eq. 12. */
+typedef struct {
+    uint32_t struct_size; /* = sizeof(u1u1_params); checked                                     */
+    int32_t init_kind;    /* 0: |phi|=eta1,|psi|=eta2 with iid uniform phases
+                             1: Gaussian-smoothed complex white noise normalised to the same moduli
+                                (BASELINE.json config 3)                                         */
+    double lambda1, lambda2; /* lambda_p0, lambda_q0   (Eq. 4)                       */
+    double e1, e2;           /* e_p0, e_q0             (Eq. 2)                       */
+    double eta1, eta2;       /* sigma_p, sigma_q: the symmetry-breaking scales     */
+    double kappa;            /* kappa_0                (PAPER.md:52 Eq. 4, :89 Eq. 12)           */
+    double dtau;             /* conformal timestep Delta eta                      */
+    double tau_norm;         /* conformal time at which a = 1 (a = (tau/tau_norm)^p), > 0        */
+    double friction;         /* every momentum is multiplied by this after the kick; 1 = off
+                                (damping prephase of BASELINE.json configs 2 and 5)              */
+    double smooth_width;     /* init_kind 1: Gaussian width in lattice units                     */
+    int32_t smooth_trunc;    /* init_kind 1: kernel truncated at |d| <= smooth_trunc (<= 32)     */
+    int32_t kernel_variant;  /* 0 = default (fastest); 1 = reference one-thread-per-site kernel   */
+} u1u1_params;
+
+/* Bytes of device memory the caller must provide for an N^3 lattice.
+ * state  : 30 fp32 words/site (20 fields + a second copy of the 10 position words, ping-pong).
+ * scratch: winding codes (6 B/site), cell arrays (2 B/site), reduction partials. */
+size_t u1u1_state_bytes(int32_t N);
+size_t u1u1_scratch_bytes(int32_t N);
+
+/* Create a context over caller-owned DEVICE buffers (256-byte aligned) and a CUDA stream.
+ * Nothing is launched.  *ctx is a small HOST object, released by u1u1_destroy. */
+int u1u1_create(u1u1_ctx **ctx, void *state_dev, size_t state_bytes, void *scratch_dev,
+                size_t scratch_bytes, void *cuda_stream);
+void u1u1_destroy(u1u1_ctx *ctx);
+const char *u1u1_last_error(const u1u1_ctx *ctx); /* ctx may be NULL: returns the create() error */
+
+/* Set lattice size, spacing and parameters without touching the fields (used before import_state).
+ * N must be a multiple of 4 with 8 <= N <= 1024 and fit the buffers given to u1u1_create. */
+int u1u1_configure(u1u1_ctx *ctx, int32_t N, double dx, const u1u1_params *params);
+
+/* init_fields(seed, N, dx, params)  [north_star; PAPER.md:162]: configure, then generate the initial
+ * condition on the device: scalars per params->init_kind from Philox4x32-10 keyed by `seed` with the
+ * site's linear index (ix + N(iy + N iz)) as counter; Pi, Psi, theta, E, H = 0. */
+int u1u1_init_fields(u1u1_ctx *ctx, uint64_t seed, int32_t N, double dx, const u1u1_params *params);
+
+/* Replace parameters between phases (friction on/off, tau_norm, couplings); N, dx unchanged. */
+int u1u1_set_params(u1u1_ctx *ctx, const u1u1_params *params);
+
+/* Declare the conformal time and background of the CURRENT state without stepping: sets the scale
+ * factor weights used by diagnostics / gauss_violation (c = cG = a(tau)^{2s}).  Needed only when a
+ * state is imported and examined before any step. */
+int u1u1_set_time(u1u1_ctx *ctx, double tau, double era_m, double s);
+
+/* step(n, tau, era, s)  [north_star; Eq. 17-26]: n fused kick+drift leapfrog steps.
+ * On entry positions are at `tau`, momenta at tau - dtau/2; step k uses tau_k = tau + k*dtau (fp64,
+ * no accumulation).  era_m = m of a ∝ t^m (0 flat, 0.5 radiation, 2/3 matter, any 0 <= m < 1);
+ * s = beta of PAPER.md:89 Eq. 12 (1 physical, 0 constant comoving width, < 0 core growth).
+ * Asynchronous: returns after enqueueing. */
+int u1u1_step(u1u1_ctx *ctx, int32_t n, double tau, double era_m, double s);
+
+/* diagnostics(out)  [north_star; PAPER.md:183-224 Eq. 31-37, :230-238]: out = HOST array of
+ * U1U1_DIAG_LEN doubles, slots named by the U1U1_D_* enum below.  Uses the scale factor of the last
+ * completed step (or of `tau_norm`-normalised a=1 before any step).  Synchronises the stream. */
+int u1u1_diagnostics(u1u1_ctx *ctx, double *out_host);
+
+/* gauss_violation(out)  [north_star; PAPER.md:73-77 Eq. 9-10, :272]: out = HOST array of 8 doubles,
+ * per sector (p then q): ||g||_2, ||rho||_2, max|g|, ||g||_2 / max(||rho||_2, ||div E||_2, tiny), with
+ * g(x) = sum_i [E_i(x)-E_i(x-i)]/dx - rho(x), rho = 2 e0^2 cG Im(conj(phi) Pi) and
+ * cG = c (1+delta)/(1+omega) of the last completed step.  Synchronises the stream. */
+int u1u1_gauss_violation(u1u1_ctx *ctx, double *out_host);
+
+/* Canonical-layout copies, DEVICE<->DEVICE (float32 [20][N][N][N]) and HOST<->DEVICE variants
+ * (the host variants copy through the same stream and synchronise it). */
+int u1u1_export_state(u1u1_ctx *ctx, void *dst_dev);
+int u1u1_import_state(u1u1_ctx *ctx, const void *src_dev);
+int u1u1_export_state_host(u1u1_ctx *ctx, void *dst_host);
+int u1u1_import_state_host(u1u1_ctx *ctx, const void *src_host);
+
+/* Canonical sub-block float32 [20][bz][by][bx] whose corner is site (x0,y0,z0), periodic wrap, to a
+ * DEVICE buffer: lets a caller inspect a 1024^3 state (for which a full canonical copy does not fit
+ * beside the state) -- used by the sampled full-size parity test. */
+int u1u1_export_block(u1u1_ctx *ctx, int32_t x0, int32_t y0, int32_t z0, int32_t bx, int32_t by, int32_t bz,
+                      void *dst_dev);
+
+/* After u1u1_diagnostics: copy out the per-plaquette windings of `sector` (0 = p, 1 = q) as
+ * int8 W[3][N][N][N] (orientation xy, yz, zx) and the near-branch-cut flags uint8 near[3][N][N][N]
+ * (1 if any of the plaquette's four link angles lies within 1e-5 of +-pi), and the pierced-cell
+ * array uint8 C[N][N][N].  DEVICE destinations; any of them may be NULL. */
+int u1u1_export_windings(u1u1_ctx *ctx, int32_t sector, void *w_dev, void *near_dev, void *cells_dev);
+
+/* Number of kernel launches issued by this context so far (for bench.py's gpu_launches). */
+uint64_t u1u1_launch_count(const u1u1_ctx *ctx);
+
+/* Slots of the diagnostics array. */
+enum {
+    U1U1_D_TAU = 0,      /* conformal time of the positions                                      */
+    U1U1_D_A,            /* scale factor a(tau)                                                  */
+    U1U1_D_C,            /* c = a^{2s} used for the weights                                      */
+    U1U1_D_SUMW_P,       /* sum over plaquettes |W^p|                             */
+    U1U1_D_SUMW_Q,
+    U1U1_D_CELLS_P,      /* cells pierced by p windings                                          */
+    U1U1_D_CELLS_Q,
+    U1U1_D_CELLS_PQ,     /* cells pierced by both (fast method, exact overlap)      */
+    U1U1_D_NEAR_P,       /* plaquettes with a link angle within 1e-5 of the branch cut            */
+    U1U1_D_NEAR_Q,
+    U1U1_D_MAXW,         /* max |W| over both sectors (never >= 2 at equal tension) */
+    U1U1_D_SUM_L,        /* sum_x L_x                         (Eq. 33)               */
+    U1U1_D_SUM_KIN_L,    /* sum_x (|Pi|^2+|Psi|^2) L_x        (Eq. 37, W = L)        */
+    U1U1_D_SUM_GRAD_L,   /* sum_x,i (|D+phi|^2+|D+psi|^2) L_x                                    */
+    U1U1_D_SUM_KIN_V,    /* same with W = V_int = kappa0(|phi|^2-s_p^2)(|psi|^2-s_q^2) (:224)     */
+    U1U1_D_SUM_GRAD_V,
+    U1U1_D_SUM_VINT,
+    U1U1_D_SUM_KIN,      /* energy components, no scale-factor weights, not multiplied by dx^3    */
+    U1U1_D_SUM_GRAD,
+    U1U1_D_SUM_ELEC,
+    U1U1_D_SUM_MAG,
+    U1U1_D_SUM_POT,
+    U1U1_D_L_P,          /* derived, Eq. 31-37 ------------------------------- */
+    U1U1_D_L_Q,
+    U1U1_D_L_PQ,
+    U1U1_D_XI_P,
+    U1U1_D_XI_Q,
+    U1U1_D_XI_PQ,
+    U1U1_D_XI_W,
+    U1U1_D_XI_L,
+    U1U1_D_F_TOTAL,
+    U1U1_D_F_P,
+    U1U1_D_V2_L,
+    U1U1_D_V2_PQ,
+    U1U1_D_ENERGY,       /* dx^3 (kin+grad+elec+mag+pot): the flat-space Hamiltonian              */
+    U1U1_D_USED          /* number of slots in use; the rest of the 48 are zero                   */
+};
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* U1U1_H */

@@ -1,0 +1,92 @@
+"""Thin ctypes binding of libu1u1.so (include/u1u1.h): same names, argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of the library; there is no CPU or PyTorch fallback:
+if the shared library is missing, `load()` raises.  PyTorch is used by the `Lattice` helper only to
+own device memory and the stream.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libu1u1.so")
+
+DIAG_LEN = 48
+GAUSS_LEN = 8
+DIAG_SLOTS = ["tau", "a", "c", "sumW_p", "sumW_q", "cells_p", "cells_q", "cells_pq", "near_p", "near_q",
+              "maxW", "sum_L", "sum_kin_L", "sum_grad_L", "sum_kin_V", "sum_grad_V", "sum_vint", "sum_kin",
+              "sum_grad", "sum_elec", "sum_mag", "sum_pot", "L_p", "L_q", "L_pq", "xi_p", "xi_q", "xi_pq",
+              "xi_W", "xi_L", "f_total", "f_p", "v2_L", "v2_pq", "energy"]
+ERRORS = {-1: "EINVAL", -2: "ESIZE", -3: "EPARAM", -4: "ESTATE", -5: "ECUDA", -6: "EUNSTABLE"}
+
+
+class Params(ctypes.Structure):
+    """u1u1_params (include/u1u1.h).  Defaults: the paper's validation couplings."""
+    _fields_ = [("struct_size", ctypes.c_uint32), ("init_kind", ctypes.c_int32),
+                ("lambda1", ctypes.c_double), ("lambda2", ctypes.c_double),
+                ("e1", ctypes.c_double), ("e2", ctypes.c_double),
+                ("eta1", ctypes.c_double), ("eta2", ctypes.c_double),
+                ("kappa", ctypes.c_double), ("dtau", ctypes.c_double),
+                ("tau_norm", ctypes.c_double), ("friction", ctypes.c_double),
+                ("smooth_width", ctypes.c_double), ("smooth_trunc", ctypes.c_int32),
+                ("kernel_variant", ctypes.c_int32)]
+
+    def __init__(self, **kw):
+        d = dict(init_kind=0, lambda1=2.0, lambda2=2.0, e1=1.0, e2=1.0, eta1=1.0, eta2=1.0, kappa=0.9,
+                 dtau=0.1, tau_norm=1.0, friction=1.0, smooth_width=5.0, smooth_trunc=20, kernel_variant=0)
+        d.update(kw)
+        super().__init__(struct_size=ctypes.sizeof(Params), **d)
+
+
+class U1U1Error(RuntimeError):
+    pass
+
+
+_lib = None
+SYMBOLS = ["u1u1_state_bytes", "u1u1_scratch_bytes", "u1u1_create", "u1u1_destroy", "u1u1_last_error",
+           "u1u1_configure", "u1u1_init_fields", "u1u1_set_params", "u1u1_set_time", "u1u1_step",
+           "u1u1_diagnostics", "u1u1_gauss_violation", "u1u1_export_state", "u1u1_import_state",
+           "u1u1_export_state_host", "u1u1_import_state_host", "u1u1_export_windings", "u1u1_export_block", "u1u1_launch_count"]
+
+
+def load():
+    """dlopen libu1u1.so (built in-tree by paper_2208_01525_b200.build).  Fails loudly if absent."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise U1U1Error(f"{LIB_PATH} not found: run `python -m paper_2208_01525_b200.build` "
+                        "(there is no CPU fallback)")
+    L = ctypes.CDLL(LIB_PATH)
+    vp, d, i32, u64 = ctypes.c_void_p, ctypes.c_double, ctypes.c_int32, ctypes.c_uint64
+    dp, pp = ctypes.POINTER(ctypes.c_double), ctypes.POINTER(Params)
+    L.u1u1_state_bytes.argtypes = [i32]; L.u1u1_state_bytes.restype = ctypes.c_size_t
+    L.u1u1_scratch_bytes.argtypes = [i32]; L.u1u1_scratch_bytes.restype = ctypes.c_size_t
+    L.u1u1_create.argtypes = [ctypes.POINTER(vp), vp, ctypes.c_size_t, vp, ctypes.c_size_t, vp]
+    L.u1u1_destroy.argtypes = [vp]; L.u1u1_destroy.restype = None
+    L.u1u1_last_error.argtypes = [vp]; L.u1u1_last_error.restype = ctypes.c_char_p
+    L.u1u1_configure.argtypes = [vp, i32, d, pp]
+    L.u1u1_init_fields.argtypes = [vp, u64, i32, d, pp]
+    L.u1u1_set_params.argtypes = [vp, pp]
+    L.u1u1_set_time.argtypes = [vp, d, d, d]
+    L.u1u1_step.argtypes = [vp, i32, d, d, d]
+    L.u1u1_diagnostics.argtypes = [vp, dp]
+    L.u1u1_gauss_violation.argtypes = [vp, dp]
+    L.u1u1_export_state.argtypes = [vp, vp]
+    L.u1u1_import_state.argtypes = [vp, vp]
+    L.u1u1_export_state_host.argtypes = [vp, vp]
+    L.u1u1_import_state_host.argtypes = [vp, vp]
+    L.u1u1_export_windings.argtypes = [vp, i32, vp, vp, vp]
+    L.u1u1_export_block.argtypes = [vp, i32, i32, i32, i32, i32, i32, vp]
+    L.u1u1_launch_count.argtypes = [vp]; L.u1u1_launch_count.restype = u64
+    _lib = L
+    return L
+
+
+def state_bytes(N: int) -> int:
+    return load().u1u1_state_bytes(N)
+
+
+def scratch_bytes(N: int) -> int:
+    return load().u1u1_scratch_bytes(N)

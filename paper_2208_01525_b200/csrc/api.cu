@@ -1,0 +1,426 @@
+// api.cu -- the C ABI of libu1u1.so (include/u1u1.h): context, host-side per-step scalars
+// (PAPER.md:133 Eq. 19, :147 Eq. 22, :89 Eq. 12), launch sequencing, derived diagnostics
+// (Eq. 31-37).  No device memory is allocated here; no CPU compute path exists.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+
+#include "../../include/u1u1.h"
+#include "common.cuh"
+#include "kernels.h"
+
+using namespace u1u1;
+
+struct u1u1_ctx {
+    float *state = nullptr;      // caller-owned: [pos0 | pos1 | mom]
+    size_t state_bytes = 0;
+    uint8_t *scratch = nullptr;  // caller-owned
+    size_t scratch_bytes = 0;
+    cudaStream_t stream = nullptr;
+    int N = 0;
+    size_t V = 0;
+    double dx = 0;
+    u1u1_params prm{};
+    bool configured = false;
+    int cur = 0;                 // which ping-pong buffer holds the current positions
+    // time bookkeeping for the diagnostic weights
+    double tau_pos = 0.0;        // conformal time of the positions
+    double a = 1.0, c = 1.0, cG = 1.0;
+    bool diag_valid = false;     // scratch holds windings of the current state
+    uint64_t launches = 0;
+    std::string err;
+};
+
+static std::string g_create_err;
+
+static int fail(u1u1_ctx *ctx, int code, const std::string &msg)
+{
+    if (ctx) ctx->err = msg; else g_create_err = msg;
+    return code;
+}
+
+static int cuda_fail(u1u1_ctx *ctx, cudaError_t e, const char *where)
+{
+    return fail(ctx, U1U1_ECUDA, std::string(where) + ": " + cudaGetErrorString(e));
+}
+
+static bool size_ok(int32_t N) { return N >= 8 && N <= 1024 && (N % 4) == 0; }
+
+// scratch layout: [winding codes 6V][cells 2V] pad-> [partials RED_MAX_BLOCKS*RED_SLOTS doubles][result 64 doubles]
+static size_t scratch_partials_offset(size_t V) { return ((8 * V + 255) / 256) * 256; }
+
+extern "C" size_t u1u1_state_bytes(int32_t N)
+{
+    if (!size_ok(N)) return 0;
+    return (size_t)(2 * NPOS + NMOM) * (size_t)N * N * N * sizeof(float);
+}
+
+extern "C" size_t u1u1_scratch_bytes(int32_t N)
+{
+    if (!size_ok(N)) return 0;
+    const size_t V = (size_t)N * N * N;
+    return scratch_partials_offset(V) + ((size_t)RED_MAX_BLOCKS * RED_SLOTS + 64) * sizeof(double);
+}
+
+extern "C" int u1u1_create(u1u1_ctx **out, void *state_dev, size_t state_bytes, void *scratch_dev,
+                           size_t scratch_bytes, void *cuda_stream)
+{
+    if (!out || !state_dev || !scratch_dev) return fail(nullptr, U1U1_EINVAL, "u1u1_create: NULL argument");
+    if (((uintptr_t)state_dev & 255) || ((uintptr_t)scratch_dev & 255))
+        return fail(nullptr, U1U1_EINVAL, "u1u1_create: device buffers must be 256-byte aligned");
+    u1u1_ctx *ctx = new (std::nothrow) u1u1_ctx;
+    if (!ctx) return fail(nullptr, U1U1_EINVAL, "u1u1_create: out of host memory");
+    ctx->state = (float *)state_dev;
+    ctx->state_bytes = state_bytes;
+    ctx->scratch = (uint8_t *)scratch_dev;
+    ctx->scratch_bytes = scratch_bytes;
+    ctx->stream = (cudaStream_t)cuda_stream;
+    *out = ctx;
+    return U1U1_OK;
+}
+
+extern "C" void u1u1_destroy(u1u1_ctx *ctx) { delete ctx; }
+
+extern "C" const char *u1u1_last_error(const u1u1_ctx *ctx)
+{
+    return ctx ? ctx->err.c_str() : g_create_err.c_str();
+}
+
+extern "C" uint64_t u1u1_launch_count(const u1u1_ctx *ctx) { return ctx ? ctx->launches : 0; }
+
+static int check_params(u1u1_ctx *ctx, const u1u1_params *p)
+{
+    if (!p) return fail(ctx, U1U1_EINVAL, "params is NULL");
+    if (p->struct_size != sizeof(u1u1_params))
+        return fail(ctx, U1U1_EINVAL, "params->struct_size does not match this library's u1u1_params");
+    if (!(p->lambda1 > 0 && p->lambda2 > 0 && p->e1 > 0 && p->e2 > 0 && p->eta1 > 0 && p->eta2 > 0))
+        return fail(ctx, U1U1_EPARAM, "couplings and symmetry-breaking scales must be positive");
+    if (!(p->kappa >= 0 && p->kappa < 0.5 * std::sqrt(p->lambda1 * p->lambda2)))
+        return fail(ctx, U1U1_EPARAM, "need 0 <= kappa < sqrt(lambda1 lambda2)/2 (PAPER.md:55)");
+    if (!(p->dtau > 0) || !(p->tau_norm > 0) || !(p->friction > 0 && p->friction <= 1.0))
+        return fail(ctx, U1U1_EPARAM, "need dtau > 0, tau_norm > 0, 0 < friction <= 1");
+    if (p->init_kind != 0 && p->init_kind != 1) return fail(ctx, U1U1_EINVAL, "init_kind must be 0 or 1");
+    if (p->init_kind == 1 && (!(p->smooth_width > 0) || p->smooth_trunc < 1 || p->smooth_trunc > 32))
+        return fail(ctx, U1U1_EINVAL, "init_kind 1 needs smooth_width > 0 and 1 <= smooth_trunc <= 32");
+    if (p->kernel_variant < 0 || p->kernel_variant > 1) return fail(ctx, U1U1_EINVAL, "kernel_variant must be 0 or 1");
+    return U1U1_OK;
+}
+
+static float *pos_buf(u1u1_ctx *ctx, int which) { return ctx->state + (size_t)which * NPOS * ctx->V; }
+static float *mom_buf(u1u1_ctx *ctx) { return ctx->state + (size_t)2 * NPOS * ctx->V; }
+static double *partials(u1u1_ctx *ctx) { return (double *)(ctx->scratch + scratch_partials_offset(ctx->V)); }
+static double *result(u1u1_ctx *ctx) { return partials(ctx) + (size_t)RED_MAX_BLOCKS * RED_SLOTS; }
+
+extern "C" int u1u1_configure(u1u1_ctx *ctx, int32_t N, double dx, const u1u1_params *params)
+{
+    if (!ctx) return U1U1_EINVAL;
+    if (!size_ok(N)) return fail(ctx, U1U1_ESIZE, "N must be a multiple of 4 with 8 <= N <= 1024");
+    if (!(dx > 0)) return fail(ctx, U1U1_EINVAL, "dx must be positive");
+    if (int rc = check_params(ctx, params)) return rc;
+    if (ctx->state_bytes < u1u1_state_bytes(N)) return fail(ctx, U1U1_ESIZE, "state buffer smaller than u1u1_state_bytes(N)");
+    if (ctx->scratch_bytes < u1u1_scratch_bytes(N)) return fail(ctx, U1U1_ESIZE, "scratch buffer smaller than u1u1_scratch_bytes(N)");
+    ctx->N = N;
+    ctx->V = (size_t)N * N * N;
+    ctx->dx = dx;
+    ctx->prm = *params;
+    ctx->configured = true;
+    ctx->cur = 0;
+    ctx->tau_pos = params->tau_norm;
+    ctx->a = ctx->c = ctx->cG = 1.0;
+    ctx->diag_valid = false;
+    return U1U1_OK;
+}
+
+extern "C" int u1u1_set_params(u1u1_ctx *ctx, const u1u1_params *params)
+{
+    if (!ctx) return U1U1_EINVAL;
+    if (!ctx->configured) return fail(ctx, U1U1_ESTATE, "set_params before configure/init_fields");
+    if (int rc = check_params(ctx, params)) return rc;
+    ctx->prm = *params;
+    return U1U1_OK;
+}
+
+extern "C" int u1u1_init_fields(u1u1_ctx *ctx, uint64_t seed, int32_t N, double dx, const u1u1_params *params)
+{
+    if (int rc = u1u1_configure(ctx, N, dx, params)) return rc;
+    const size_t V = ctx->V;
+    cudaError_t e = cudaMemsetAsync(ctx->state, 0, u1u1_state_bytes(N), ctx->stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "init_fields memset");
+    if (params->init_kind == 0) {
+        e = launch_init_random_phase(pos_buf(ctx, 0), V, seed, params->eta1, params->eta2, ctx->stream);
+        ctx->launches += 1;
+    } else {
+        // the second position buffer is free at init time: use 8 of its planes as temporaries
+        float *tmp = pos_buf(ctx, 1);
+        e = launch_init_smoothed(pos_buf(ctx, 0), tmp, tmp + 4 * V, V, N, seed, params->smooth_width,
+                                 params->smooth_trunc, params->eta1, params->eta2, ctx->stream);
+        ctx->launches += 5;
+        if (e == cudaSuccess) e = cudaMemsetAsync(tmp, 0, (size_t)NPOS * V * sizeof(float), ctx->stream);
+    }
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "init_fields");
+    return U1U1_OK;
+}
+
+// a, c = a^{2s}, delta, omega at conformal time tau (fp64).
+static void scalars_at(const u1u1_ctx *ctx, double tau, double m, double s, double &a, double &c,
+                       double &delta, double &omega)
+{
+    const double p = m / (1.0 - m);
+    a = (m == 0.0) ? 1.0 : std::pow(tau / ctx->prm.tau_norm, p);
+    c = std::pow(a, 2.0 * s);
+    delta = (m == 0.0) ? 0.0 : p * ctx->prm.dtau / tau;   // (1/2) alpha (dln a/dln tau) dtau/tau, alpha = 2
+    omega = delta * (1.0 - s);
+}
+
+extern "C" int u1u1_set_time(u1u1_ctx *ctx, double tau, double era_m, double s)
+{
+    if (!ctx) return U1U1_EINVAL;
+    if (!ctx->configured) return fail(ctx, U1U1_ESTATE, "set_time before configure/init_fields");
+    if (!(era_m >= 0 && era_m < 1) || !(tau > 0 || era_m == 0)) return fail(ctx, U1U1_EINVAL, "need 0 <= era_m < 1 and tau > 0");
+    double delta, omega;
+    scalars_at(ctx, tau, era_m, s, ctx->a, ctx->c, delta, omega);
+    ctx->cG = ctx->c;
+    ctx->tau_pos = tau;
+    return U1U1_OK;
+}
+
+extern "C" int u1u1_step(u1u1_ctx *ctx, int32_t n, double tau, double era_m, double s)
+{
+    if (!ctx) return U1U1_EINVAL;
+    if (!ctx->configured) return fail(ctx, U1U1_ESTATE, "step before configure/init_fields");
+    if (n < 0) return fail(ctx, U1U1_EINVAL, "n must be >= 0");
+    if (!(era_m >= 0 && era_m < 1)) return fail(ctx, U1U1_EINVAL, "era_m must satisfy 0 <= m < 1");
+    if (era_m != 0 && !(tau > 0)) return fail(ctx, U1U1_EINVAL, "tau must be positive in an expanding background");
+    const u1u1_params &P = ctx->prm;
+    const double dx = ctx->dx, dt = P.dtau, f = P.friction;
+    const bool tiled = P.kernel_variant == 0 && step_tiled_supports(ctx->N);
+    for (int k = 0; k < n; k++) {
+        const double tk = tau + k * dt;
+        double a, c, delta, omega;
+        scalars_at(ctx, tk, era_m, s, a, c, delta, omega);
+        const double lam = std::fmax(P.lambda1 * P.eta1 * P.eta1, P.lambda2 * P.eta2 * P.eta2) +
+                           2.0 * P.kappa * std::fmax(P.eta1 * P.eta1, P.eta2 * P.eta2);
+        if (dt * dt * (12.0 / (dx * dx) + lam * c) >= 4.0) {
+            char buf[160];
+            snprintf(buf, sizeof buf, "leapfrog unstable at tau=%g: dtau^2 (12/dx^2 + (lambda+2kappa) sigma^2 a^{2s}) >= 4 (a^{2s}=%g)", tk, c);
+            return fail(ctx, U1U1_EUNSTABLE, buf);
+        }
+        StepCoef q;
+        q.aS = (float)(f * (1.0 - delta) / (1.0 + delta));
+        q.bS = (float)(f * dt / (1.0 + delta));
+        q.aG = (float)(f * (1.0 - omega) / (1.0 + omega));
+        q.bG = (float)(f * dt / (1.0 + omega));
+        q.lamh1 = (float)(0.5 * P.lambda1 * c);
+        q.lamh2 = (float)(0.5 * P.lambda2 * c);
+        q.kap = (float)(P.kappa * c);
+        q.sig1sq = (float)(P.eta1 * P.eta1);
+        q.sig2sq = (float)(P.eta2 * P.eta2);
+        q.cur1 = (float)(2.0 * P.e1 * P.e1 * c / dx);
+        q.cur2 = (float)(2.0 * P.e2 * P.e2 * c / dx);
+        q.inv_dx2 = (float)(1.0 / (dx * dx));
+        q.inv_dx3 = (float)(1.0 / (dx * dx * dx));
+        q.dtau = (float)dt;
+        q.dtau_dx = (float)(dt * dx);
+        Lattice L{pos_buf(ctx, ctx->cur), pos_buf(ctx, ctx->cur ^ 1), mom_buf(ctx), ctx->V, ctx->N};
+        cudaError_t e = tiled ? launch_step_tiled(L, q, ctx->stream) : launch_step_ref(L, q, ctx->stream);
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "step kernel launch");
+        ctx->launches += 1;
+        ctx->cur ^= 1;
+        ctx->tau_pos = tk + dt;
+        // weights for the diagnostics of the state just produced
+        double a1, c1, d1, o1;
+        scalars_at(ctx, ctx->tau_pos, era_m, s, a1, c1, d1, o1);
+        ctx->a = a1;
+        ctx->c = c1;
+        ctx->cG = c * (1.0 + delta) / (1.0 + omega);
+        ctx->diag_valid = false;
+    }
+    return U1U1_OK;
+}
+
+static DiagCoef diag_coef(const u1u1_ctx *ctx)
+{
+    const u1u1_params &P = ctx->prm;
+    DiagCoef k;
+    k.c = ctx->c;
+    k.cG = ctx->cG;
+    k.inv_dx = 1.0 / ctx->dx;
+    k.inv_dx2 = 1.0 / (ctx->dx * ctx->dx);
+    k.e1 = P.e1; k.e2 = P.e2; k.lam1 = P.lambda1; k.lam2 = P.lambda2; k.kappa = P.kappa;
+    k.sig1sq = P.eta1 * P.eta1; k.sig2sq = P.eta2 * P.eta2;
+    return k;
+}
+
+static int fetch(u1u1_ctx *ctx, double *host, int n)
+{
+    cudaError_t e = cudaMemcpyAsync(host, result(ctx), n * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "result readback");
+    return U1U1_OK;
+}
+
+extern "C" int u1u1_gauss_violation(u1u1_ctx *ctx, double *out)
+{
+    if (!ctx || !out) return ctx ? fail(ctx, U1U1_EINVAL, "out is NULL") : U1U1_EINVAL;
+    if (!ctx->configured) return fail(ctx, U1U1_ESTATE, "gauss_violation before configure/init_fields");
+    cudaError_t e = launch_gauss(pos_buf(ctx, ctx->cur), mom_buf(ctx), ctx->V, ctx->N, diag_coef(ctx),
+                                 partials(ctx), result(ctx), ctx->stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "gauss kernel launch");
+    ctx->launches += 2;
+    double r[8];
+    if (int rc = fetch(ctx, r, 8)) return rc;
+    for (int s = 0; s < 2; s++) {
+        const double l2g = std::sqrt(r[3 * s]), l2r = std::sqrt(r[3 * s + 1]), l2d = std::sqrt(r[3 * s + 2]);
+        out[4 * s + 0] = l2g;
+        out[4 * s + 1] = l2r;
+        out[4 * s + 2] = r[6 + s];
+        out[4 * s + 3] = l2g / std::fmax(std::fmax(l2r, l2d), 1e-300);
+    }
+    return U1U1_OK;
+}
+
+extern "C" int u1u1_diagnostics(u1u1_ctx *ctx, double *out)
+{
+    if (!ctx || !out) return ctx ? fail(ctx, U1U1_EINVAL, "out is NULL") : U1U1_EINVAL;
+    if (!ctx->configured) return fail(ctx, U1U1_ESTATE, "diagnostics before configure/init_fields");
+    const size_t V = ctx->V;
+    uint8_t *codes = ctx->scratch, *cells = ctx->scratch + 6 * V;
+    double *res = result(ctx);
+    // result slots: [0..4] windings, [8..10] cells, [16..26] densities
+    cudaError_t e = launch_windings(pos_buf(ctx, ctx->cur), V, ctx->N, codes, cells, partials(ctx), res, ctx->stream);
+    if (e == cudaSuccess)
+        e = launch_densities(pos_buf(ctx, ctx->cur), mom_buf(ctx), V, ctx->N, diag_coef(ctx), partials(ctx),
+                             res + 16, ctx->stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "diagnostics kernel launch");
+    ctx->launches += 6;
+    double r[32];
+    if (int rc = fetch(ctx, r, 32)) return rc;
+    ctx->diag_valid = true;
+    memset(out, 0, U1U1_DIAG_LEN * sizeof(double));
+    const double dx = ctx->dx, vol = (double)V * dx * dx * dx;
+    out[U1U1_D_TAU] = ctx->tau_pos;
+    out[U1U1_D_A] = ctx->a;
+    out[U1U1_D_C] = ctx->c;
+    out[U1U1_D_SUMW_P] = r[0];
+    out[U1U1_D_SUMW_Q] = r[1];
+    out[U1U1_D_NEAR_P] = r[2];
+    out[U1U1_D_NEAR_Q] = r[3];
+    out[U1U1_D_MAXW] = r[4];
+    out[U1U1_D_CELLS_P] = r[8];
+    out[U1U1_D_CELLS_Q] = r[9];
+    out[U1U1_D_CELLS_PQ] = r[10];
+    for (int k = 0; k < 11; k++) out[U1U1_D_SUM_L + k] = r[16 + k];
+    // derived scalars, Eq. 31-37; L_pq = dx N_pq, L_p = dx sum|W^p| - L_pq (:188)
+    const double L_pq = dx * r[10], L_p = dx * r[0] - L_pq, L_q = dx * r[1] - L_pq, tot = L_pq + L_p + L_q;
+    const double inf = INFINITY;
+    out[U1U1_D_L_P] = L_p;
+    out[U1U1_D_L_Q] = L_q;
+    out[U1U1_D_L_PQ] = L_pq;
+    out[U1U1_D_XI_P] = L_p > 0 ? std::sqrt(vol / L_p) : inf;
+    out[U1U1_D_XI_Q] = L_q > 0 ? std::sqrt(vol / L_q) : inf;
+    out[U1U1_D_XI_PQ] = L_pq > 0 ? std::sqrt(vol / L_pq) : inf;
+    out[U1U1_D_XI_W] = tot > 0 ? std::sqrt(vol / tot) : inf;
+    const double mu = 2.0 * 3.14159265358979323846 * ctx->prm.eta1 * ctx->prm.eta1;
+    const double sumL = dx * dx * dx * r[16];
+    out[U1U1_D_XI_L] = sumL < 0 ? std::sqrt(-mu * vol / sumL) : NAN;
+    out[U1U1_D_F_TOTAL] = tot > 0 ? L_pq / tot : 0.0;
+    out[U1U1_D_F_P] = L_p > 0 ? L_pq / L_p : 0.0;
+    const double RL = r[18] != 0 ? r[17] / r[18] : NAN, RV = r[20] != 0 ? r[19] / r[20] : NAN;
+    out[U1U1_D_V2_L] = 2.0 * RL / (1.0 + RL);
+    out[U1U1_D_V2_PQ] = 2.0 * RV / (1.0 + RV);
+    out[U1U1_D_ENERGY] = dx * dx * dx * (r[22] + r[23] + r[24] + r[25] + r[26]);
+    return U1U1_OK;
+}
+
+static int relayout(u1u1_ctx *ctx, float *canon, int to_canonical)
+{
+    cudaError_t e = launch_relayout(pos_buf(ctx, ctx->cur), mom_buf(ctx), canon, ctx->V, to_canonical, ctx->stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "relayout kernel launch");
+    ctx->launches += 1;
+    if (!to_canonical) ctx->diag_valid = false;
+    return U1U1_OK;
+}
+
+extern "C" int u1u1_export_state(u1u1_ctx *ctx, void *dst_dev)
+{
+    if (!ctx || !dst_dev) return ctx ? fail(ctx, U1U1_EINVAL, "dst is NULL") : U1U1_EINVAL;
+    if (!ctx->configured) return fail(ctx, U1U1_ESTATE, "export_state before configure/init_fields");
+    return relayout(ctx, (float *)dst_dev, 1);
+}
+
+extern "C" int u1u1_import_state(u1u1_ctx *ctx, const void *src_dev)
+{
+    if (!ctx || !src_dev) return ctx ? fail(ctx, U1U1_EINVAL, "src is NULL") : U1U1_EINVAL;
+    if (!ctx->configured) return fail(ctx, U1U1_ESTATE, "import_state before configure");
+    return relayout(ctx, (float *)src_dev, 0);
+}
+
+extern "C" int u1u1_export_block(u1u1_ctx *ctx, int32_t x0, int32_t y0, int32_t z0, int32_t bx, int32_t by,
+                                 int32_t bz, void *dst_dev)
+{
+    if (!ctx || !dst_dev) return ctx ? fail(ctx, U1U1_EINVAL, "dst is NULL") : U1U1_EINVAL;
+    if (!ctx->configured) return fail(ctx, U1U1_ESTATE, "export_block before configure/init_fields");
+    if (bx < 1 || by < 1 || bz < 1 || bx > ctx->N || by > ctx->N || bz > ctx->N)
+        return fail(ctx, U1U1_EINVAL, "block extents must lie in [1, N]");
+    cudaError_t e = launch_export_block(pos_buf(ctx, ctx->cur), mom_buf(ctx), ctx->V, ctx->N, x0, y0, z0, bx, by,
+                                        bz, (float *)dst_dev, ctx->stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "export_block launch");
+    ctx->launches += 1;
+    return U1U1_OK;
+}
+
+// Host variants: plane-by-plane cudaMemcpyAsync between the canonical host array and the internal
+// planes (no staging buffer needed: every canonical component is one contiguous internal plane).
+static int host_copy(u1u1_ctx *ctx, void *host, int to_host)
+{
+    const size_t V = ctx->V, bytes = V * sizeof(float);
+    for (int c = 0; c < 20; c++) {
+        int is_mom, plane;
+        canonical_to_internal(c, is_mom, plane);
+        float *dev = (is_mom ? mom_buf(ctx) : pos_buf(ctx, ctx->cur)) + (size_t)plane * V;
+        float *h = (float *)host + (size_t)c * V;
+        cudaError_t e = to_host ? cudaMemcpyAsync(h, dev, bytes, cudaMemcpyDeviceToHost, ctx->stream)
+                                : cudaMemcpyAsync(dev, h, bytes, cudaMemcpyHostToDevice, ctx->stream);
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "host<->device state copy");
+    }
+    cudaError_t e = cudaStreamSynchronize(ctx->stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "host<->device state copy (sync)");
+    if (!to_host) ctx->diag_valid = false;
+    return U1U1_OK;
+}
+
+extern "C" int u1u1_export_state_host(u1u1_ctx *ctx, void *dst_host)
+{
+    if (!ctx || !dst_host) return ctx ? fail(ctx, U1U1_EINVAL, "dst is NULL") : U1U1_EINVAL;
+    if (!ctx->configured) return fail(ctx, U1U1_ESTATE, "export_state_host before configure/init_fields");
+    return host_copy(ctx, dst_host, 1);
+}
+
+extern "C" int u1u1_import_state_host(u1u1_ctx *ctx, const void *src_host)
+{
+    if (!ctx || !src_host) return ctx ? fail(ctx, U1U1_EINVAL, "src is NULL") : U1U1_EINVAL;
+    if (!ctx->configured) return fail(ctx, U1U1_ESTATE, "import_state_host before configure");
+    return host_copy(ctx, const_cast<void *>(src_host), 0);
+}
+
+extern "C" int u1u1_export_windings(u1u1_ctx *ctx, int32_t sector, void *w_dev, void *near_dev, void *cells_dev)
+{
+    if (!ctx) return U1U1_EINVAL;
+    if (sector != 0 && sector != 1) return fail(ctx, U1U1_EINVAL, "sector must be 0 or 1");
+    if (!ctx->diag_valid) return fail(ctx, U1U1_ESTATE, "export_windings needs u1u1_diagnostics on the current state first");
+    const size_t V = ctx->V;
+    if (w_dev || near_dev) {
+        cudaError_t e = launch_decode_windings(ctx->scratch + (size_t)3 * sector * V, 3 * V, (int8_t *)w_dev,
+                                               (uint8_t *)near_dev, ctx->stream);
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "decode_windings launch");
+        ctx->launches += 1;
+    }
+    if (cells_dev) {
+        cudaError_t e = cudaMemcpyAsync(cells_dev, ctx->scratch + 6 * V + (size_t)sector * V, V,
+                                        cudaMemcpyDeviceToDevice, ctx->stream);
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "cells copy");
+    }
+    return U1U1_OK;
+}

@@ -1,0 +1,107 @@
+// common.cuh -- internal layout, per-step coefficients and reduction helpers shared by the CUDA
+// kernels of libu1u1.so.  Nothing here is shared with oracle/ (separate code base by design).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace u1u1 {
+
+// ------------------------------------------------------------------------------------------------
+// Internal HBM layout: structure of arrays, each plane [z][y][x], x fastest.
+//   pos[b]  b = 0,1 (ping-pong): 10 planes  0 phi_re 1 phi_im 2 psi_re 3 psi_im 4..6 thetaA 7..9 thetaB
+//   mom             : 10 planes  0 Pi_re 1 Pi_im 2 Psi_re 3 Psi_im 4..6 E 7..9 H
+// state buffer = [pos0 | pos1 | mom], 30 N^3 floats.
+// ------------------------------------------------------------------------------------------------
+constexpr int NPOS = 10;
+constexpr int NMOM = 10;
+
+struct Lattice {
+    const float *pos_in;  // positions at tau (read)
+    float *pos_out;       // positions at tau + dtau (written)
+    float *mom;           // momenta, updated in place
+    size_t V;             // N^3
+    int N;
+};
+
+// canonical component -> (is_momentum, internal plane)
+__host__ __device__ inline void canonical_to_internal(int c, int &is_mom, int &plane)
+{
+    // canonical: 0 phi_re 1 phi_im 2 Pi_re 3 Pi_im 4 psi_re 5 psi_im 6 Psi_re 7 Psi_im
+    //            8..10 thetaA 11..13 E 14..16 thetaB 17..19 H
+    if (c < 8) {
+        is_mom = (c >> 1) & 1;
+        plane = (c >> 2) * 2 + (c & 1);
+    } else if (c < 14) {
+        is_mom = c >= 11;
+        plane = 4 + (c - (is_mom ? 11 : 8));
+    } else {
+        is_mom = c >= 17;
+        plane = 7 + (c - (is_mom ? 17 : 14));
+    }
+}
+
+// Per-step coefficients, computed on the host in fp64 (PAPER.md:133 Eq. 19, :147 Eq. 22, :89 Eq. 12)
+// and rounded once to fp32.  Friction (BASELINE.json prephase) is folded into the four kick factors.
+struct StepCoef {
+    float aS, bS;          // Pi+  = aS Pi-  + bS [lap - c phi (...)],  aS = f(1-delta)/(1+delta), bS = f dtau/(1+delta)
+    float aG, bG;          // E+   = aG E-   + bG [-curl + current],    aG = f(1-omega)/(1+omega), bG = f dtau/(1+omega)
+    float lamh1, lamh2;    // c lambda_p0/2, c lambda_q0/2
+    float kap;             // c kappa_0
+    float sig1sq, sig2sq;  // sigma_p^2, sigma_q^2
+    float cur1, cur2;      // 2 e_p0^2 c / dx, 2 e_q0^2 c / dx
+    float inv_dx2;         // 1/dx^2
+    float inv_dx3;         // 1/dx^3
+    float dtau;            // drift of the scalars
+    float dtau_dx;         // drift of the link phases: theta += dtau dx E
+};
+
+// Coefficients of the diagnostic sweeps.
+struct DiagCoef {
+    double c;              // a^{2s}
+    double cG;             // Gauss-law coefficient c (1+delta)/(1+omega) of the last step
+    double inv_dx;
+    double inv_dx2;
+    double e1, e2, lam1, lam2, kappa, sig1sq, sig2sq;
+};
+
+// ------------------------------------------------------------------------------------------------
+// Deterministic two-stage reductions: every block writes NRED doubles of partial sums (and maxima),
+// a one-block kernel folds the partials.  No atomics, so results are bit-reproducible run to run.
+// ------------------------------------------------------------------------------------------------
+constexpr int RED_BLOCK = 256;
+constexpr int RED_MAX_BLOCKS = 148 * 8;
+constexpr int RED_SLOTS = 32;
+
+__device__ inline double warp_sum(double v)
+{
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    return v;
+}
+__device__ inline double warp_max(double v)
+{
+    for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_down_sync(0xffffffffu, v, o));
+    return v;
+}
+
+// Reduce `n` per-thread values (first n_sum are summed, the rest are maxima) over the block and
+// store them at out[blockIdx.x * RED_SLOTS + k].
+template <int NVAL>
+__device__ inline void block_reduce_store(const double (&v)[NVAL], int n_sum, double *out)
+{
+    __shared__ double sm[NVAL][RED_BLOCK / 32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int k = 0; k < NVAL; k++) {
+        double r = (k < n_sum) ? warp_sum(v[k]) : warp_max(v[k]);
+        if (lane == 0) sm[k][warp] = r;
+    }
+    __syncthreads();
+    if (threadIdx.x < NVAL) {
+        const int k = threadIdx.x;
+        double r = sm[k][0];
+        for (int w = 1; w < RED_BLOCK / 32; w++) r = (k < n_sum) ? r + sm[k][w] : fmax(r, sm[k][w]);
+        out[(size_t)blockIdx.x * RED_SLOTS + k] = r;
+    }
+}
+
+}  // namespace u1u1

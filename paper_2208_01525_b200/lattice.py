@@ -1,0 +1,115 @@
+"""`Lattice`: owns the device buffers (torch tensors) and a context of libu1u1.so; its methods are the
+C-ABI calls of include/u1u1.h under the same names (init_fields, step, diagnostics, gauss_violation,
+...).  Argument marshalling only -- all arithmetic happens in the CUDA kernels."""
+from __future__ import annotations
+
+import ctypes
+
+import numpy as np
+
+from . import binding as B
+
+
+class Lattice:
+    def __init__(self, N: int, device: str = "cuda:0", stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise B.U1U1Error("CUDA device required: libu1u1 has no CPU fallback")
+        self._torch = torch
+        self.lib = B.load()
+        self.N = int(N)
+        self.device = torch.device(device)
+        sb, cb = B.state_bytes(self.N), B.scratch_bytes(self.N)
+        if sb == 0:
+            raise B.U1U1Error(f"unsupported lattice size N={N}")
+        with torch.cuda.device(self.device):
+            self.state = torch.empty(sb, dtype=torch.uint8, device=self.device)
+            self.scratch = torch.empty(cb, dtype=torch.uint8, device=self.device)
+            self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        self._ctx = ctypes.c_void_p()
+        rc = self.lib.u1u1_create(ctypes.byref(self._ctx), self.state.data_ptr(), sb,
+                                  self.scratch.data_ptr(), cb, self.stream.cuda_stream)
+        if rc:
+            raise B.U1U1Error(f"u1u1_create: {self.lib.u1u1_last_error(None).decode()}")
+
+    # -- helpers ---------------------------------------------------------------------------------
+    def _check(self, rc, what):
+        if rc:
+            msg = self.lib.u1u1_last_error(self._ctx).decode()
+            raise B.U1U1Error(f"{what}: {B.ERRORS.get(rc, rc)}: {msg}")
+
+    def close(self):
+        if self._ctx:
+            self.lib.u1u1_destroy(self._ctx)
+            self._ctx = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- the C ABI, same names ---------------------------------------------------------------------
+    def configure(self, dx: float, params: B.Params):
+        self._check(self.lib.u1u1_configure(self._ctx, self.N, dx, ctypes.byref(params)), "configure")
+
+    def init_fields(self, seed: int, dx: float, params: B.Params):
+        self._check(self.lib.u1u1_init_fields(self._ctx, seed, self.N, dx, ctypes.byref(params)), "init_fields")
+
+    def set_params(self, params: B.Params):
+        self._check(self.lib.u1u1_set_params(self._ctx, ctypes.byref(params)), "set_params")
+
+    def set_time(self, tau: float, era_m: float, s: float):
+        self._check(self.lib.u1u1_set_time(self._ctx, tau, era_m, s), "set_time")
+
+    def step(self, n: int, tau: float, era_m: float, s: float):
+        self._check(self.lib.u1u1_step(self._ctx, n, tau, era_m, s), "step")
+
+    def diagnostics(self) -> dict:
+        out = (ctypes.c_double * B.DIAG_LEN)()
+        self._check(self.lib.u1u1_diagnostics(self._ctx, out), "diagnostics")
+        return {k: out[i] for i, k in enumerate(B.DIAG_SLOTS)}
+
+    def gauss_violation(self) -> np.ndarray:
+        out = (ctypes.c_double * B.GAUSS_LEN)()
+        self._check(self.lib.u1u1_gauss_violation(self._ctx, out), "gauss_violation")
+        return np.array(out[:])
+
+    def export_state(self):
+        """Canonical float32 [20, N, N, N] torch tensor on the device."""
+        t = self._torch.empty((20, self.N, self.N, self.N), dtype=self._torch.float32, device=self.device)
+        self._check(self.lib.u1u1_export_state(self._ctx, t.data_ptr()), "export_state")
+        return t
+
+    def import_state(self, t):
+        torch = self._torch
+        t = t.to(device=self.device, dtype=torch.float32).contiguous()
+        assert tuple(t.shape) == (20, self.N, self.N, self.N), t.shape
+        self._check(self.lib.u1u1_import_state(self._ctx, t.data_ptr()), "import_state")
+        self.stream.synchronize()   # `t` may be a temporary
+
+    def export_state_host(self, host_tensor):
+        self._check(self.lib.u1u1_export_state_host(self._ctx, host_tensor.data_ptr()), "export_state_host")
+
+    def import_state_host(self, host_tensor):
+        self._check(self.lib.u1u1_import_state_host(self._ctx, host_tensor.data_ptr()), "import_state_host")
+
+    def export_windings(self, sector: int):
+        """(W int8 [3,N,N,N], near uint8 [3,N,N,N], cells uint8 [N,N,N]) after diagnostics()."""
+        torch, N = self._torch, self.N
+        W = torch.empty((3, N, N, N), dtype=torch.int8, device=self.device)
+        near = torch.empty((3, N, N, N), dtype=torch.uint8, device=self.device)
+        cells = torch.empty((N, N, N), dtype=torch.uint8, device=self.device)
+        self._check(self.lib.u1u1_export_windings(self._ctx, sector, W.data_ptr(), near.data_ptr(),
+                                                  cells.data_ptr()), "export_windings")
+        self.stream.synchronize()
+        return W, near, cells
+
+    def export_block(self, x0, y0, z0, bx, by, bz):
+        t = self._torch.empty((20, bz, by, bx), dtype=self._torch.float32, device=self.device)
+        self._check(self.lib.u1u1_export_block(self._ctx, x0, y0, z0, bx, by, bz, t.data_ptr()), "export_block")
+        self.stream.synchronize()
+        return t
+
+    def launch_count(self) -> int:
+        return int(self.lib.u1u1_launch_count(self._ctx))
