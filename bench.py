@@ -1,0 +1,305 @@
+#!/usr/bin/env python
+"""bench.py -- site-updates/s of the fused U(1)xU(1) leapfrog step on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--size 1024] [--impl ours|reference]
+
+Workload (config.workload): BASELINE.json config 5 -- 1024^3 periodic lattice, dx=0.5, dtau=0.1,
+radiation era, s=1, lambda=2, e=1, eta=1, kappa=0.9, seeded uniform random-phase init, damped
+prephase (friction 0.5), full diagnostics every 100 steps.  A "step" is one fused kick+drift launch
+(SURVEY.md 8(a) rows a1-a5); the diagnostic sweeps (a6-a10) run inside the timed region at the
+config's cadence (after every 100th timed step).  Inputs (the 129 GB state) are far larger than L2.
+
+One JSON line on stdout (rank 0).  N > 1: replicas only (independent seeds per GPU, no collective on the
+data path), launched by torchrun, timed as the max over ranks.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "lattice site-updates/sec (full 2-field step)"
+UNIT = "site-updates/s"
+BYTES_PER_SITE_UPDATE = 160          # read 20 + write 20 fp32 words
+DX, DTAU, TAU0, ERA, S = 0.5, 0.1, 1.0, 0.5, 1.0
+DIAG_EVERY = 100
+PREPHASE_STEPS = 200                 # 20 tau units of friction 0.5 (config 5)
+
+
+def workload_name(n):
+    return (f"{n}^3 periodic, dx=0.5, dtau=0.1, fp32, radiation era, s=1, lambda=2, e=1, eta=1, kappa=0.9, "
+            f"uniform random-phase init (seed 5+rank), friction-0.5 prephase, diagnostics every {DIAG_EVERY} steps "
+            "(BASELINE.json config 5)")
+
+
+def measured_peak_gbs():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms during the timed region."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.path = tempfile.mktemp(prefix="u1u1_clocks_", suffix=".csv")
+        self.proc = None
+        self.gpu = gpu_index
+
+    def start(self):
+        try:
+            self.f = open(self.path, "w")
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.gpu), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=self.f, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.proc is None:
+            return out
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        self.f.close()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in open(self.path):
+            p = [t.strip() for t in line.split(",")]
+            if len(p) < 9:
+                continue
+            try:
+                sm.append(float(p[1])); mx.append(float(p[2]))
+            except ValueError:
+                continue
+            for name, v in zip(names, p[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        try:
+            os.unlink(self.path)
+        except OSError:
+            pass
+        if sm:
+            out.update(sm_mhz=statistics.median(sm), sm_max_mhz=max(mx), reasons=sorted(reasons), samples=len(sm))
+        return out
+
+
+def oracle_sample(n, steps, seed=5):
+    """The oracle as it stands on an n^3 sample of the same workload; returns (site-updates/s, cores)."""
+    from oracle import oracle as O
+    s = O.init_random_phase(n, seed)
+    K = O.Couplings()
+    O.step(s, DX, K, TAU0, ERA, S, DTAU, tau_norm=256.0, friction=0.5, n=1)          # warm caches / page in
+    t0 = time.perf_counter()
+    O.step(s, DX, K, TAU0 + DTAU, ERA, S, DTAU, tau_norm=256.0, friction=0.5, n=steps)
+    dt = time.perf_counter() - t0
+    cores = int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
+    return n ** 3 * steps / dt, cores, dt
+
+
+def run_reference(args):
+    """--impl reference: the fp64 oracle on host cores (rank 0 only), bounded sample per step."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    n = 128
+    from oracle import oracle as O
+    s = O.init_random_phase(n, 5)
+    K = O.Couplings()
+    for k in range(args.warmup):
+        O.step(s, DX, K, TAU0 + k * DTAU, ERA, S, DTAU, tau_norm=256.0, friction=0.5)
+    t0 = time.perf_counter()
+    for k in range(args.steps):
+        O.step(s, DX, K, TAU0 + (args.warmup + k) * DTAU, ERA, S, DTAU, tau_norm=256.0, friction=0.5)
+    dt = time.perf_counter() - t0
+    value = n ** 3 * args.steps / dt
+    cores = int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
+    sample = f"{n}^3 sub-lattice of the workload per step (oracle fp64, gcc -O2, OpenMP over z-planes of the kick loops)"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_name(args.size), "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+def run_ours(args):
+    import torch
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: CUDA device required (the library has no CPU fallback)")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+
+    from paper_2208_01525_b200 import Lattice, Params, build
+    build.build()
+    N = args.size
+    V = N ** 3
+    lat = Lattice(N, device=f"cuda:{local}")
+    prm = Params(tau_norm=256.0, friction=0.5, kernel_variant=args.variant)
+    lat.init_fields(5 + rank, DX, prm)
+    lat.step(args.prephase, TAU0, ERA, S)                    # damped prephase (shortened; --prephase 200 = config 5)
+    prm.friction = 1.0
+    lat.set_params(prm)
+    tau = TAU0 + args.prephase * DTAU
+    lat.step(args.warmup, tau, ERA, S)                       # W >= 3 untimed warm-up steps
+    tau += args.warmup * DTAU
+    lat.gauss_violation(); lat.diagnostics()                 # warm the diagnostic kernels too
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    clocks = ClockSampler(local)
+    launches0 = lat.launch_count()
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    t_start, t_end, segs = ev(), ev(), []
+    barrier()
+    clocks.start()
+    t_start.record()
+    done, ndiag, diag, gauss = 0, 0, None, None
+    while done < args.steps:
+        n = min(DIAG_EVERY - (done % DIAG_EVERY), args.steps - done)
+        e0, e1 = ev(), ev()
+        e0.record(); lat.step(n, tau, ERA, S); e1.record()
+        segs.append((e0, e1))
+        tau += n * DTAU
+        done += n
+        if done % DIAG_EVERY == 0:
+            gauss = lat.gauss_violation(); diag = lat.diagnostics(); ndiag += 1
+    t_end.record()
+    barrier()
+    clk = clocks.stop()
+    launches = lat.launch_count() - launches0
+    ms_total = t_start.elapsed_time(t_end)
+    ms_steps = sum(a.elapsed_time(b) for a, b in segs)
+    if dist is not None:
+        t = torch.tensor([ms_total, ms_steps], device=f"cuda:{local}", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total, ms_steps = t.tolist()
+    value = world * args.steps * V / (ms_total * 1e-3)
+    kernel_ms = ms_steps / args.steps
+    achieved = BYTES_PER_SITE_UPDATE * V / (kernel_ms * 1e-3) / 1e9
+    peak, peak_src = measured_peak_gbs()
+    if gauss is None:
+        gauss = lat.gauss_violation(); diag = lat.diagnostics()        # untimed: for the report only
+
+    e2e = run_e2e(args, lat, tau, world, dist, local)
+
+    if rank != 0:
+        return
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        n_s, steps_s = 192, 3
+        v, cores, dt = oracle_sample(n_s, steps_s)
+        cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "sample": f"{n_s}^3 sub-lattice of the workload, {steps_s} steps ({dt:.1f} s), fp64 oracle as it stands"}
+    traffic = None
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            traffic = json.load(f).get(f"step_{N}")
+    except Exception:
+        pass
+    print(json.dumps({
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_total / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": workload_name(N), "N": N, "state_GB": 120 * V / 1e9,
+                   "l2_policy": "inputs (129 GB state) far larger than the 126 MB L2; no flush needed",
+                   "prephase_steps_before_timing": args.prephase, "diag_calls_in_timed_region": ndiag,
+                   "kernel_variant": args.variant, "parallelism": "replicas" if world > 1 else "single"},
+        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                     "traffic": traffic, "peak_source": peak_src, "kernel": "fused kick+drift step",
+                     "kernel_ms": kernel_ms, "bytes_per_site_update": BYTES_PER_SITE_UPDATE,
+                     "frac_of_8TBs_spec": achieved / 8000.0},
+        "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clk,
+        "diagnostics": {"tau": diag["tau"], "xi_W": diag["xi_W"], "xi_L": diag["xi_L"], "v2_L": diag["v2_L"],
+                        "f_total": diag["f_total"], "maxW": diag["maxW"],
+                        "gauss_rel_p": float(gauss[3]), "gauss_rel_q": float(gauss[7])},
+    }))
+
+
+def run_e2e(args, lat, tau, world, dist, local):
+    """Same metric through the C ABI with HOST buffers: import_state_host (H2D of the 80 B/site state from
+    pinned memory) -> K steps -> diagnostics + gauss (D2H scalars) -> export_state_host (D2H), all timed."""
+    import torch
+    V = args.size ** 3
+    nbytes = 80 * V
+    try:
+        import psutil
+        avail = psutil.virtual_memory().available
+    except Exception:
+        avail = 0
+    if args.no_e2e or avail < 1.4 * nbytes * max(1, world):
+        return {"value": None, "unit": UNIT, "h2d_bytes_per_step": None, "d2h_bytes_per_step": None,
+                "note": f"skipped: needs {nbytes / 1e9:.0f} GB pinned host memory per rank, {avail / 1e9:.0f} GB available"}
+    host = torch.empty(20 * V, dtype=torch.float32, pin_memory=True)
+    lat.export_state_host(host)                              # untimed: a valid checkpoint in host memory
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t0.record()
+    lat.import_state_host(host)
+    lat.step(args.steps, tau, ERA, S)
+    lat.gauss_violation(); lat.diagnostics()
+    lat.export_state_host(host)
+    t1.record()
+    torch.cuda.synchronize()
+    ms = t0.elapsed_time(t1)
+    if dist is not None:
+        t = torch.tensor([ms], device=f"cuda:{local}", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = t.item()
+    del host
+    return {"value": world * args.steps * V / (ms * 1e-3), "unit": UNIT,
+            "h2d_bytes_per_step": nbytes / args.steps, "d2h_bytes_per_step": (nbytes + 8 * 56) / args.steps,
+            "ms_total": ms, "note": "checkpoint in pinned host memory -> H2D -> K steps -> diagnostics -> D2H"}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--size", type=int, default=1024)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--prephase", type=int, default=20)
+    ap.add_argument("--variant", type=int, default=0)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

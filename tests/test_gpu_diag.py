@@ -1,0 +1,148 @@
+"""GPU parity of the IC generator, the Gauss monitor and the diagnostics (windings, cells, sums) against
+the oracle, from the SAME fp32 snapshot.  Integer work must match bit-exactly, except plaquettes flagged
+near the branch cut by either side (north_star; reading R-15), which are counted."""
+import numpy as np
+import pytest
+
+import inputs
+from oracle import oracle as O
+
+pytestmark = pytest.mark.gpu
+DX, DTAU = 0.5, 0.1
+
+
+def evolved_snapshot(N, seed, nsteps, m=0.5, s=1.0, tau_norm=1.0, kind=0, friction=1.0):
+    """Run the GPU from a seeded init and return (lattice, canonical fp64 snapshot of its state)."""
+    from paper_2208_01525_b200 import Lattice, Params
+    lat = Lattice(N)
+    prm = Params(init_kind=kind, tau_norm=tau_norm, friction=friction, smooth_width=2.0, smooth_trunc=8)
+    lat.init_fields(seed, DX, prm)
+    lat.step(nsteps, 1.0, m, s)
+    snap = lat.export_state().cpu().numpy().astype(np.float64)
+    return lat, snap
+
+
+def test_init_random_phase_matches_oracle():
+    from paper_2208_01525_b200 import Lattice, Params
+    N = 32
+    lat = Lattice(N)
+    lat.init_fields(7, DX, Params(eta2=1.25))
+    gpu = lat.export_state().cpu().numpy().astype(np.float64)
+    ref = O.init_random_phase(N, 7, O.Couplings(eta2=1.25))
+    # fp64 phase evaluation rounded once to fp32 on the GPU: half an ulp of values <= 1.25
+    assert np.max(np.abs(gpu - ref)) <= 2.0 ** -24 * 1.25 * 1.01
+    assert not gpu[inputs.MOM].any() and not gpu[[8, 9, 10, 14, 15, 16]].any()
+    # a different seed gives a different field; the same seed the same bits
+    lat.init_fields(8, DX, Params(eta2=1.25))
+    assert np.max(np.abs(lat.export_state().cpu().numpy() - gpu)) > 0.5
+    lat.init_fields(7, DX, Params(eta2=1.25))
+    assert np.array_equal(lat.export_state().cpu().numpy().astype(np.float64), gpu)
+
+
+def test_init_smoothed_matches_oracle():
+    from paper_2208_01525_b200 import Lattice, Params
+    N = 32
+    lat = Lattice(N)
+    lat.init_fields(3, DX, Params(init_kind=1, smooth_width=2.0, smooth_trunc=8))
+    gpu = lat.export_state().cpu().numpy().astype(np.float64)
+    ref = O.init_smoothed(N, 3, width=2.0, trunc=8)
+    # fp32 intermediates: phase error ~ 1e-6 / |smoothed noise|; bound it by the conditioning
+    assert np.max(np.abs(gpu - ref)) < 2e-4
+    assert np.median(np.abs(gpu - ref)[[0, 1, 4, 5]]) < 2e-7
+    assert not gpu[inputs.MOM].any()
+
+
+@pytest.mark.parametrize("m,s,f", [(0.5, 1.0, 1.0), (2 / 3, 0.0, 1.0), (0.5, -1.0, 0.5)])
+def test_gauss_monitor_matches_oracle(m, s, f):
+    N = 32
+    lat, snap = evolved_snapshot(N, 11, 12, m=m, s=s, friction=f)
+    g = lat.gauss_violation()
+    cG = O.gauss_coefficient(1.0 + 11 * DTAU, m, s, DTAU, 1.0)
+    ref = O.gauss_violation(snap, DX, O.Couplings(), cG)
+    # rho norms agree to fp64-accumulation accuracy; g itself is a roundoff residue of the fp32 run
+    # (or the scheme's own eps^3 injection for (rad, s=-1), G-notes), evaluated from the same snapshot
+    assert np.allclose(g[[1, 5]], ref[[1, 5]], rtol=1e-10)
+    assert np.allclose(g[[0, 4]], ref[[0, 4]], rtol=1e-6, atol=1e-12)
+    assert np.allclose(g[[2, 6]], ref[[2, 6]], rtol=1e-6, atol=1e-12)
+    assert np.allclose(g[[3, 7]], ref[[3, 7]], rtol=1e-6, atol=1e-14)
+
+
+def test_gauss_monitor_on_generic_state():
+    """A state that violates Gauss at O(1): every term of g is exercised with large values."""
+    from paper_2208_01525_b200 import Lattice, Params
+    import torch
+    N = 24
+    s0 = inputs.to_f32_exact(inputs.random_state((N, N, N), seed=2))
+    lat = Lattice(N)
+    prm = Params(e1=1.1, e2=0.7, tau_norm=2.0)
+    lat.configure(DX, prm)
+    lat.import_state(torch.from_numpy(s0.astype(np.float32)))
+    lat.set_time(3.0, 0.5, 1.0)
+    g = lat.gauss_violation()
+    ref = O.gauss_violation(s0, DX, O.Couplings(e1=1.1, e2=0.7), 1.5 ** 2)
+    assert np.allclose(g, ref, rtol=1e-10)
+
+
+@pytest.mark.parametrize("N,nsteps,kind", [(48, 40, 0), (32, 25, 1), (64, 32, 0)])
+def test_diagnostics_match_oracle(N, nsteps, kind):
+    lat, snap = evolved_snapshot(N, 21 + N, nsteps, kind=kind)
+    d = lat.diagnostics()
+    _, c, _, _ = O.scalars(1.0 + nsteps * DTAU, 0.5, 1.0, DTAU, 1.0)
+    ref = O.diagnostics(snap, DX, O.Couplings(), c)
+    assert np.isclose(d["tau"], 1.0 + nsteps * DTAU) and np.isclose(d["c"], c)
+    tot_near = 0
+    cells_gpu = []
+    for sec, tag in ((0, "p"), (1, "q")):
+        W, near, cells = (t.cpu().numpy() for t in lat.export_windings(sec))
+        Wr, near_r = O.windings(snap, DX, sec)
+        excl = (near > 0) | (near_r > 0)
+        assert np.array_equal(W[~excl], Wr[~excl].astype(np.int8))          # bit-exact off the cut
+        assert np.sum(W != Wr) <= np.sum(excl)
+        tot_near += int(np.sum(excl))
+        assert d[f"sumW_{tag}"] == np.sum(np.abs(W.astype(np.int64)))          # counters agree with arrays
+        assert d[f"near_{tag}"] == np.sum(near)
+        # cells from the GPU's own windings through the oracle's cell rule: bit-exact
+        assert np.array_equal(cells.astype(np.int32), O.cells(W.astype(np.int32)))
+        assert d[f"cells_{tag}"] == np.sum(cells > 0)
+        cells_gpu.append(cells)
+        if not excl.any():
+            assert d[f"sumW_{tag}"] == ref[f"sumW_{tag}"] and d[f"cells_{tag}"] == ref[f"cells_{tag}"]
+        assert d[f"sumW_{tag}"] > 0                                            # there are strings
+    assert d["cells_pq"] == np.sum((cells_gpu[0] > 0) & (cells_gpu[1] > 0))
+    if tot_near == 0:
+        assert d["cells_pq"] == ref["cells_pq"]
+    assert d["maxW"] == max(ref["maxW_p"], ref["maxW_q"]) or tot_near > 0
+    # floating-point sums: fp32 per-site terms, fp64 accumulation.  Scale = sum of |terms|.
+    scale = ref["sum_kin"] + ref["sum_grad"] + ref["sum_elec"] + ref["sum_mag"] + abs(ref["sum_pot"])
+    for k in ("sum_kin", "sum_grad", "sum_elec", "sum_mag", "sum_pot", "sum_vint", "sum_L"):
+        assert abs(d[k] - ref[k]) < 2e-6 * scale, (k, d[k], ref[k])
+    for k in ("sum_kin_L", "sum_grad_L", "sum_kin_V", "sum_grad_V"):
+        assert abs(d[k] - ref[k]) < 1e-5 * max(abs(ref["sum_kin_L"]), abs(ref["sum_grad_L"])), (k, d[k], ref[k])
+    assert ref["sum_pot"] >= 0 and np.isclose(d["energy"], DX ** 3 * scale, rtol=1e-5)
+    if tot_near == 0:
+        for k in ("L_p", "L_q", "L_pq", "xi_p", "xi_q", "xi_W", "f_total", "f_p"):
+            assert np.isclose(d[k], ref[k], rtol=1e-12), k
+    for k in ("xi_L", "v2_L", "v2_pq"):
+        assert np.isclose(d[k], ref[k], rtol=1e-4), (k, d[k], ref[k])
+
+
+def test_known_vortex_lines_on_gpu():
+    """Hand-built straight p and q lines: exact counts, cell value 2, N_pq = line length."""
+    from paper_2208_01525_b200 import Lattice, Params
+    import torch
+    N = 16
+    shape = (N, N, N)
+    lines = [((3.5, 7.5), +1), ((11.5, 7.5), -1)]
+    ph = inputs.vortex_pair_phase(shape, [c for c, _ in lines], [q for _, q in lines])
+    s0 = np.zeros((20,) + shape)
+    s0[0], s0[1] = np.cos(ph), np.sin(ph)
+    s0[4], s0[5] = np.cos(ph), np.sin(ph)
+    lat = Lattice(N)
+    lat.configure(1.0, Params())
+    lat.import_state(torch.from_numpy(s0.astype(np.float32)))
+    d = lat.diagnostics()
+    assert d["sumW_p"] == 2 * N and d["sumW_q"] == 2 * N and d["cells_pq"] == 2 * N and d["maxW"] == 1
+    assert d["L_pq"] == 2.0 * N and d["L_p"] == 0.0 and d["f_total"] == 1.0
+    W, near, cells = lat.export_windings(0)
+    assert int(cells.max()) == 2 and int((cells == 2).sum()) == 2 * N
+    assert bool((W[0, :, 7, 3] == 1).all()) and bool((W[0, :, 7, 11] == -1).all())

@@ -1,0 +1,128 @@
+"""GPU parity of the fused leapfrog step (through the C ABI) against the fp64 oracle, element by element
+on identical (fp32-representable) seeded inputs.  Tolerances are north_star's: max relative error per
+field group (max|gpu-oracle| / max|oracle|, reading R-16) 1e-5 after 1 step, 1e-3 after 32."""
+import numpy as np
+import pytest
+
+import inputs
+from oracle import oracle as O
+
+pytestmark = pytest.mark.gpu
+
+DX, DTAU = 0.5, 0.1
+VARIANTS = [0, 1]          # 0 = default (tiled when supported), 1 = reference kernel
+
+
+def _torch():
+    import torch
+    return torch
+
+
+def group_errors(gpu, ref):
+    out = {}
+    for name, comps in inputs.GROUPS.items():
+        den = np.max(np.abs(ref[comps]))
+        num = np.max(np.abs(gpu[comps] - ref[comps]))
+        out[name] = num / den if den > 0 else num
+    return out
+
+
+def run_gpu(state64, N, params, calls):
+    """calls = [(n, tau, m, s), ...]; returns canonical float64 numpy state."""
+    from paper_2208_01525_b200 import Lattice
+    torch = _torch()
+    lat = Lattice(N)
+    lat.configure(DX, params)
+    lat.import_state(torch.from_numpy(state64.astype(np.float32)))
+    for (n, tau, m, s) in calls:
+        lat.step(n, tau, m, s)
+    out = lat.export_state().cpu().numpy().astype(np.float64)
+    return out, lat
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_config1_one_and_32_steps(variant):
+    """BASELINE.json config 1: 64^3, radiation, s=1, tau0=1, seeded uniform random phases."""
+    from paper_2208_01525_b200 import Params
+    N = 64
+    s0 = inputs.to_f32_exact(O.init_random_phase(N, seed=1))
+    K = O.Couplings()
+    prm = Params(kernel_variant=variant)
+    ref = s0.copy()
+    O.step(ref, DX, K, 1.0, 0.5, 1.0, DTAU, tau_norm=1.0, n=1)
+    gpu, _ = run_gpu(s0, N, prm, [(1, 1.0, 0.5, 1.0)])
+    err1 = group_errors(gpu, ref)
+    assert max(err1.values()) < 1e-5, err1
+    O.step(ref, DX, K, 1.0 + DTAU, 0.5, 1.0, DTAU, tau_norm=1.0, n=31)
+    gpu, lat = run_gpu(s0, N, prm, [(32, 1.0, 0.5, 1.0)])
+    err32 = group_errors(gpu, ref)
+    assert max(err32.values()) < 1e-3, err32
+    # Gauss law below 1e-5 relative (config 1 is a roundoff case: radiation, s=1; G-notes)
+    g = lat.gauss_violation()
+    cG = O.gauss_coefficient(1.0 + 31 * DTAU, 0.5, 1.0, DTAU, 1.0)
+    g_ref = O.gauss_violation(inputs.to_f32_exact(gpu), DX, K, cG)
+    assert g[3] < 1e-5 and g[7] < 1e-5, g
+    assert np.allclose(g[[1, 5]], g_ref[[1, 5]], rtol=1e-5)
+    # splitting the 32 steps into several calls gives the bit-identical state
+    gpu2, _ = run_gpu(s0, N, prm, [(5, 1.0, 0.5, 1.0), (27, 1.0 + 5 * DTAU, 0.5, 1.0)])
+    assert np.array_equal(gpu, gpu2)
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("N,m,s,f", [(24, 2 / 3, 1.0, 1.0), (40, 0.5, -1.0, 0.5), (8, 0.0, 1.0, 1.0),
+                                      (36, 0.9, 0.0, 1.0), (132, 0.5, 0.0, 1.0)])
+def test_generic_state_every_term(variant, N, m, s, f):
+    """All 20 components non-trivial, unequal couplings, friction, sizes that are not multiples of the
+    tile (ragged tails), minimum size 8, flat / radiation / matter / damping eras, s in {1, 0, -1}."""
+    from paper_2208_01525_b200 import Params
+    K = O.Couplings(lambda1=2.0, lambda2=1.7, e1=1.0, e2=0.9, eta1=1.0, eta2=1.2, kappa=0.8)
+    prm = Params(lambda1=2.0, lambda2=1.7, e1=1.0, e2=0.9, eta1=1.0, eta2=1.2, kappa=0.8, tau_norm=1.5,
+                 friction=f, kernel_variant=variant)
+    s0 = inputs.to_f32_exact(inputs.random_state((N, N, N), seed=N))
+    ref = s0.copy()
+    nsteps = 1 if N > 100 else 3
+    O.step(ref, DX, K, 2.0, m, s, DTAU, tau_norm=1.5, friction=f, n=nsteps)
+    gpu, _ = run_gpu(s0, N, prm, [(nsteps, 2.0, m, s)])
+    err = group_errors(gpu, ref)
+    assert max(err.values()) < (1e-5 if nsteps == 1 else 3e-5), err
+
+
+def test_variants_agree_closely():
+    """The tiled kernel and the reference kernel evaluate the same formulas in fp32 (different order)."""
+    from paper_2208_01525_b200 import Params
+    N = 48
+    s0 = inputs.to_f32_exact(inputs.random_state((N, N, N), seed=5))
+    a, _ = run_gpu(s0, N, Params(kernel_variant=0), [(4, 1.0, 0.5, 1.0)])
+    b, _ = run_gpu(s0, N, Params(kernel_variant=1), [(4, 1.0, 0.5, 1.0)])
+    assert max(group_errors(a, b).values()) < 5e-6
+
+
+def test_sector_symmetry_and_periodic_shift_on_gpu():
+    """PAPER.md:79 symmetry and translation covariance (exercises every periodic wrap of the kernel)."""
+    from paper_2208_01525_b200 import Params
+    N = 32
+    s0 = inputs.to_f32_exact(inputs.random_state((N, N, N), seed=9))
+    prm = Params()
+    a, _ = run_gpu(s0, N, prm, [(3, 1.0, 0.5, 1.0)])
+    sw = s0.copy()
+    sw[0:4], sw[4:8] = s0[4:8], s0[0:4]
+    sw[8:14], sw[14:20] = s0[14:20], s0[8:14]
+    b, _ = run_gpu(sw, N, prm, [(3, 1.0, 0.5, 1.0)])
+    assert np.array_equal(a[0:4], b[4:8]) and np.array_equal(a[8:14], b[14:20])
+    sh = np.roll(s0, shift=(5, -7, 13), axis=(1, 2, 3))
+    c, _ = run_gpu(sh, N, prm, [(3, 1.0, 0.5, 1.0)])
+    assert np.array_equal(np.roll(a, shift=(5, -7, 13), axis=(1, 2, 3)), c)
+
+
+def test_error_paths_on_gpu():
+    from paper_2208_01525_b200 import Lattice, Params, U1U1Error
+    lat = Lattice(16)
+    with pytest.raises(U1U1Error, match="ESTATE"):
+        lat.step(1, 1.0, 0.5, 1.0)
+    lat.init_fields(3, DX, Params())
+    with pytest.raises(U1U1Error, match="EUNSTABLE"):
+        lat.step(1, 20.0, 0.5, 1.0)
+    with pytest.raises(U1U1Error, match="ESTATE"):
+        lat.export_windings(0)
+    lat.step(2, 1.0, 0.5, 1.0)
+    assert lat.launch_count() == 3
