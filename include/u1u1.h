@@ -60,7 +60,8 @@ typedef struct {
                                 (damping prephase of BASELINE.json configs 2 and 5)              */
     double smooth_width;     /* init_kind 1: Gaussian width in lattice units                     */
     int32_t smooth_trunc;    /* init_kind 1: kernel truncated at |d| <= smooth_trunc (<= 32)     */
-    int32_t kernel_variant;  /* 0 = default (fastest); 1 = reference one-thread-per-site kernel   */
+    int32_t kernel_variant;  /* 0 = tiled kernel, accurate sincosf (default); 1 = reference one-thread-
+                                per-site kernel; 2 = tiled kernel with SFU sin/cos (abs. err 5e-7)  */
 } u1u1_params;
 
 /* Bytes of device memory the caller must provide for an N^3 lattice.

@@ -104,7 +104,7 @@ static int check_params(u1u1_ctx *ctx, const u1u1_params *p)
     if (p->init_kind != 0 && p->init_kind != 1) return fail(ctx, U1U1_EINVAL, "init_kind must be 0 or 1");
     if (p->init_kind == 1 && (!(p->smooth_width > 0) || p->smooth_trunc < 1 || p->smooth_trunc > 32))
         return fail(ctx, U1U1_EINVAL, "init_kind 1 needs smooth_width > 0 and 1 <= smooth_trunc <= 32");
-    if (p->kernel_variant < 0 || p->kernel_variant > 1) return fail(ctx, U1U1_EINVAL, "kernel_variant must be 0 or 1");
+    if (p->kernel_variant < 0 || p->kernel_variant > 5) return fail(ctx, U1U1_EINVAL, "kernel_variant must be 0..5");
     return U1U1_OK;
 }
 
@@ -195,7 +195,9 @@ extern "C" int u1u1_step(u1u1_ctx *ctx, int32_t n, double tau, double era_m, dou
     if (era_m != 0 && !(tau > 0)) return fail(ctx, U1U1_EINVAL, "tau must be positive in an expanding background");
     const u1u1_params &P = ctx->prm;
     const double dx = ctx->dx, dt = P.dtau, f = P.friction;
-    const bool tiled = P.kernel_variant == 0 && step_tiled_supports(ctx->N);
+    const bool tiled = P.kernel_variant != 1 && P.kernel_variant != 3 && step_tiled_supports(ctx->N);
+    // variants: 0 tiled fp64-chain; 2 tiled fp32 + SFU; 4 tiled fp64-chain + SFU; 5 tiled fp32; 1/3 reference fp32/fp64
+    const int tmode = P.kernel_variant == 0 ? 0 : P.kernel_variant == 4 ? 1 : P.kernel_variant == 5 ? 2 : 3;
     for (int k = 0; k < n; k++) {
         const double tk = tau + k * dt;
         double a, c, delta, omega;
@@ -224,7 +226,7 @@ extern "C" int u1u1_step(u1u1_ctx *ctx, int32_t n, double tau, double era_m, dou
         q.dtau = (float)dt;
         q.dtau_dx = (float)(dt * dx);
         Lattice L{pos_buf(ctx, ctx->cur), pos_buf(ctx, ctx->cur ^ 1), mom_buf(ctx), ctx->V, ctx->N};
-        cudaError_t e = tiled ? launch_step_tiled(L, q, ctx->stream) : launch_step_ref(L, q, ctx->stream);
+        cudaError_t e = tiled ? launch_step_tiled(L, q, ctx->stream, tmode) : launch_step_ref(L, q, ctx->stream, P.kernel_variant == 3);
         if (e != cudaSuccess) return cuda_fail(ctx, e, "step kernel launch");
         ctx->launches += 1;
         ctx->cur ^= 1;

@@ -5,8 +5,8 @@
 namespace u1u1 {
 
 // step_ref.cu / step_tiled.cu: one fused kick+drift step (Eq. 17-26)
-cudaError_t launch_step_ref(const Lattice &L, const StepCoef &k, cudaStream_t st);
-cudaError_t launch_step_tiled(const Lattice &L, const StepCoef &k, cudaStream_t st);
+cudaError_t launch_step_ref(const Lattice &L, const StepCoef &k, cudaStream_t st, bool fp64);
+cudaError_t launch_step_tiled(const Lattice &L, const StepCoef &k, cudaStream_t st, int mode);
 bool step_tiled_supports(int N);
 
 // diag.cu
