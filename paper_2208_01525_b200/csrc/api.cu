@@ -338,7 +338,7 @@ extern "C" int u1u1_diagnostics(u1u1_ctx *ctx, double *out)
 
 static int relayout(u1u1_ctx *ctx, float *canon, int to_canonical)
 {
-    cudaError_t e = launch_relayout(pos_buf(ctx, ctx->cur), mom_buf(ctx), canon, ctx->V, to_canonical, ctx->stream);
+    cudaError_t e = launch_relayout(pos_buf(ctx, ctx->cur), mom_buf(ctx), canon, ctx->V, 0, 20, to_canonical, ctx->stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "relayout kernel launch");
     ctx->launches += 1;
     if (!to_canonical) ctx->diag_valid = false;
@@ -373,23 +373,30 @@ extern "C" int u1u1_export_block(u1u1_ctx *ctx, int32_t x0, int32_t y0, int32_t 
     return U1U1_OK;
 }
 
-// Host variants: plane-by-plane cudaMemcpyAsync between the canonical host array and the internal
-// planes (no staging buffer needed: every canonical component is one contiguous internal plane).
+// Host variants: one canonical component at a time is gathered into (scattered from) the scratch buffer
+// by the relayout kernel and moved with cudaMemcpyAsync, so no second full-size device buffer is needed
+// (a canonical copy of a 1024^3 state would not fit beside the state).  Clobbers the winding scratch.
 static int host_copy(u1u1_ctx *ctx, void *host, int to_host)
 {
     const size_t V = ctx->V, bytes = V * sizeof(float);
+    float *stage = (float *)ctx->scratch;                 // scratch >= 8 V bytes >= one component plane
+    ctx->diag_valid = false;
     for (int c = 0; c < 20; c++) {
-        int is_mom, plane;
-        canonical_to_internal(c, is_mom, plane);
-        float *dev = (is_mom ? mom_buf(ctx) : pos_buf(ctx, ctx->cur)) + (size_t)plane * V;
+        float *buf = stage;
         float *h = (float *)host + (size_t)c * V;
-        cudaError_t e = to_host ? cudaMemcpyAsync(h, dev, bytes, cudaMemcpyDeviceToHost, ctx->stream)
-                                : cudaMemcpyAsync(dev, h, bytes, cudaMemcpyHostToDevice, ctx->stream);
+        cudaError_t e;
+        if (to_host) {
+            e = launch_relayout(pos_buf(ctx, ctx->cur), mom_buf(ctx), buf, V, c, 1, 1, ctx->stream);
+            if (e == cudaSuccess) e = cudaMemcpyAsync(h, buf, bytes, cudaMemcpyDeviceToHost, ctx->stream);
+        } else {
+            e = cudaMemcpyAsync(buf, h, bytes, cudaMemcpyHostToDevice, ctx->stream);
+            if (e == cudaSuccess) e = launch_relayout(pos_buf(ctx, ctx->cur), mom_buf(ctx), buf, V, c, 1, 0, ctx->stream);
+        }
         if (e != cudaSuccess) return cuda_fail(ctx, e, "host<->device state copy");
+        ctx->launches += 1;
     }
     cudaError_t e = cudaStreamSynchronize(ctx->stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "host<->device state copy (sync)");
-    if (!to_host) ctx->diag_valid = false;
     return U1U1_OK;
 }
 

@@ -7,10 +7,16 @@
 namespace u1u1 {
 
 // ------------------------------------------------------------------------------------------------
-// Internal HBM layout: structure of arrays, each plane [z][y][x], x fastest.
-//   pos[b]  b = 0,1 (ping-pong): 10 planes  0 phi_re 1 phi_im 2 psi_re 3 psi_im 4..6 thetaA 7..9 thetaB
-//   mom             : 10 planes  0 Pi_re 1 Pi_im 2 Psi_re 3 Psi_im 4..6 E 7..9 H
-// state buffer = [pos0 | pos1 | mom], 30 N^3 floats.
+// Internal HBM layout: packed vectors per site, site index lin = x + N (y + N z).
+// A position buffer (10 V floats) and the momentum buffer (10 V floats) have the same shape:
+//   pack A: float4[V]  (phi_re, phi_im, psi_re, psi_im)        | momenta: (Pi_re, Pi_im, Psi_re, Psi_im)
+//   pack B: float4[V]  (thetaA_x, thetaA_y, thetaB_x, thetaB_y) | (E_x, E_y, H_x, H_y)
+//   pack C: float2[V]  (thetaA_z, thetaB_z)                     | (E_z, H_z)
+// so one site moves as 3 vector loads + 6 vector stores, and a stencil neighbour's scalars (both
+// sectors) or in-plane links (both sectors) arrive in one 128-bit shared-memory read.
+// state buffer = [pos0 | pos1 | mom], 30 V floats.
+// "Logical" component order used by the scalar accessors: 0 phi_re 1 phi_im 2 psi_re 3 psi_im
+// 4..6 thetaA_xyz 7..9 thetaB_xyz (momenta: Pi, Psi, E_xyz, H_xyz).
 // ------------------------------------------------------------------------------------------------
 constexpr int NPOS = 10;
 constexpr int NMOM = 10;
@@ -23,7 +29,19 @@ struct Lattice {
     int N;
 };
 
-// canonical component -> (is_momentum, internal plane)
+__host__ __device__ inline size_t packA_off(size_t V) { (void)V; return 0; }
+__host__ __device__ inline size_t packB_off(size_t V) { return 4 * V; }
+__host__ __device__ inline size_t packC_off(size_t V) { return 8 * V; }
+
+// float offset of logical component c (0..9) of site lin inside a 10 V-float buffer
+__host__ __device__ inline size_t comp_off(int c, size_t lin, size_t V)
+{
+    if (c < 4) return 4 * lin + (size_t)c;
+    const int s = (c - 4) / 3, i = (c - 4) % 3;
+    return i < 2 ? 4 * V + 4 * lin + (size_t)(2 * s + i) : 8 * V + 2 * lin + (size_t)s;
+}
+
+// canonical component -> (is_momentum, logical component)
 __host__ __device__ inline void canonical_to_internal(int c, int &is_mom, int &plane)
 {
     // canonical: 0 phi_re 1 phi_im 2 Pi_re 3 Pi_im 4 psi_re 5 psi_im 6 Psi_re 7 Psi_im

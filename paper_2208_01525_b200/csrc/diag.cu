@@ -43,13 +43,13 @@ __global__ void __launch_bounds__(RED_BLOCK) gauss_kernel(const float *pos, cons
         const size_t nb[3] = {w.at(w.m(x), y, z), w.at(x, w.m(y), z), w.at(x, y, w.m(z))};
 #pragma unroll
         for (int s = 0; s < 2; s++) {
-            const float *E = mom + (size_t)(4 + 3 * s) * V;
             double div = 0.0;
 #pragma unroll
             for (int i = 0; i < 3; i++)
-                div += ((double)E[(size_t)i * V + lin] - (double)E[(size_t)i * V + nb[i]]) * k.inv_dx;
-            const double fr = pos[(size_t)(2 * s) * V + lin], fi = pos[(size_t)(2 * s + 1) * V + lin];
-            const double pr = mom[(size_t)(2 * s) * V + lin], pi = mom[(size_t)(2 * s + 1) * V + lin];
+                div += ((double)mom[comp_off(4 + 3 * s + i, lin, V)] -
+                        (double)mom[comp_off(4 + 3 * s + i, nb[i], V)]) * k.inv_dx;
+            const double fr = pos[comp_off(2 * s, lin, V)], fi = pos[comp_off(2 * s + 1, lin, V)];
+            const double pr = mom[comp_off(2 * s, lin, V)], pi = mom[comp_off(2 * s + 1, lin, V)];
             const double e0 = s ? k.e2 : k.e1;
             const double rho = 2.0 * e0 * e0 * k.cG * (fr * pi - fi * pr);
             const double g = div - rho;
@@ -65,14 +65,13 @@ __global__ void __launch_bounds__(RED_BLOCK) gauss_kernel(const float *pos, cons
 // ---------------------------------------------------------------------------------------------
 // Link angle chi_i(x) = arg( conj(f(x)) U_i(x) f(x+i) ) in (-pi, pi], atan2(0,0) = 0.
 // ---------------------------------------------------------------------------------------------
-__device__ inline float link_angle(const float *fre, const float *fim, const float *th_dir, size_t c,
-                                   size_t nb)
+__device__ inline float link_angle(const float *pos, int f0, int tcomp, size_t V, size_t c, size_t nb)
 {
     float sn, cs;
-    sincosf(th_dir[c], &sn, &cs);
-    const float ar = fre[nb], ai = fim[nb];
+    sincosf(pos[comp_off(tcomp, c, V)], &sn, &cs);
+    const float ar = pos[comp_off(f0, nb, V)], ai = pos[comp_off(f0 + 1, nb, V)];
     const float hr = cs * ar + sn * ai, hi = cs * ai - sn * ar;
-    const float fr = fre[c], fi = fim[c];
+    const float fr = pos[comp_off(f0, c, V)], fi = pos[comp_off(f0 + 1, c, V)];
     const float re = fr * hr + fi * hi, im = fr * hi - fi * hr;
     return (re == 0.f && im == 0.f) ? 0.f : atan2f(im, re);
 }
@@ -100,11 +99,10 @@ __global__ void __launch_bounds__(RED_BLOCK) winding_kernel(const float *pos, si
         const int xs[3] = {w.p(x), x, x}, ys[3] = {y, w.p(y), y}, zs[3] = {z, z, w.p(z)};
 #pragma unroll
         for (int s = 0; s < 2; s++) {
-            const float *fre = pos + (size_t)(2 * s) * V, *fim = fre + V;
-            const float *th = pos + (size_t)(4 + 3 * s) * V;
+            const int f0 = 2 * s, t0 = 4 + 3 * s;
             float chi0[3];
 #pragma unroll
-            for (int i = 0; i < 3; i++) chi0[i] = link_angle(fre, fim, th + (size_t)i * V, lin, nb[i]);
+            for (int i = 0; i < 3; i++) chi0[i] = link_angle(pos, f0, t0 + i, V, lin, nb[i]);
 #pragma unroll
             for (int o = 0; o < 3; o++) {
                 const int i = o, j = (o + 1) % 3;              // (xy), (yz), (zx)
@@ -112,11 +110,11 @@ __global__ void __launch_bounds__(RED_BLOCK) winding_kernel(const float *pos, si
                 const size_t nij = w.at(j == 0 ? w.p(xs[i]) : xs[i], j == 1 ? w.p(ys[i]) : ys[i],
                                         j == 2 ? w.p(zs[i]) : zs[i]);
                 const float c1 = chi0[i];
-                const float c2 = link_angle(fre, fim, th + (size_t)j * V, nb[i], nij);  // chi_j(x+i)
-                const float c3 = link_angle(fre, fim, th + (size_t)i * V, nb[j], nij);  // chi_i(x+j)
+                const float c2 = link_angle(pos, f0, t0 + j, V, nb[i], nij);  // chi_j(x+i)
+                const float c3 = link_angle(pos, f0, t0 + i, V, nb[j], nij);  // chi_i(x+j)
                 const float c4 = chi0[j];
-                const float P = th[(size_t)i * V + lin] + th[(size_t)j * V + nb[i]] -
-                                th[(size_t)i * V + nb[j]] - th[(size_t)j * V + lin];
+                const float P = pos[comp_off(t0 + i, lin, V)] + pos[comp_off(t0 + j, nb[i], V)] -
+                                pos[comp_off(t0 + i, nb[j], V)] - pos[comp_off(t0 + j, lin, V)];
                 const float sum = c1 + c2 - c3 - c4 + P;
                 const int W = __float2int_rn(sum * 0.15915494309189535f);
                 const int nr = near_cut(c1) | near_cut(c2) | near_cut(c3) | near_cut(c4);
@@ -172,31 +170,29 @@ __global__ void __launch_bounds__(RED_BLOCK) density_kernel(const float *pos, co
         double kin = 0, grad = 0, elec = 0, mag = 0, m2[2];
 #pragma unroll
         for (int s = 0; s < 2; s++) {
-            const float *fre = pos + (size_t)(2 * s) * V, *fim = fre + V;
-            const float *th = pos + (size_t)(4 + 3 * s) * V;
-            const float *E = mom + (size_t)(4 + 3 * s) * V;
-            const float fr = fre[lin], fi = fim[lin];
-            const float pr = mom[(size_t)(2 * s) * V + lin], pi = mom[(size_t)(2 * s + 1) * V + lin];
+            const int f0 = 2 * s, t0 = 4 + 3 * s;
+            const float fr = pos[comp_off(f0, lin, V)], fi = pos[comp_off(f0 + 1, lin, V)];
+            const float pr = mom[comp_off(f0, lin, V)], pi = mom[comp_off(f0 + 1, lin, V)];
             const double inv2e2 = 1.0 / (2.0 * (s ? k.e2 * k.e2 : k.e1 * k.e1));
             kin += (double)pr * pr + (double)pi * pi;
             m2[s] = (double)fr * fr + (double)fi * fi;
             float thc[3];
 #pragma unroll
             for (int i = 0; i < 3; i++) {
-                thc[i] = th[(size_t)i * V + lin];
+                thc[i] = pos[comp_off(t0 + i, lin, V)];
                 float sn, cs;
                 sincosf(thc[i], &sn, &cs);
-                const float ar = fre[nb[i]], ai = fim[nb[i]];
+                const float ar = pos[comp_off(f0, nb[i], V)], ai = pos[comp_off(f0 + 1, nb[i], V)];
                 const float dr = (cs * ar + sn * ai) - fr, di = (cs * ai - sn * ar) - fi;
                 grad += ((double)dr * dr + (double)di * di) * k.inv_dx2;
-                const double e = E[(size_t)i * V + lin];
+                const double e = mom[comp_off(t0 + i, lin, V)];
                 elec += e * e * inv2e2;
             }
 #pragma unroll
             for (int i = 0; i < 3; i++)
 #pragma unroll
                 for (int j = i + 1; j < 3; j++) {
-                    const float P = thc[i] + th[(size_t)j * V + nb[i]] - th[(size_t)i * V + nb[j]] - thc[j];
+                    const float P = thc[i] + pos[comp_off(t0 + j, nb[i], V)] - pos[comp_off(t0 + i, nb[j], V)] - thc[j];
                     const double F = (double)P * k.inv_dx2;
                     mag += F * F * inv2e2;
                 }

@@ -34,11 +34,13 @@ __global__ void init_random_phase_kernel(float *pos, size_t V, uint64_t seed, do
         philox4x32_10((uint32_t)lin, (uint32_t)(lin >> 32), 0u, 0u, (uint32_t)seed, (uint32_t)(seed >> 32), r);
         double sn, cs;
         sincospi(2.0 * ((double)r[0] * (1.0 / 4294967296.0)), &sn, &cs);
-        pos[0 * V + lin] = (float)(eta1 * cs);
-        pos[1 * V + lin] = (float)(eta1 * sn);
+        float4 a;
+        a.x = (float)(eta1 * cs);
+        a.y = (float)(eta1 * sn);
         sincospi(2.0 * ((double)r[1] * (1.0 / 4294967296.0)), &sn, &cs);
-        pos[2 * V + lin] = (float)(eta2 * cs);
-        pos[3 * V + lin] = (float)(eta2 * sn);
+        a.z = (float)(eta2 * cs);
+        a.w = (float)(eta2 * sn);
+        reinterpret_cast<float4 *>(pos)[lin] = a;           // pack A
     }
 }
 
@@ -96,22 +98,24 @@ __global__ void normalise_kernel(const float *src, float *pos, size_t V, double 
         for (int s = 0; s < 2; s++) {
             const double re = src[(size_t)(2 * s) * V + lin], im = src[(size_t)(2 * s + 1) * V + lin];
             const double n = sqrt(re * re + im * im), eta = s ? eta2 : eta1;
-            pos[(size_t)(2 * s) * V + lin] = (float)(n > 0 ? eta * re / n : eta);
-            pos[(size_t)(2 * s + 1) * V + lin] = (float)(n > 0 ? eta * im / n : 0.0);
+            pos[comp_off(2 * s, lin, V)] = (float)(n > 0 ? eta * re / n : eta);
+            pos[comp_off(2 * s + 1, lin, V)] = (float)(n > 0 ? eta * im / n : 0.0);
         }
     }
 }
 
-// canonical [20][V] <-> internal (pos[10][V], mom[10][V]); 128-bit copies (V is a multiple of 4).
-__global__ void relayout_kernel(float4 *pos, float4 *mom, float4 *canon, size_t V4, int to_canonical)
+// canonical [20][V] (component planes) <-> internal packed vectors.  ncomp canonical components
+// starting at c0 are moved; `canon` points at component c0's plane.
+__global__ void relayout_kernel(float *pos, float *mom, float *canon, size_t V, int c0, int ncomp,
+                                int to_canonical)
 {
-    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < 20 * V4;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < (size_t)ncomp * V;
          i += (size_t)gridDim.x * blockDim.x) {
-        const int c = (int)(i / V4);
-        const size_t r = i - (size_t)c * V4;
-        int is_mom, plane;
-        canonical_to_internal(c, is_mom, plane);
-        float4 *internal = (is_mom ? mom : pos) + (size_t)plane * V4 + r;
+        const int c = c0 + (int)(i / V);
+        const size_t lin = i % V;
+        int is_mom, comp;
+        canonical_to_internal(c, is_mom, comp);
+        float *internal = (is_mom ? mom : pos) + comp_off(comp, lin, V);
         if (to_canonical) canon[i] = *internal;
         else *internal = canon[i];
     }
@@ -132,7 +136,7 @@ __global__ void export_block_kernel(const float *pos, const float *mom, size_t V
         const int x = ((x0 + ix) % N + N) % N, y = ((y0 + iy) % N + N) % N, z = ((z0 + iz) % N + N) % N;
         int is_mom, plane;
         canonical_to_internal(c, is_mom, plane);
-        dst[i] = (is_mom ? mom : pos)[(size_t)plane * V + (size_t)x + (size_t)N * ((size_t)y + (size_t)N * z)];
+        dst[i] = (is_mom ? mom : pos)[comp_off(plane, (size_t)x + (size_t)N * ((size_t)y + (size_t)N * z), V)];
     }
 }
 
@@ -170,9 +174,10 @@ cudaError_t launch_export_block(const float *pos, const float *mom, size_t V, in
     return cudaGetLastError();
 }
 
-cudaError_t launch_relayout(float *pos, float *mom, float *canon, size_t V, int to_canonical, cudaStream_t st)
+cudaError_t launch_relayout(float *pos, float *mom, float *canon, size_t V, int c0, int ncomp, int to_canonical,
+                            cudaStream_t st)
 {
-    relayout_kernel<<<GRID, 256, 0, st>>>((float4 *)pos, (float4 *)mom, (float4 *)canon, V / 4, to_canonical);
+    relayout_kernel<<<GRID, 256, 0, st>>>(pos, mom, canon, V, c0, ncomp, to_canonical);
     return cudaGetLastError();
 }
 
