@@ -100,6 +100,26 @@ class ClockSampler:
         return out
 
 
+def replica_seed(rank):
+    """Replicas only: rank r evolves its own lattice from seed 5 + r."""
+    return 5 + int(rank)
+
+
+def max_over_ranks(values, dist, device):
+    """Element-wise MAX of a list of floats over all ranks (identity when not distributed)."""
+    if dist is None:
+        return [float(v) for v in values]
+    import torch
+    t = torch.tensor([float(v) for v in values], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return t.tolist()
+
+
+def whole_job_rate(world, steps, sites, ms):
+    """Site-updates/s of the whole job: every rank advanced `sites` sites by `steps` steps in `ms` (max over ranks)."""
+    return world * steps * sites / (ms * 1e-3)
+
+
 def oracle_sample(n, steps, seed=5):
     """The oracle as it stands on an n^3 sample of the same workload; returns (site-updates/s, cores)."""
     from oracle import oracle as O
@@ -160,7 +180,7 @@ def run_ours(args):
     V = N ** 3
     lat = Lattice(N, device=f"cuda:{local}")
     prm = Params(tau_norm=256.0, friction=0.5, kernel_variant=args.variant)
-    lat.init_fields(5 + rank, DX, prm)
+    lat.init_fields(replica_seed(rank), DX, prm)
     lat.step(args.prephase, TAU0, ERA, S)                    # damped prephase (shortened; --prephase 200 = config 5)
     prm.friction = 1.0
     lat.set_params(prm)
@@ -198,11 +218,8 @@ def run_ours(args):
     launches = lat.launch_count() - launches0
     ms_total = t_start.elapsed_time(t_end)
     ms_steps = sum(a.elapsed_time(b) for a, b in segs)
-    if dist is not None:
-        t = torch.tensor([ms_total, ms_steps], device=f"cuda:{local}", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total, ms_steps = t.tolist()
-    value = world * args.steps * V / (ms_total * 1e-3)
+    ms_total, ms_steps = max_over_ranks([ms_total, ms_steps], dist, f"cuda:{local}")
+    value = whole_job_rate(world, args.steps, V, ms_total)
     kernel_ms = ms_steps / args.steps
     achieved = BYTES_PER_SITE_UPDATE * V / (kernel_ms * 1e-3) / 1e9
     peak, peak_src = measured_peak_gbs()
@@ -272,12 +289,9 @@ def run_e2e(args, lat, tau, world, dist, local):
     t1.record()
     torch.cuda.synchronize()
     ms = t0.elapsed_time(t1)
-    if dist is not None:
-        t = torch.tensor([ms], device=f"cuda:{local}", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = t.item()
+    ms, = max_over_ranks([ms], dist, f"cuda:{local}")
     del host
-    return {"value": world * args.steps * V / (ms * 1e-3), "unit": UNIT,
+    return {"value": whole_job_rate(world, args.steps, V, ms), "unit": UNIT,
             "h2d_bytes_per_step": nbytes / args.steps, "d2h_bytes_per_step": (nbytes + 8 * 56) / args.steps,
             "ms_total": ms, "note": "checkpoint in pinned host memory -> H2D -> K steps -> diagnostics -> D2H"}
 

@@ -60,8 +60,10 @@ typedef struct {
                                 (damping prephase of BASELINE.json configs 2 and 5)              */
     double smooth_width;     /* init_kind 1: Gaussian width in lattice units                     */
     int32_t smooth_trunc;    /* init_kind 1: kernel truncated at |d| <= smooth_trunc (<= 32)     */
-    int32_t kernel_variant;  /* 0 = tiled kernel, accurate sincosf (default); 1 = reference one-thread-
-                                per-site kernel; 2 = tiled kernel with SFU sin/cos (abs. err 5e-7)  */
+    int32_t kernel_variant;  /* step kernel (DESIGN.md sections 7-8): 0 = tiled, fp64 kick chain, SFU phasor
+                                (default); 2 = tiled, fp32 chain, SFU phasor (fastest; Gauss residual ~30x
+                                the fp32 storage floor); 4 / 5 = as 0 / 2 with libm sincosf; 1 / 3 = reference
+                                one-thread-per-site kernel in fp32 / fp64                              */
 } u1u1_params;
 
 /* Bytes of device memory the caller must provide for an N^3 lattice.

@@ -196,8 +196,9 @@ extern "C" int u1u1_step(u1u1_ctx *ctx, int32_t n, double tau, double era_m, dou
     const u1u1_params &P = ctx->prm;
     const double dx = ctx->dx, dt = P.dtau, f = P.friction;
     const bool tiled = P.kernel_variant != 1 && P.kernel_variant != 3 && step_tiled_supports(ctx->N);
-    // variants: 0 tiled fp64-chain; 2 tiled fp32 + SFU; 4 tiled fp64-chain + SFU; 5 tiled fp32; 1/3 reference fp32/fp64
-    const int tmode = P.kernel_variant == 0 ? 0 : P.kernel_variant == 4 ? 1 : P.kernel_variant == 5 ? 2 : 3;
+    // variants: 0 tiled fp64-chain + SFU phasor (default); 2 tiled fp32 + SFU; 4 tiled fp64-chain + libm sincosf;
+    // 5 tiled fp32 + libm sincosf; 1/3 reference one-thread-per-site fp32/fp64
+    const int tmode = P.kernel_variant == 0 ? 1 : P.kernel_variant == 4 ? 0 : P.kernel_variant == 5 ? 2 : 3;
     for (int k = 0; k < n; k++) {
         const double tk = tau + k * dt;
         double a, c, delta, omega;

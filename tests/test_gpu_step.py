@@ -10,7 +10,7 @@ from oracle import oracle as O
 pytestmark = pytest.mark.gpu
 
 DX, DTAU = 0.5, 0.1
-VARIANTS = [0, 1, 2, 4, 5]  # 0 tiled fp64-chain (default); 1 reference; 2 tiled fp32+SFU; 4 tiled fp64-chain+SFU; 5 tiled fp32
+VARIANTS = [0, 1, 2, 4, 5]  # 0 tiled fp64-chain+SFU (default); 1 reference; 2 tiled fp32+SFU; 4 tiled fp64-chain+libm; 5 tiled fp32+libm
 
 
 def _torch():
