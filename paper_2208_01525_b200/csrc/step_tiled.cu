@@ -26,6 +26,11 @@ constexpr int SLOT_BYTES = NELEM * (16 + 16 + 8);
 constexpr int OFF_B = NELEM * 16, OFF_C = NELEM * 32;
 constexpr int NSLOT = 4;            // ring: z-1, z, z+1 in use, z+2 in flight
 constexpr int NITEM = (3 * NELEM + NTHREADS - 1) / NTHREADS;   // copies per thread per plane (4)
+// momentum ring: every thread prefetches ITS OWN site's three momentum packs one plane ahead (private data:
+// no barrier needed, only cp.async.wait_group), 2 slots of MA float4[NTHREADS] | MB float4[NTHREADS] | MC float2[NTHREADS]
+constexpr int MSLOT_BYTES = NTHREADS * (16 + 16 + 8);
+constexpr int MOFF_B = NTHREADS * 16, MOFF_C = NTHREADS * 32;
+constexpr int SMEM_BYTES = NSLOT * SLOT_BYTES + 2 * MSLOT_BYTES;
 
 __device__ inline void cp_async16(void *smem_dst, const void *gsrc)
 {
@@ -86,11 +91,9 @@ template <bool FAST>
 __device__ inline void phasor(float th, float &sn, float &cs)
 {
     if (FAST) {
-        const float n = rintf(th * 0.15915494309189535f);
-        float r = fmaf(n, -6.2831854820251465f, th);     // 2 pi = 6.2831854820251465 - 1.7484556e-7
-        r = fmaf(n, 1.7484556000744883e-7f, r);
-        sn = __sinf(r);
-        cs = __cosf(r);
+        // MUFU.SIN/COS take the angle in turns and reduce it themselves: one FMUL by 1/(2 pi) + 2 MUFU.
+        // Error max(5e-7, 6e-8 |theta|): the explicit two-constant reduction only pays for |theta| >> 8.
+        __sincosf(th, &sn, &cs);
     } else {
         sincosf(th, &sn, &cs);
     }
@@ -115,7 +118,8 @@ __device__ inline void set2(float2 &v, int i, float a) { if (i == 0) v.x = a; el
 template <bool FAST, typename R>
 __global__ void __launch_bounds__(NTHREADS, sizeof(R) == 8 ? 2 : 3) step_tiled_kernel(Lattice L, StepCoef k, int zchunk)
 {
-    extern __shared__ __align__(16) char ring[];    // NSLOT * SLOT_BYTES
+    extern __shared__ __align__(16) char ring[];    // NSLOT * SLOT_BYTES | 2 * MSLOT_BYTES
+    char *const mring = ring + NSLOT * SLOT_BYTES;
     const int N = L.N;
     const size_t V = L.V, NN = (size_t)N * N;
     const int tx = threadIdx.x & (TX - 1), ty = threadIdx.x / TX;
@@ -131,6 +135,15 @@ __global__ void __launch_bounds__(NTHREADS, sizeof(R) == 8 ? 2 : 3) step_tiled_k
 
     const int e_own = (ty + 1) * COLS + tx + 1;     // this thread's site inside a staged plane
     const size_t gsite = (size_t)(y0 + ty) * N + (size_t)(x0 + tx);
+    const char *momb = reinterpret_cast<const char *>(L.mom);
+    auto load_mom = [&](int slot, size_t lin) {
+        char *m = mring + slot * MSLOT_BYTES;
+        cp_async16(m + threadIdx.x * 16, momb + lin * 16);
+        cp_async16(m + MOFF_B + threadIdx.x * 16, momb + 16 * V + lin * 16);
+        cp_async8(m + MOFF_C + threadIdx.x * 8, momb + 32 * V + lin * 8);
+    };
+    if (active) load_mom(0, (size_t)z0 * NN + gsite);
+    cp_async_commit();
     const R aS = k.aS, bS = k.bS, aG = k.aG, bG = k.bG, inv_dx2 = k.inv_dx2, inv_dx3 = k.inv_dx3;
     const R dtau = k.dtau, dtau_dx = k.dtau_dx;
     constexpr int XP = 1, XM = -1, YP = COLS, YM = -COLS;
@@ -140,8 +153,10 @@ __global__ void __launch_bounds__(NTHREADS, sizeof(R) == 8 ? 2 : 3) step_tiled_k
         // thread's copies and guarantees slot (iz+3)%4 (plane z-2) is no longer being read
         cp_async_wait<0>();
         __syncthreads();
-        if (iz + 1 < nz)
+        if (iz + 1 < nz) {
+            if (active) load_mom((iz + 1) & 1, (size_t)(z0 + iz + 1) * NN + gsite);
             load_plane(plan, pos, ring + ((iz + 3) & 3) * SLOT_BYTES, (size_t)wrapi(z0 + iz + 2, N) * NN);
+        }
         if (!active) continue;
 
         const char *sm = ring + ((iz + 0) & 3) * SLOT_BYTES;   // plane z-1
@@ -152,10 +167,11 @@ __global__ void __launch_bounds__(NTHREADS, sizeof(R) == 8 ? 2 : 3) step_tiled_k
         auto C = [&](const char *s, int d) { return *reinterpret_cast<const float2 *>(s + OFF_C + (e_own + d) * 8); };
         const size_t lin = (size_t)(z0 + iz) * NN + gsite;
 
-        // momenta of this site: issued first so their latency overlaps the arithmetic
-        float4 MA = __ldcs(reinterpret_cast<const float4 *>(L.mom) + lin);
-        float4 MB = __ldcs(reinterpret_cast<const float4 *>(L.mom + 4 * V) + lin);
-        float2 MC = __ldcs(reinterpret_cast<const float2 *>(L.mom + 8 * V) + lin);
+        // momenta of this site: prefetched one plane ahead into this thread's private ring entry
+        const char *mslot = mring + (iz & 1) * MSLOT_BYTES;
+        float4 MA = *reinterpret_cast<const float4 *>(mslot + threadIdx.x * 16);
+        float4 MB = *reinterpret_cast<const float4 *>(mslot + MOFF_B + threadIdx.x * 16);
+        float2 MC = *reinterpret_cast<const float2 *>(mslot + MOFF_C + threadIdx.x * 8);
 
         const float4 Ac = A(sc, 0), Axp = A(sc, XP), Axm = A(sc, XM), Ayp = A(sc, YP), Aym = A(sc, YM);
         const float4 Azp = A(sp, 0), Azm = A(sm, 0);
@@ -251,7 +267,7 @@ int pick_zchunk(int N)
 template <bool FAST, typename R>
 cudaError_t launch_one(const Lattice &L, const StepCoef &k, cudaStream_t st)
 {
-    constexpr int SMEM = NSLOT * SLOT_BYTES;
+    constexpr int SMEM = SMEM_BYTES;
     static bool configured = false;
     if (!configured) {
         cudaError_t e = cudaFuncSetAttribute(step_tiled_kernel<FAST, R>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM);
