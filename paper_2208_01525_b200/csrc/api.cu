@@ -104,7 +104,8 @@ static int check_params(u1u1_ctx *ctx, const u1u1_params *p)
     if (p->init_kind != 0 && p->init_kind != 1) return fail(ctx, U1U1_EINVAL, "init_kind must be 0 or 1");
     if (p->init_kind == 1 && (!(p->smooth_width > 0) || p->smooth_trunc < 1 || p->smooth_trunc > 32))
         return fail(ctx, U1U1_EINVAL, "init_kind 1 needs smooth_width > 0 and 1 <= smooth_trunc <= 32");
-    if (p->kernel_variant < 0 || p->kernel_variant > 5) return fail(ctx, U1U1_EINVAL, "kernel_variant must be 0..5");
+    if (p->kernel_variant < 0 || (p->kernel_variant & 15) > 5 || p->kernel_variant > 255)
+        return fail(ctx, U1U1_EINVAL, "kernel_variant must be 0..5 (+16*tuning flags)");
     return U1U1_OK;
 }
 
@@ -195,10 +196,11 @@ extern "C" int u1u1_step(u1u1_ctx *ctx, int32_t n, double tau, double era_m, dou
     if (era_m != 0 && !(tau > 0)) return fail(ctx, U1U1_EINVAL, "tau must be positive in an expanding background");
     const u1u1_params &P = ctx->prm;
     const double dx = ctx->dx, dt = P.dtau, f = P.friction;
-    const bool tiled = P.kernel_variant != 1 && P.kernel_variant != 3 && step_tiled_supports(ctx->N);
+    const int kv = P.kernel_variant & 15;
+    const bool tiled = kv != 1 && kv != 3 && step_tiled_supports(ctx->N);
     // variants: 0 tiled fp64-chain + SFU phasor (default); 2 tiled fp32 + SFU; 4 tiled fp64-chain + libm sincosf;
     // 5 tiled fp32 + libm sincosf; 1/3 reference one-thread-per-site fp32/fp64
-    const int tmode = P.kernel_variant == 0 ? 1 : P.kernel_variant == 4 ? 0 : P.kernel_variant == 5 ? 2 : 3;
+    const int tmode = kv == 0 ? 1 : kv == 4 ? 0 : kv == 5 ? 2 : 3;
     for (int k = 0; k < n; k++) {
         const double tk = tau + k * dt;
         double a, c, delta, omega;
@@ -226,8 +228,9 @@ extern "C" int u1u1_step(u1u1_ctx *ctx, int32_t n, double tau, double era_m, dou
         q.inv_dx3 = (float)(1.0 / (dx * dx * dx));
         q.dtau = (float)dt;
         q.dtau_dx = (float)(dt * dx);
+        q.flags = P.kernel_variant >> 4;
         Lattice L{pos_buf(ctx, ctx->cur), pos_buf(ctx, ctx->cur ^ 1), mom_buf(ctx), ctx->V, ctx->N};
-        cudaError_t e = tiled ? launch_step_tiled(L, q, ctx->stream, tmode) : launch_step_ref(L, q, ctx->stream, P.kernel_variant == 3);
+        cudaError_t e = tiled ? launch_step_tiled(L, q, ctx->stream, tmode) : launch_step_ref(L, q, ctx->stream, kv == 3);
         if (e != cudaSuccess) return cuda_fail(ctx, e, "step kernel launch");
         ctx->launches += 1;
         ctx->cur ^= 1;

@@ -71,6 +71,7 @@ struct StepCoef {
     float inv_dx3;         // 1/dx^3
     float dtau;            // drift of the scalars
     float dtau_dx;         // drift of the link phases: theta += dtau dx E
+    int flags;             // tuning switches of the tiled kernel (kernel_variant >> 4); 0 in production
 };
 
 // Coefficients of the diagnostic sweeps.

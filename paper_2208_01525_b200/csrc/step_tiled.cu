@@ -1,13 +1,21 @@
 // step_tiled.cu -- the production fused kick+drift kernel (Eq. 17-26).
 //
 // One CTA owns an xy tile of TX x TY sites and marches through a chunk of z planes.  The three position
-// packs of each plane (A = phi,psi; B = in-plane links of both sectors; C = z links; tile + one-site halo,
-// periodic wrap resolved at load time) are staged into a 4-slot shared-memory ring with cp.async
-// (LDGSTS 16 B / 8 B), one plane ahead of the arithmetic.  Every stencil operand -- the covariant
-// 7-point Laplacian of phi, psi through the link phases and the plaquette curl of theta^A, theta^B -- is
-// a vector read from shared memory (7 + 11 LDS.128 and 8 LDS.64 per site for BOTH sectors), and each
-// site's 20 words make one HBM round trip: 3 vector loads of positions (+ halo, served by L2), 3 of
-// momenta, 3 + 3 vector stores (new positions to the other ping-pong buffer, momenta in place).
+// packs of each plane (A = phi,psi; B = in-plane links of both sectors; C = z links; tile + one-site halo)
+// are staged into a 4-slot shared-memory ring TWO planes ahead of the arithmetic:
+//   * tiles that do not touch the lattice boundary: three TMA box loads per plane (cp.async.bulk.tensor,
+//     issued by one thread, completion on an mbarrier), plus three TMA boxes for the tile's momenta;
+//   * boundary / ragged tiles (periodic wrap cannot be expressed as a TMA box): per-thread cp.async
+//     (LDGSTS) with the wrap resolved in a per-thread load plan.
+// Only planes z and z+1 live in shared memory: everything a site needs from plane z-1 -- the backward z hop
+// conj(U_z(x-z)) f(x-z) and the plaquettes P_yz(x-z), P_zx(x-z) -- was computed by the SAME thread one
+// iteration earlier and is carried in registers (the plaquettes bit-identically, see plaq()).
+// Every stencil operand is a vector read from shared memory, and each site's 20 words make one HBM round
+// trip: positions in through the ring (+ halo, served by L2), momenta in, 3 + 3 vector stores out (new
+// positions to the other ping-pong buffer, momenta in place).
+#include <cuda.h>
+#include <cstring>
+
 #include "common.cuh"
 #include "kernels.h"
 
@@ -21,82 +29,81 @@ constexpr int NTHREADS = TX * TY;
 constexpr int ROWS = TY + 2;        // + halo rows y0-1, y0+wy
 constexpr int COLS = TX + 2;        // + halo columns x0-1, x0+wx
 constexpr int NELEM = ROWS * COLS;  // staged sites per plane (340)
-// one ring slot: A float4[NELEM] | B float4[NELEM] | C float2[NELEM]  = 13 600 B
-constexpr int SLOT_BYTES = NELEM * (16 + 16 + 8);
-constexpr int OFF_B = NELEM * 16, OFF_C = NELEM * 32;
-constexpr int NSLOT = 4;            // ring: z-1, z, z+1 in use, z+2 in flight
-constexpr int NITEM = (3 * NELEM + NTHREADS - 1) / NTHREADS;   // copies per thread per plane (4)
-// momentum ring: every thread prefetches ITS OWN site's three momentum packs one plane ahead (private data:
-// no barrier needed, only cp.async.wait_group), 2 slots of MA float4[NTHREADS] | MB float4[NTHREADS] | MC float2[NTHREADS]
-constexpr int MSLOT_BYTES = NTHREADS * (16 + 16 + 8);
-constexpr int MOFF_B = NTHREADS * 16, MOFF_C = NTHREADS * 32;
-constexpr int SMEM_BYTES = NSLOT * SLOT_BYTES + 2 * MSLOT_BYTES;
+// one ring slot: A float4[NELEM] | B float4[NELEM] | C float2[NELEM], each 128-byte aligned (TMA destination)
+// TMA needs a 16-byte aligned box origin: pack C (8 B per site) is staged from x0-2, i.e. CCOLS = COLS + 2 columns
+// per row with site column c at index c + 1.
+constexpr int CCOLS = COLS + 2;
+constexpr int OFF_B = 5504, OFF_C = 11008, SLOT_BYTES = 13952;
+constexpr int POS_TX_BYTES = NELEM * 32 + ROWS * CCOLS * 8;    // bytes one plane's three boxes deliver
+constexpr int NSLOT = 4;            // ring: z, z+1 in use, z+2 and z+3 in flight
+constexpr int NITEM = (3 * NELEM + NTHREADS - 1) / NTHREADS;   // cp.async copies per thread per plane (4)
+// momentum ring (TMA tiles only): 2 slots of MA float4[NTHREADS] | MB float4[NTHREADS] | MC float2[NTHREADS]
+constexpr int MOFF_B = NTHREADS * 16, MOFF_C = NTHREADS * 32, MSLOT_BYTES = NTHREADS * 40;
+constexpr int OFF_MRING = NSLOT * SLOT_BYTES;
+constexpr int OFF_BARS = OFF_MRING + 2 * MSLOT_BYTES;           // fullP[4], fullM[2]
+constexpr int SMEM_BYTES = OFF_BARS + 64;                       // 76 352 B -> 3 CTAs per SM
+static_assert(NELEM * 16 <= OFF_B && OFF_B + NELEM * 16 <= OFF_C && OFF_C + ROWS * CCOLS * 8 <= SLOT_BYTES, "slot layout");
 
-__device__ inline void cp_async16(void *smem_dst, const void *gsrc)
+// Tensor maps of one launch: position packs of the buffer being read (boxes with halo), momentum packs.
+struct alignas(64) StepMaps {
+    CUtensorMap pA, pB, pC, mA, mB, mC;
+};
+
+__device__ inline unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+
+__device__ inline void cp_async16(unsigned sdst, const void *gsrc)
 {
-    const unsigned s = (unsigned)__cvta_generic_to_shared(smem_dst);
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(s), "l"(gsrc) : "memory");
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(sdst), "l"(gsrc) : "memory");
 }
-__device__ inline void cp_async8(void *smem_dst, const void *gsrc)
+__device__ inline void cp_async8(unsigned sdst, const void *gsrc)
 {
-    const unsigned s = (unsigned)__cvta_generic_to_shared(smem_dst);
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(s), "l"(gsrc) : "memory");
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(sdst), "l"(gsrc) : "memory");
 }
 __device__ inline void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
 template <int N_>
 __device__ inline void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N_) : "memory"); }
 
+__device__ inline void mbar_init(unsigned bar, unsigned count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ inline void mbar_expect_tx(unsigned bar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ inline void mbar_wait(unsigned bar, unsigned parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_LOOP:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra WAIT_DONE;\n"
+        "bra WAIT_LOOP;\n"
+        "WAIT_DONE:\n"
+        "}\n" ::"r"(bar), "r"(parity)
+        : "memory");
+}
+// TMA box load of a 3-d (W x + component, y, z) float tensor
+__device__ inline void tma_load_3d(unsigned sdst, const CUtensorMap *map, int c0, int c1, int c2, unsigned bar)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];\n" ::
+            "r"(sdst), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(bar)
+        : "memory");
+}
+
 __device__ inline int wrapi(int v, int N) { return v < 0 ? v + N : (v >= N ? v - N : v); }
 
-// What one thread copies for every plane (fixed across planes; only the z offset changes).
-struct LoadPlan {
-    size_t goff[NITEM];   // global BYTE offset inside the position buffer, without z
-    int soff[NITEM];      // shared byte offset inside a slot; -1 = nothing
-    int width[NITEM];     // bytes per site of this pack (16 or 8): z stride = width * N^2
-};
-
-__device__ inline LoadPlan make_plan(int N, size_t V, int x0, int y0, int wx, int wy)
-{
-    LoadPlan p;
-#pragma unroll
-    for (int k = 0; k < NITEM; k++) {
-        const int item = threadIdx.x + k * NTHREADS;      // pack-major, then row, then column
-        const int pack = item / NELEM, e = item - pack * NELEM, r = e / COLS, c = e - r * COLS;
-        const bool ok = pack < 3 && r <= wy + 1 && c <= wx + 1;
-        const int y = wrapi(r == wy + 1 ? y0 + wy : y0 - 1 + r, N);
-        const int x = wrapi(c == wx + 1 ? x0 + wx : x0 - 1 + c, N);
-        const size_t lin = (size_t)y * N + (size_t)x;
-        const int w = pack == 2 ? 8 : 16;
-        p.width[k] = w;
-        p.goff[k] = (pack == 0 ? 0 : pack == 1 ? 16 * V : 32 * V) + lin * w;
-        p.soff[k] = ok ? (pack == 0 ? 0 : pack == 1 ? OFF_B : OFF_C) + e * w : -1;
-    }
-    return p;
-}
-
-__device__ inline void load_plane(const LoadPlan &p, const char *pos, char *slot, size_t zplane /* z N^2 */)
-{
-#pragma unroll
-    for (int k = 0; k < NITEM; k++) {
-        if (p.soff[k] < 0) continue;
-        if (p.width[k] == 16) cp_async16(slot + p.soff[k], pos + p.goff[k] + zplane * 16);
-        else cp_async8(slot + p.soff[k], pos + p.goff[k] + zplane * 8);
-    }
-    cp_async_commit();
-}
-
-// exp(-i theta): accurate sincosf (1-2 ulp) or, with FAST, two-constant range reduction to [-pi, pi]
-// followed by the SFU approximations (abs. error ~ 5e-7).
+// exp(-i theta): libm sincosf (1-2 ulp) or, with FAST, the SFU approximations.  MUFU.SIN/COS take the angle
+// in turns and reduce it themselves (one FMUL by 1/(2 pi) + 2 MUFU); error max(5e-7, 6e-8 |theta|).  The
+// discrete Gauss law holds for ANY complex U used consistently for a link, so this error never enters it
+// (DESIGN.md section 8).
 template <bool FAST>
 __device__ inline void phasor(float th, float &sn, float &cs)
 {
-    if (FAST) {
-        // MUFU.SIN/COS take the angle in turns and reduce it themselves: one FMUL by 1/(2 pi) + 2 MUFU.
-        // Error max(5e-7, 6e-8 |theta|): the explicit two-constant reduction only pays for |theta| >> 8.
-        __sincosf(th, &sn, &cs);
-    } else {
-        sincosf(th, &sn, &cs);
-    }
+    if (FAST) __sincosf(th, &sn, &cs);
+    else sincosf(th, &sn, &cs);
 }
 
 // P = ((a + b) - c) - d, always in this order: a plaquette evaluated at two different sites from the same
@@ -114,72 +121,162 @@ __device__ inline void set2(float2 &v, int i, float a) { if (i == 0) v.x = a; el
 
 // R = arithmetic type of the kick chain (hops, Laplacian, currents, potential, momentum update):
 // double keeps the discrete Gauss identity Im(phi* D-D+ phi) = d-_i Im(phi* D+_i phi) at fp32-STORAGE
-// roundoff instead of fp32-ARITHMETIC roundoff (measured 10-40x smaller residual).
+// roundoff instead of fp32-ARITHMETIC roundoff (measured ~30x smaller residual).
 template <bool FAST, typename R>
-__global__ void __launch_bounds__(NTHREADS, sizeof(R) == 8 ? 2 : 3) step_tiled_kernel(Lattice L, StepCoef k, int zchunk)
+__global__ void __launch_bounds__(NTHREADS, sizeof(R) == 8 ? 2 : 3)
+step_tiled_kernel(Lattice L, StepCoef k, int zchunk, const __grid_constant__ StepMaps maps)
 {
-    extern __shared__ __align__(16) char ring[];    // NSLOT * SLOT_BYTES | 2 * MSLOT_BYTES
-    char *const mring = ring + NSLOT * SLOT_BYTES;
+    extern __shared__ __align__(128) char smem[];
+    const unsigned sbase = smem_u32(smem), bars = sbase + OFF_BARS;
     const int N = L.N;
     const size_t V = L.V, NN = (size_t)N * N;
-    const int tx = threadIdx.x & (TX - 1), ty = threadIdx.x / TX;
+    const int tid = threadIdx.x, tx = tid & (TX - 1), ty = tid / TX;
     const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY, z0 = blockIdx.z * zchunk;
     const int wx = min(TX, N - x0), wy = min(TY, N - y0), nz = min(zchunk, N - z0);
     const bool active = tx < wx && ty < wy;
-    const LoadPlan plan = make_plan(N, V, x0, y0, wx, wy);
+    // TMA boxes cannot wrap: only tiles whose halo lies inside the lattice take the TMA path (CTA-uniform)
+    const bool tma = !(k.flags & 2) && x0 >= 2 && x0 + TX + 2 <= N && y0 >= 1 && y0 + TY + 1 <= N;
+    const bool tmom = tma && !(k.flags & 4);
     const char *pos = reinterpret_cast<const char *>(L.pos_in);
 
-    // prologue: planes z0-1, z0, z0+1 into slots 0, 1, 2
+    // ---- staging of relative plane j (z = z0 + j, j = -1 .. nz) into ring slot (j + 1) & 3 ----
+    int plan_lin[NITEM];          // cp.async path: in-plane site index of each of this thread's copies (-1: none)
+    if (!tma) {
 #pragma unroll
-    for (int j = 0; j < 3; j++) load_plane(plan, pos, ring + j * SLOT_BYTES, (size_t)wrapi(z0 - 1 + j, N) * NN);
+        for (int q = 0; q < NITEM; q++) {
+            const int item = tid + q * NTHREADS;
+            const int pack = item / NELEM, e = item - pack * NELEM, r = e / COLS, c = e - r * COLS;
+            const int y = wrapi(r == wy + 1 ? y0 + wy : y0 - 1 + r, N), x = wrapi(c == wx + 1 ? x0 + wx : x0 - 1 + c, N);
+            plan_lin[q] = (pack < 3 && r <= wy + 1 && c <= wx + 1) ? y * N + x : -1;
+        }
+    }
+    auto stage_cp = [&](int j) {          // every thread; caller commits the group
+        const size_t zp = (size_t)wrapi(z0 + j, N) * NN;
+        const unsigned slot = sbase + ((j + 1) & 3) * SLOT_BYTES;
+#pragma unroll
+        for (int q = 0; q < NITEM; q++) {
+            if (plan_lin[q] < 0) continue;
+            const int item = tid + q * NTHREADS;
+            const int pack = item < NELEM ? 0 : item < 2 * NELEM ? 1 : 2, e = item - pack * NELEM;
+            const size_t site = zp + (size_t)plan_lin[q];
+            if (pack == 0) cp_async16(slot + e * 16, pos + site * 16);
+            else if (pack == 1) cp_async16(slot + OFF_B + e * 16, pos + 16 * V + site * 16);
+            else cp_async8(slot + OFF_C + (e + 2 * (e / COLS) + 1) * 8, pos + 32 * V + site * 8);
+        }
+    };
+    auto stage_tma = [&](int j) {         // one thread
+        const int z = wrapi(z0 + j, N);
+        const unsigned slot = sbase + ((j + 1) & 3) * SLOT_BYTES, bar = bars + 8 * ((j + 1) & 3);
+        mbar_expect_tx(bar, POS_TX_BYTES);
+        tma_load_3d(slot, &maps.pA, 4 * (x0 - 1), y0 - 1, z, bar);
+        tma_load_3d(slot + OFF_B, &maps.pB, 4 * (x0 - 1), y0 - 1, z, bar);
+        tma_load_3d(slot + OFF_C, &maps.pC, 2 * (x0 - 2), y0 - 1, z, bar);
+    };
+    auto stage_mom_tma = [&](int m) {     // one thread; momenta of relative plane m into ring slot m & 1
+        const unsigned slot = sbase + OFF_MRING + (m & 1) * MSLOT_BYTES, bar = bars + 8 * (4 + (m & 1));
+        mbar_expect_tx(bar, MSLOT_BYTES);
+        tma_load_3d(slot, &maps.mA, 4 * x0, y0, z0 + m, bar);
+        tma_load_3d(slot + MOFF_B, &maps.mB, 4 * x0, y0, z0 + m, bar);
+        tma_load_3d(slot + MOFF_C, &maps.mC, 2 * x0, y0, z0 + m, bar);
+    };
+
+    // ---- prologue: planes -1 .. 2 in flight, wait for -1 and 0 ----
+    if (tma) {
+        if (tid == 0) {
+#pragma unroll
+            for (int b = 0; b < 6; b++) mbar_init(bars + 8 * b, 1);
+            asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+        }
+        __syncthreads();
+        if (tid == 0) {
+            for (int j = -1; j <= 2; j++)
+                if (j <= nz) stage_tma(j);
+            if (tmom) stage_mom_tma(0);
+        }
+        mbar_wait(bars + 0, 0);
+        mbar_wait(bars + 8, 0);
+    } else {
+        for (int j = -1; j <= 2; j++) {
+            if (j <= nz) stage_cp(j);
+            cp_async_commit();
+        }
+        cp_async_wait<2>();
+        __syncthreads();
+    }
 
     const int e_own = (ty + 1) * COLS + tx + 1;     // this thread's site inside a staged plane
     const size_t gsite = (size_t)(y0 + ty) * N + (size_t)(x0 + tx);
-    const char *momb = reinterpret_cast<const char *>(L.mom);
-    auto load_mom = [&](int slot, size_t lin) {
-        char *m = mring + slot * MSLOT_BYTES;
-        cp_async16(m + threadIdx.x * 16, momb + lin * 16);
-        cp_async16(m + MOFF_B + threadIdx.x * 16, momb + 16 * V + lin * 16);
-        cp_async8(m + MOFF_C + threadIdx.x * 8, momb + 32 * V + lin * 8);
-    };
-    if (active) load_mom(0, (size_t)z0 * NN + gsite);
-    cp_async_commit();
     const R aS = k.aS, bS = k.bS, aG = k.aG, bG = k.bG, inv_dx2 = k.inv_dx2, inv_dx3 = k.inv_dx3;
-    const R dtau = k.dtau, dtau_dx = k.dtau_dx;
     constexpr int XP = 1, XM = -1, YP = COLS, YM = -COLS;
+    auto A = [&](const char *s, int d) { return *reinterpret_cast<const float4 *>(s + (e_own + d) * 16); };
+    auto B = [&](const char *s, int d) { return *reinterpret_cast<const float4 *>(s + OFF_B + (e_own + d) * 16); };
+    const int e_ownC = (ty + 1) * CCOLS + tx + 2;
+    auto C = [&](const char *s, int d) { return *reinterpret_cast<const float2 *>(s + OFF_C + (e_ownC + d) * 8); };
+    constexpr int CYP = CCOLS, CYM = -CCOLS;
+
+    // ---- carried from plane z-1: backward z hop and the two plaquettes that contain theta_z(x - z) ----
+    R bzr[2] = {0, 0}, bzi[2] = {0, 0};
+    float Pyz_c[2] = {0.f, 0.f}, Pzx_c[2] = {0.f, 0.f};
+    if (active) {
+        const char *sc = smem, *sp = smem + SLOT_BYTES;          // planes -1 and 0
+        const float4 Ac = A(sc, 0), Bc = B(sc, 0), Bzp = B(sp, 0);
+        const float2 Cc = C(sc, 0), Cxp = C(sc, XP), Cyp = C(sc, CYP);
+#pragma unroll
+        for (int s = 0; s < 2; s++) {
+            const int a0 = 2 * s, a1 = 2 * s + 1;
+            const float thz = ln2(Cc, s);
+            float snf, csf;
+            phasor<FAST>(thz, snf, csf);
+            const R sn = snf, cs = csf, fr = ln4(Ac, a0), fi = ln4(Ac, a1);
+            bzr[s] = cs * fr - sn * fi;
+            bzi[s] = cs * fi + sn * fr;
+            Pyz_c[s] = plaq(ln4(Bc, a1), ln2(Cyp, s), ln4(Bzp, a1), thz);
+            Pzx_c[s] = plaq(thz, ln4(Bzp, a0), ln2(Cxp, s), ln4(Bc, a0));
+        }
+    }
 
     for (int iz = 0; iz < nz; iz++) {
-        // plane z+1 (issued one iteration ago) has landed for this thread; the barrier publishes every
-        // thread's copies and guarantees slot (iz+3)%4 (plane z-2) is no longer being read
-        cp_async_wait<0>();
-        __syncthreads();
-        if (iz + 1 < nz) {
-            if (active) load_mom((iz + 1) & 1, (size_t)(z0 + iz + 1) * NN + gsite);
-            load_plane(plan, pos, ring + ((iz + 3) & 3) * SLOT_BYTES, (size_t)wrapi(z0 + iz + 2, N) * NN);
+        // plane iz+1 must have landed; the slot of plane iz-1 (read by every thread in the previous
+        // iteration) is recycled for plane iz+3, so its refill is issued after the barrier
+        if (tma) {
+            __syncthreads();
+            if (tid == 0) {
+                if (iz + 3 <= nz) stage_tma(iz + 3);
+                if (tmom && iz + 1 < nz) stage_mom_tma(iz + 1);
+            }
+            mbar_wait(bars + 8 * ((iz + 2) & 3), ((iz + 2) >> 2) & 1);
+            if (tmom) mbar_wait(bars + 8 * (4 + (iz & 1)), (iz >> 1) & 1);
+        } else {
+            cp_async_wait<1>();
+            __syncthreads();
+            if (iz + 3 <= nz) stage_cp(iz + 3);
+            cp_async_commit();
         }
         if (!active) continue;
 
-        const char *sm = ring + ((iz + 0) & 3) * SLOT_BYTES;   // plane z-1
-        const char *sc = ring + ((iz + 1) & 3) * SLOT_BYTES;   // plane z
-        const char *sp = ring + ((iz + 2) & 3) * SLOT_BYTES;   // plane z+1
-        auto A = [&](const char *s, int d) { return *reinterpret_cast<const float4 *>(s + (e_own + d) * 16); };
-        auto B = [&](const char *s, int d) { return *reinterpret_cast<const float4 *>(s + OFF_B + (e_own + d) * 16); };
-        auto C = [&](const char *s, int d) { return *reinterpret_cast<const float2 *>(s + OFF_C + (e_own + d) * 8); };
+        const char *sc = smem + ((iz + 1) & 3) * SLOT_BYTES;   // plane z
+        const char *sp = smem + ((iz + 2) & 3) * SLOT_BYTES;   // plane z+1
         const size_t lin = (size_t)(z0 + iz) * NN + gsite;
 
-        // momenta of this site: prefetched one plane ahead into this thread's private ring entry
-        const char *mslot = mring + (iz & 1) * MSLOT_BYTES;
-        float4 MA = *reinterpret_cast<const float4 *>(mslot + threadIdx.x * 16);
-        float4 MB = *reinterpret_cast<const float4 *>(mslot + MOFF_B + threadIdx.x * 16);
-        float2 MC = *reinterpret_cast<const float2 *>(mslot + MOFF_C + threadIdx.x * 8);
+        float4 MA, MB;
+        float2 MC;
+        if (tmom) {
+            const char *ms = smem + OFF_MRING + (iz & 1) * MSLOT_BYTES;
+            MA = *reinterpret_cast<const float4 *>(ms + tid * 16);
+            MB = *reinterpret_cast<const float4 *>(ms + MOFF_B + tid * 16);
+            MC = *reinterpret_cast<const float2 *>(ms + MOFF_C + tid * 8);
+        } else {
+            MA = __ldcs(reinterpret_cast<const float4 *>(L.mom) + lin);
+            MB = __ldcs(reinterpret_cast<const float4 *>(L.mom + 4 * V) + lin);
+            MC = __ldcs(reinterpret_cast<const float2 *>(L.mom + 8 * V) + lin);
+        }
 
         const float4 Ac = A(sc, 0), Axp = A(sc, XP), Axm = A(sc, XM), Ayp = A(sc, YP), Aym = A(sc, YM);
-        const float4 Azp = A(sp, 0), Azm = A(sm, 0);
+        const float4 Azp = A(sp, 0);
         const float4 Bc = B(sc, 0), Bxp = B(sc, XP), Bxm = B(sc, XM), Byp = B(sc, YP), Bym = B(sc, YM);
         const float4 Bxmyp = B(sc, XM + YP), Bxpym = B(sc, XP + YM);
-        const float4 Bzp = B(sp, 0), Bxmzp = B(sp, XM), Bymzp = B(sp, YM), Bzm = B(sm, 0);
-        const float2 Cc = C(sc, 0), Cxp = C(sc, XP), Cxm = C(sc, XM), Cyp = C(sc, YP), Cym = C(sc, YM);
-        const float2 Czm = C(sm, 0), Cxpzm = C(sm, XP), Cypzm = C(sm, YP);
+        const float4 Bzp = B(sp, 0), Bxmzp = B(sp, XM), Bymzp = B(sp, YM);
+        const float2 Cc = C(sc, 0), Cxp = C(sc, XP), Cxm = C(sc, XM), Cyp = C(sc, CYP), Cym = C(sc, CYM);
 
         const R m2p = (R)Ac.x * (R)Ac.x + (R)Ac.y * (R)Ac.y;
         const R m2q = (R)Ac.z * (R)Ac.z + (R)Ac.w * (R)Ac.w;
@@ -192,24 +289,30 @@ __global__ void __launch_bounds__(NTHREADS, sizeof(R) == 8 ? 2 : 3) step_tiled_k
             const R fr = ln4(Ac, a0), fi = ln4(Ac, a1);
             // ---- covariant Laplacian and currents (Eq. 17-18; current of Eq. 20-21) ----
             const float thc[3] = {ln4(Bc, a0), ln4(Bc, a1), ln2(Cc, s)};
-            const float thm[3] = {ln4(Bxm, a0), ln4(Bym, a1), ln2(Czm, s)};        // theta_i(x - i)
+            const float thm[2] = {ln4(Bxm, a0), ln4(Bym, a1)};                      // theta_i(x - i), i = x, y
             const float fpr[3] = {ln4(Axp, a0), ln4(Ayp, a0), ln4(Azp, a0)};       // f(x + i)
             const float fpi[3] = {ln4(Axp, a1), ln4(Ayp, a1), ln4(Azp, a1)};
-            const float fmr[3] = {ln4(Axm, a0), ln4(Aym, a0), ln4(Azm, a0)};       // f(x - i)
-            const float fmi[3] = {ln4(Axm, a1), ln4(Aym, a1), ln4(Azm, a1)};
-            R lap_re = (R)-6 * fr, lap_im = (R)-6 * fi, J[3];
+            const float fmr[2] = {ln4(Axm, a0), ln4(Aym, a0)};                      // f(x - i), i = x, y
+            const float fmi[2] = {ln4(Axm, a1), ln4(Aym, a1)};
+            R lap_re = (R)-6 * fr + bzr[s], lap_im = (R)-6 * fi + bzi[s], J[3];
 #pragma unroll
             for (int i = 0; i < 3; i++) {
                 float snf, csf;
                 phasor<FAST>(thc[i], snf, csf);
                 R sn = snf, cs = csf;
                 const R hr = cs * (R)fpr[i] + sn * (R)fpi[i], hi = cs * (R)fpi[i] - sn * (R)fpr[i];
-                phasor<FAST>(thm[i], snf, csf);
-                sn = snf; cs = csf;
-                const R br = cs * (R)fmr[i] - sn * (R)fmi[i], bi = cs * (R)fmi[i] + sn * (R)fmr[i];
-                lap_re += hr + br;
-                lap_im += hi + bi;
+                lap_re += hr;
+                lap_im += hi;
                 J[i] = fr * hi - fi * hr;
+                if (i == 2) {                  // backward z hop of the NEXT plane: conj(U_z(x)) f(x)
+                    bzr[s] = cs * fr - sn * fi;
+                    bzi[s] = cs * fi + sn * fr;
+                } else {
+                    phasor<FAST>(thm[i], snf, csf);
+                    sn = snf; cs = csf;
+                    lap_re += cs * (R)fmr[i] - sn * (R)fmi[i];
+                    lap_im += cs * (R)fmi[i] + sn * (R)fmr[i];
+                }
             }
             const R sig = s ? k.sig2sq : k.sig1sq, sigo = s ? k.sig1sq : k.sig2sq;
             const R m2 = s ? m2q : m2p, m2o = s ? m2p : m2q;
@@ -226,11 +329,13 @@ __global__ void __launch_bounds__(NTHREADS, sizeof(R) == 8 ? 2 : 3) step_tiled_k
             const float Pxy_my = plaq(ln4(Bym, a0), ln4(Bxpym, a1), thc[0], thm[1]);
             const float Pxy_mx = plaq(thm[0], thc[1], ln4(Bxmyp, a0), ln4(Bxm, a1));
             const float Pyz = plaq(thc[1], ln2(Cyp, s), ln4(Bzp, a1), thc[2]);
-            const float Pyz_mz = plaq(ln4(Bzm, a1), ln2(Cypzm, s), thc[1], thm[2]);
+            const float Pyz_mz = Pyz_c[s];
             const float Pyz_my = plaq(thm[1], thc[2], ln4(Bymzp, a1), ln2(Cym, s));
             const float Pzx = plaq(thc[2], ln4(Bzp, a0), ln2(Cxp, s), thc[0]);
             const float Pzx_mx = plaq(ln2(Cxm, s), ln4(Bxmzp, a0), thc[2], thm[0]);
-            const float Pzx_mz = plaq(thm[2], thc[0], ln2(Cxpzm, s), ln4(Bzm, a0));
+            const float Pzx_mz = Pzx_c[s];
+            Pyz_c[s] = Pyz;
+            Pzx_c[s] = Pzx;
             const float cc[3] = {(Pxy - Pxy_my) - (Pzx - Pzx_mz), (Pyz - Pyz_mz) - (Pxy - Pxy_mx),
                                  (Pzx - Pzx_mx) - (Pyz - Pyz_my)};
             const R cur = s ? k.cur2 : k.cur1;
@@ -244,7 +349,6 @@ __global__ void __launch_bounds__(NTHREADS, sizeof(R) == 8 ? 2 : 3) step_tiled_k
             set4(OB, a1, fmaf(k.dtau_dx, e1, thc[1]));
             set2(OC, s, fmaf(k.dtau_dx, e2, thc[2]));
         }
-        (void)dtau; (void)dtau_dx;
         __stcs(reinterpret_cast<float4 *>(L.mom) + lin, MA);
         __stcs(reinterpret_cast<float4 *>(L.mom + 4 * V) + lin, MB);
         __stcs(reinterpret_cast<float2 *>(L.mom + 8 * V) + lin, MC);
@@ -252,7 +356,7 @@ __global__ void __launch_bounds__(NTHREADS, sizeof(R) == 8 ? 2 : 3) step_tiled_k
         __stcs(reinterpret_cast<float4 *>(L.pos_out + 4 * V) + lin, OB);
         __stcs(reinterpret_cast<float2 *>(L.pos_out + 8 * V) + lin, OC);
     }
-    cp_async_wait<0>();
+    if (!tma) cp_async_wait<0>();
 }
 
 int pick_zchunk(int N)
@@ -264,19 +368,85 @@ int pick_zchunk(int N)
     return zc < N ? zc : N;
 }
 
-template <bool FAST, typename R>
-cudaError_t launch_one(const Lattice &L, const StepCoef &k, cudaStream_t st)
+// ---- tensor maps (host) -------------------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_fn()
 {
-    constexpr int SMEM = SMEM_BYTES;
+    static EncodeTiledFn fn = nullptr;
+    static bool tried = false;
+    if (!tried) {
+        tried = true;
+        void *p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = (EncodeTiledFn)p;
+    }
+    return fn;
+}
+
+// A pack of W floats per site at `base`: 3-d float tensor (W x + component, y, z), box (W bx, by, 1): x and the
+// component form ONE contiguous innermost run, so a box row is a single bx*W*4-byte request.  The box origin
+// must be 16-byte aligned, i.e. (W x) a multiple of 4 floats: any x for W = 4, even x for W = 2.
+bool encode_pack(CUtensorMap *m, const float *base, int W, int N, int bx, int by)
+{
+    const cuuint64_t n = (cuuint64_t)N, w = (cuuint64_t)W;
+    const cuuint64_t dims[3] = {w * n, n, n}, strides[2] = {4 * w * n, 4 * w * n * n};
+    const cuuint32_t box[3] = {(cuuint32_t)(W * bx), (cuuint32_t)by, 1}, es[3] = {1, 1, 1};
+    return encode_fn()(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, (void *)base, dims, strides, box, es,
+                       CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                       CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+// Maps are pure functions of (buffer addresses, N); a context alternates between two position buffers, so a
+// tiny cache avoids re-encoding on every launch.
+struct MapCacheEntry {
+    const float *pos = nullptr, *mom = nullptr;
+    int N = 0;
+    StepMaps maps;
+};
+
+bool get_maps(const Lattice &L, StepMaps &out)
+{
+    static MapCacheEntry cache[4];
+    static int next = 0;
+    for (auto &c : cache)
+        if (c.pos == L.pos_in && c.mom == L.mom && c.N == L.N) { out = c.maps; return true; }
+    if (!encode_fn()) return false;
+    MapCacheEntry &c = cache[next];
+    next = (next + 1) & 3;
+    const size_t V = L.V;
+    const bool ok = encode_pack(&c.maps.pA, L.pos_in, 4, L.N, COLS, ROWS) && encode_pack(&c.maps.pB, L.pos_in + 4 * V, 4, L.N, COLS, ROWS) &&
+                    encode_pack(&c.maps.pC, L.pos_in + 8 * V, 2, L.N, CCOLS, ROWS) && encode_pack(&c.maps.mA, L.mom, 4, L.N, TX, TY) &&
+                    encode_pack(&c.maps.mB, L.mom + 4 * V, 4, L.N, TX, TY) && encode_pack(&c.maps.mC, L.mom + 8 * V, 2, L.N, TX, TY);
+    if (!ok) { c.pos = nullptr; return false; }
+    c.pos = L.pos_in; c.mom = L.mom; c.N = L.N;
+    out = c.maps;
+    return true;
+}
+
+template <bool FAST, typename R>
+cudaError_t launch_one(const Lattice &L, StepCoef k, cudaStream_t st)
+{
     static bool configured = false;
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(step_tiled_kernel<FAST, R>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM);
+        cudaError_t e = cudaFuncSetAttribute(step_tiled_kernel<FAST, R>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
         if (e != cudaSuccess) return e;
         configured = true;
     }
+    StepMaps maps;
+    if (L.N < COLS + 2) {
+        memset(&maps, 0, sizeof maps);
+        k.flags |= 2;                       // no tile can lie strictly inside such a lattice: cp.async path only
+    } else if (!get_maps(L, maps)) {
+        return cudaErrorNotSupported;       // cuTensorMapEncodeTiled unavailable or rejected the layout: fail loudly
+    }
     const int zc = pick_zchunk(L.N);
     dim3 grid((L.N + TX - 1) / TX, (L.N + TY - 1) / TY, (L.N + zc - 1) / zc);
-    step_tiled_kernel<FAST, R><<<grid, NTHREADS, SMEM, st>>>(L, k, zc);
+    step_tiled_kernel<FAST, R><<<grid, NTHREADS, SMEM_BYTES, st>>>(L, k, zc, maps);
     return cudaGetLastError();
 }
 
