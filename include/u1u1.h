@@ -60,10 +60,14 @@ typedef struct {
                                 (damping prephase of BASELINE.json configs 2 and 5)              */
     double smooth_width;     /* init_kind 1: Gaussian width in lattice units                     */
     int32_t smooth_trunc;    /* init_kind 1: kernel truncated at |d| <= smooth_trunc (<= 32)     */
-    int32_t kernel_variant;  /* step kernel (DESIGN.md sections 7-8): 0 = tiled, fp64 kick chain, SFU phasor
-                                (default); 2 = tiled, fp32 chain, SFU phasor (fastest; Gauss residual ~30x
-                                the fp32 storage floor); 4 / 5 = as 0 / 2 with libm sincosf; 1 / 3 = reference
-                                one-thread-per-site kernel in fp32 / fp64                              */
+    int32_t kernel_variant;  /* step kernel (DESIGN.md sections 7-8):
+                                0 = tiled, fp32 chain in DIFFERENCE FORM, SFU phasor (default: fp32 speed, Gauss
+                                    residual within ~1-3x of the fp32 storage floor);
+                                2 = tiled, plain fp32 chain, SFU phasor (Gauss residual ~30x the floor);
+                                4 = tiled, fp64 kick chain, SFU phasor (Gauss residual AT the storage floor);
+                                5 / 6 / 7 = 2 / 4 / 0 with libm sincosf instead of the SFU phasor;
+                                1 / 3 = reference one-thread-per-site kernel in fp32 / fp64.
+                                Bits 4.. are tuning switches of the tiled kernel (0 in production).        */
 } u1u1_params;
 
 /* Bytes of device memory the caller must provide for an N^3 lattice.

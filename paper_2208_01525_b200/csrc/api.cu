@@ -104,8 +104,8 @@ static int check_params(u1u1_ctx *ctx, const u1u1_params *p)
     if (p->init_kind != 0 && p->init_kind != 1) return fail(ctx, U1U1_EINVAL, "init_kind must be 0 or 1");
     if (p->init_kind == 1 && (!(p->smooth_width > 0) || p->smooth_trunc < 1 || p->smooth_trunc > 32))
         return fail(ctx, U1U1_EINVAL, "init_kind 1 needs smooth_width > 0 and 1 <= smooth_trunc <= 32");
-    if (p->kernel_variant < 0 || (p->kernel_variant & 15) > 5 || p->kernel_variant > 255)
-        return fail(ctx, U1U1_EINVAL, "kernel_variant must be 0..5 (+16*tuning flags)");
+    if (p->kernel_variant < 0 || (p->kernel_variant & 15) > 7 || p->kernel_variant > 255)
+        return fail(ctx, U1U1_EINVAL, "kernel_variant must be 0..7 (+16*tuning flags)");
     return U1U1_OK;
 }
 
@@ -198,9 +198,10 @@ extern "C" int u1u1_step(u1u1_ctx *ctx, int32_t n, double tau, double era_m, dou
     const double dx = ctx->dx, dt = P.dtau, f = P.friction;
     const int kv = P.kernel_variant & 15;
     const bool tiled = kv != 1 && kv != 3 && step_tiled_supports(ctx->N);
-    // variants: 0 tiled fp64-chain + SFU phasor (default); 2 tiled fp32 + SFU; 4 tiled fp64-chain + libm sincosf;
-    // 5 tiled fp32 + libm sincosf; 1/3 reference one-thread-per-site fp32/fp64
-    const int tmode = kv == 0 ? 1 : kv == 4 ? 0 : kv == 5 ? 2 : 3;
+    // variants (include/u1u1.h): 0 tiled fp32 difference form + SFU phasor (default); 2 tiled plain fp32 + SFU;
+    // 4 tiled fp64 chain + SFU; 5 / 6 / 7 = 2 / 4 / 0 with libm sincosf; 1 / 3 reference one-thread-per-site fp32 / fp64
+    static const int tmode_of[8] = {5, -1, 3, -1, 1, 2, 0, 4};
+    const int tmode = tmode_of[kv];
     for (int k = 0; k < n; k++) {
         const double tk = tau + k * dt;
         double a, c, delta, omega;
@@ -228,6 +229,8 @@ extern "C" int u1u1_step(u1u1_ctx *ctx, int32_t n, double tau, double era_m, dou
         q.inv_dx3 = (float)(1.0 / (dx * dx * dx));
         q.dtau = (float)dt;
         q.dtau_dx = (float)(dt * dx);
+        q.aSm1 = (float)(f * (1.0 - delta) / (1.0 + delta) - 1.0);
+        q.aGm1 = (float)(f * (1.0 - omega) / (1.0 + omega) - 1.0);
         q.flags = P.kernel_variant >> 4;
         Lattice L{pos_buf(ctx, ctx->cur), pos_buf(ctx, ctx->cur ^ 1), mom_buf(ctx), ctx->V, ctx->N};
         cudaError_t e = tiled ? launch_step_tiled(L, q, ctx->stream, tmode) : launch_step_ref(L, q, ctx->stream, kv == 3);

@@ -71,6 +71,7 @@ struct StepCoef {
     float inv_dx3;         // 1/dx^3
     float dtau;            // drift of the scalars
     float dtau_dx;         // drift of the link phases: theta += dtau dx E
+    float aSm1, aGm1;      // aS - 1, aG - 1 (rounded from fp64): Pi+ = Pi- + [(aS-1) Pi- + bS (...)] keeps ONE rounding at |Pi|
     int flags;             // tuning switches of the tiled kernel (kernel_variant >> 4); 0 in production
 };
 

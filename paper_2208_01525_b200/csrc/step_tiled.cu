@@ -59,6 +59,12 @@ __device__ inline void cp_async8(unsigned sdst, const void *gsrc)
 {
     asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(sdst), "l"(gsrc) : "memory");
 }
+__device__ inline unsigned long long policy_evict_first()
+{
+    unsigned long long pol;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;\n" : "=l"(pol));
+    return pol;
+}
 __device__ inline void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
 template <int N_>
 __device__ inline void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N_) : "memory"); }
@@ -93,6 +99,17 @@ __device__ inline void tma_load_3d(unsigned sdst, const CUtensorMap *map, int c0
         : "memory");
 }
 
+// same, with an L2 evict-first hint: data that is read exactly once (the momenta) must not push the position
+// planes, which the neighbouring tiles re-read as halo, out of L2
+__device__ inline void tma_load_3d_stream(unsigned sdst, const CUtensorMap *map, int c0, int c1, int c2, unsigned bar,
+                                          unsigned long long pol)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%2, %3, %4}], [%5], %6;\n" ::
+            "r"(sdst), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(bar), "l"(pol)
+        : "memory");
+}
+
 __device__ inline int wrapi(int v, int N) { return v < 0 ? v + N : (v >= N ? v - N : v); }
 
 // exp(-i theta): libm sincosf (1-2 ulp) or, with FAST, the SFU approximations.  MUFU.SIN/COS take the angle
@@ -104,6 +121,17 @@ __device__ inline void phasor(float th, float &sn, float &cs)
 {
     if (FAST) __sincosf(th, &sn, &cs);
     else sincosf(th, &sn, &cs);
+}
+
+// Difference-form phasor: sn = sin(theta) and c1 = 1 - cos(theta) = 2 sin^2(theta/2) from the half angle, so
+// that U f' - f = (f' - f) - c1 f' -/+ i sn f' is formed from SMALL terms (no cancellation against f itself).
+template <bool FAST>
+__device__ inline void phasor_diff(float th, float &sn, float &c1)
+{
+    float sh, ch;
+    phasor<FAST>(0.5f * th, sh, ch);
+    sn = 2.f * sh * ch;
+    c1 = 2.f * sh * sh;
 }
 
 // P = ((a + b) - c) - d, always in this order: a plaquette evaluated at two different sites from the same
@@ -122,7 +150,11 @@ __device__ inline void set2(float2 &v, int i, float a) { if (i == 0) v.x = a; el
 // R = arithmetic type of the kick chain (hops, Laplacian, currents, potential, momentum update):
 // double keeps the discrete Gauss identity Im(phi* D-D+ phi) = d-_i Im(phi* D+_i phi) at fp32-STORAGE
 // roundoff instead of fp32-ARITHMETIC roundoff (measured ~30x smaller residual).
-template <bool FAST, typename R>
+// DIFF (fp32 chain only): the hops enter as differences d_i = U_i f(x+i) - f(x), d'_i = conj(U_i(x-i)) f(x-i) - f(x),
+// evaluated without cancellation; the Laplacian is their plain sum and the current is Im(f* d_i).  Rounding
+// errors then scale with |D f| dx instead of |f|, which brings the fp32 chain's Gauss residual close to the
+// storage floor wherever the fields are smooth.
+template <bool FAST, typename R, bool DIFF>
 __global__ void __launch_bounds__(NTHREADS, sizeof(R) == 8 ? 2 : 3)
 step_tiled_kernel(Lattice L, StepCoef k, int zchunk, const __grid_constant__ StepMaps maps)
 {
@@ -136,8 +168,9 @@ step_tiled_kernel(Lattice L, StepCoef k, int zchunk, const __grid_constant__ Ste
     const bool active = tx < wx && ty < wy;
     // TMA boxes cannot wrap: only tiles whose halo lies inside the lattice take the TMA path (CTA-uniform)
     const bool tma = !(k.flags & 2) && x0 >= 2 && x0 + TX + 2 <= N && y0 >= 1 && y0 + TY + 1 <= N;
-    const bool tmom = tma && !(k.flags & 4);
+    const bool tmom = tma && !(k.flags & 4);        // momenta by TMA boxes (default on TMA tiles), else ld.global.cs
     const char *pos = reinterpret_cast<const char *>(L.pos_in);
+    const unsigned long long pol_stream = policy_evict_first();
 
     // ---- staging of relative plane j (z = z0 + j, j = -1 .. nz) into ring slot (j + 1) & 3 ----
     int plan_lin[NITEM];          // cp.async path: in-plane site index of each of this thread's copies (-1: none)
@@ -175,9 +208,9 @@ step_tiled_kernel(Lattice L, StepCoef k, int zchunk, const __grid_constant__ Ste
     auto stage_mom_tma = [&](int m) {     // one thread; momenta of relative plane m into ring slot m & 1
         const unsigned slot = sbase + OFF_MRING + (m & 1) * MSLOT_BYTES, bar = bars + 8 * (4 + (m & 1));
         mbar_expect_tx(bar, MSLOT_BYTES);
-        tma_load_3d(slot, &maps.mA, 4 * x0, y0, z0 + m, bar);
-        tma_load_3d(slot + MOFF_B, &maps.mB, 4 * x0, y0, z0 + m, bar);
-        tma_load_3d(slot + MOFF_C, &maps.mC, 2 * x0, y0, z0 + m, bar);
+        tma_load_3d_stream(slot, &maps.mA, 4 * x0, y0, z0 + m, bar, pol_stream);
+        tma_load_3d_stream(slot + MOFF_B, &maps.mB, 4 * x0, y0, z0 + m, bar, pol_stream);
+        tma_load_3d_stream(slot + MOFF_C, &maps.mC, 2 * x0, y0, z0 + m, bar, pol_stream);
     };
 
     // ---- prologue: planes -1 .. 2 in flight, wait for -1 and 0 ----
@@ -225,11 +258,20 @@ step_tiled_kernel(Lattice L, StepCoef k, int zchunk, const __grid_constant__ Ste
         for (int s = 0; s < 2; s++) {
             const int a0 = 2 * s, a1 = 2 * s + 1;
             const float thz = ln2(Cc, s);
-            float snf, csf;
-            phasor<FAST>(thz, snf, csf);
-            const R sn = snf, cs = csf, fr = ln4(Ac, a0), fi = ln4(Ac, a1);
-            bzr[s] = cs * fr - sn * fi;
-            bzi[s] = cs * fi + sn * fr;
+            if (DIFF) {
+                const float4 Azp = A(sp, 0);
+                const float fr = ln4(Ac, a0), fi = ln4(Ac, a1);
+                float sn, c1;
+                phasor_diff<FAST>(thz, sn, c1);
+                bzr[s] = fmaf(-sn, fi, fmaf(-c1, fr, fr - ln4(Azp, a0)));
+                bzi[s] = fmaf(sn, fr, fmaf(-c1, fi, fi - ln4(Azp, a1)));
+            } else {
+                float snf, csf;
+                phasor<FAST>(thz, snf, csf);
+                const R sn = snf, cs = csf, fr = ln4(Ac, a0), fi = ln4(Ac, a1);
+                bzr[s] = cs * fr - sn * fi;
+                bzi[s] = cs * fi + sn * fr;
+            }
             Pyz_c[s] = plaq(ln4(Bc, a1), ln2(Cyp, s), ln4(Bzp, a1), thz);
             Pzx_c[s] = plaq(thz, ln4(Bzp, a0), ln2(Cxp, s), ln4(Bc, a0));
         }
@@ -294,9 +336,32 @@ step_tiled_kernel(Lattice L, StepCoef k, int zchunk, const __grid_constant__ Ste
             const float fpi[3] = {ln4(Axp, a1), ln4(Ayp, a1), ln4(Azp, a1)};
             const float fmr[2] = {ln4(Axm, a0), ln4(Aym, a0)};                      // f(x - i), i = x, y
             const float fmi[2] = {ln4(Axm, a1), ln4(Aym, a1)};
-            R lap_re = (R)-6 * fr + bzr[s], lap_im = (R)-6 * fi + bzi[s], J[3];
+            R lap_re = bzr[s], lap_im = bzi[s], J[3];
+            if (!DIFF) {
+                lap_re += (R)-6 * fr;
+                lap_im += (R)-6 * fi;
+            }
 #pragma unroll
             for (int i = 0; i < 3; i++) {
+                if (DIFF) {
+                    const float f_r = ln4(Ac, a0), f_i = ln4(Ac, a1);
+                    float sn, c1;
+                    phasor_diff<FAST>(thc[i], sn, c1);
+                    const float dr = fmaf(sn, fpi[i], fmaf(-c1, fpr[i], fpr[i] - f_r));
+                    const float di = fmaf(-sn, fpr[i], fmaf(-c1, fpi[i], fpi[i] - f_i));
+                    lap_re += dr;
+                    lap_im += di;
+                    J[i] = f_r * di - f_i * dr;
+                    if (i == 2) {              // backward z difference of the NEXT plane: conj(U_z(x)) f(x) - f(x+z)
+                        bzr[s] = fmaf(-sn, f_i, fmaf(-c1, f_r, f_r - fpr[2]));
+                        bzi[s] = fmaf(sn, f_r, fmaf(-c1, f_i, f_i - fpi[2]));
+                    } else {
+                        phasor_diff<FAST>(thm[i], sn, c1);
+                        lap_re += fmaf(-sn, fmi[i], fmaf(-c1, fmr[i], fmr[i] - f_r));
+                        lap_im += fmaf(sn, fmr[i], fmaf(-c1, fmi[i], fmi[i] - f_i));
+                    }
+                    continue;
+                }
                 float snf, csf;
                 phasor<FAST>(thc[i], snf, csf);
                 R sn = snf, cs = csf;
@@ -317,8 +382,15 @@ step_tiled_kernel(Lattice L, StepCoef k, int zchunk, const __grid_constant__ Ste
             const R sig = s ? k.sig2sq : k.sig1sq, sigo = s ? k.sig1sq : k.sig2sq;
             const R m2 = s ? m2q : m2p, m2o = s ? m2p : m2q;
             const R bracket = (R)(s ? k.lamh2 : k.lamh1) * (m2 - sig) - (R)k.kap * (m2o - sigo);
-            const float pr = (float)(aS * (R)ln4(MA, a0) + bS * (lap_re * inv_dx2 - fr * bracket));
-            const float pi = (float)(aS * (R)ln4(MA, a1) + bS * (lap_im * inv_dx2 - fi * bracket));
+            float pr, pi;
+            if (DIFF) {                 // small increment first, then ONE rounding at the size of the momentum
+                const float m0 = ln4(MA, a0), m1 = ln4(MA, a1);
+                pr = m0 + fmaf(k.aSm1, m0, k.bS * (float)(lap_re * inv_dx2 - fr * bracket));
+                pi = m1 + fmaf(k.aSm1, m1, k.bS * (float)(lap_im * inv_dx2 - fi * bracket));
+            } else {
+                pr = (float)(aS * (R)ln4(MA, a0) + bS * (lap_re * inv_dx2 - fr * bracket));
+                pi = (float)(aS * (R)ln4(MA, a1) + bS * (lap_im * inv_dx2 - fi * bracket));
+            }
             set4(MA, a0, pr);
             set4(MA, a1, pi);
             set4(OA, a0, fmaf(k.dtau, pr, ln4(Ac, a0)));
@@ -339,9 +411,17 @@ step_tiled_kernel(Lattice L, StepCoef k, int zchunk, const __grid_constant__ Ste
             const float cc[3] = {(Pxy - Pxy_my) - (Pzx - Pzx_mz), (Pyz - Pyz_mz) - (Pxy - Pxy_mx),
                                  (Pzx - Pzx_mx) - (Pyz - Pyz_my)};
             const R cur = s ? k.cur2 : k.cur1;
-            const float e0 = (float)(aG * (R)ln4(MB, a0) + bG * (cur * J[0] - (R)cc[0] * inv_dx3));
-            const float e1 = (float)(aG * (R)ln4(MB, a1) + bG * (cur * J[1] - (R)cc[1] * inv_dx3));
-            const float e2 = (float)(aG * (R)ln2(MC, s) + bG * (cur * J[2] - (R)cc[2] * inv_dx3));
+            float e0, e1, e2;
+            if (DIFF) {
+                const float g0 = ln4(MB, a0), g1 = ln4(MB, a1), g2 = ln2(MC, s);
+                e0 = g0 + fmaf(k.aGm1, g0, k.bG * (float)(cur * J[0] - (R)cc[0] * inv_dx3));
+                e1 = g1 + fmaf(k.aGm1, g1, k.bG * (float)(cur * J[1] - (R)cc[1] * inv_dx3));
+                e2 = g2 + fmaf(k.aGm1, g2, k.bG * (float)(cur * J[2] - (R)cc[2] * inv_dx3));
+            } else {
+                e0 = (float)(aG * (R)ln4(MB, a0) + bG * (cur * J[0] - (R)cc[0] * inv_dx3));
+                e1 = (float)(aG * (R)ln4(MB, a1) + bG * (cur * J[1] - (R)cc[1] * inv_dx3));
+                e2 = (float)(aG * (R)ln2(MC, s) + bG * (cur * J[2] - (R)cc[2] * inv_dx3));
+            }
             set4(MB, a0, e0);
             set4(MB, a1, e1);
             set2(MC, s, e2);
@@ -428,12 +508,12 @@ bool get_maps(const Lattice &L, StepMaps &out)
     return true;
 }
 
-template <bool FAST, typename R>
+template <bool FAST, typename R, bool DIFF>
 cudaError_t launch_one(const Lattice &L, StepCoef k, cudaStream_t st)
 {
     static bool configured = false;
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(step_tiled_kernel<FAST, R>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+        cudaError_t e = cudaFuncSetAttribute(step_tiled_kernel<FAST, R, DIFF>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
         if (e != cudaSuccess) return e;
         configured = true;
     }
@@ -446,7 +526,7 @@ cudaError_t launch_one(const Lattice &L, StepCoef k, cudaStream_t st)
     }
     const int zc = pick_zchunk(L.N);
     dim3 grid((L.N + TX - 1) / TX, (L.N + TY - 1) / TY, (L.N + zc - 1) / zc);
-    step_tiled_kernel<FAST, R><<<grid, NTHREADS, SMEM_BYTES, st>>>(L, k, zc, maps);
+    step_tiled_kernel<FAST, R, DIFF><<<grid, NTHREADS, SMEM_BYTES, st>>>(L, k, zc, maps);
     return cudaGetLastError();
 }
 
@@ -454,14 +534,16 @@ cudaError_t launch_one(const Lattice &L, StepCoef k, cudaStream_t st)
 
 bool step_tiled_supports(int N) { return N >= 8 && (N % 4) == 0; }
 
-// mode bit 0: SFU sin/cos; bit 1: fp32 kick chain (default is the fp64 chain)
+// mode bit 0: SFU sin/cos; bit 1: fp32 kick chain (default is the fp64 chain); 4 / 5: fp32 chain in difference form
 cudaError_t launch_step_tiled(const Lattice &L, const StepCoef &k, cudaStream_t st, int mode)
 {
-    switch (mode & 3) {
-        case 0: return launch_one<false, double>(L, k, st);
-        case 1: return launch_one<true, double>(L, k, st);
-        case 2: return launch_one<false, float>(L, k, st);
-        default: return launch_one<true, float>(L, k, st);
+    switch (mode) {
+        case 0: return launch_one<false, double, false>(L, k, st);
+        case 1: return launch_one<true, double, false>(L, k, st);
+        case 2: return launch_one<false, float, false>(L, k, st);
+        case 3: return launch_one<true, float, false>(L, k, st);
+        case 4: return launch_one<false, float, true>(L, k, st);
+        default: return launch_one<true, float, true>(L, k, st);
     }
 }
 

@@ -10,7 +10,7 @@ from oracle import oracle as O
 pytestmark = pytest.mark.gpu
 
 DX, DTAU = 0.5, 0.1
-VARIANTS = [0, 1, 2, 4, 5]  # 0 tiled fp64-chain+SFU (default); 1 reference; 2 tiled fp32+SFU; 4 tiled fp64-chain+libm; 5 tiled fp32+libm
+VARIANTS = [0, 1, 2, 4, 5, 6, 7]  # 0 tiled fp32 difference form (default); 1 reference; 2 tiled plain fp32; 4 tiled fp64 chain; 5/6/7 = 2/4/0 with libm sincosf
 
 
 def _torch():
