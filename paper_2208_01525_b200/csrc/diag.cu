@@ -35,21 +35,25 @@ __global__ void __launch_bounds__(RED_BLOCK) gauss_kernel(const float *pos, cons
                                                           int N, DiagCoef k, double *partials)
 {
     const Wrap w{N};
+    const float4 *PA = reinterpret_cast<const float4 *>(pos);
+    const float4 *MA = reinterpret_cast<const float4 *>(mom), *MB = reinterpret_cast<const float4 *>(mom + 4 * V);
+    const float2 *MC = reinterpret_cast<const float2 *>(mom + 8 * V);
     double acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     for (size_t lin = (size_t)blockIdx.x * blockDim.x + threadIdx.x; lin < V;
          lin += (size_t)gridDim.x * blockDim.x) {
         int x, y, z;
         site_xyz(lin, N, x, y, z);
-        const size_t nb[3] = {w.at(w.m(x), y, z), w.at(x, w.m(y), z), w.at(x, y, w.m(z))};
+        const float4 a = PA[lin], ma = MA[lin], eb = MB[lin], ebx = MB[w.at(w.m(x), y, z)], eby = MB[w.at(x, w.m(y), z)];
+        const float2 ec = MC[lin], ecz = MC[w.at(x, y, w.m(z))];
 #pragma unroll
         for (int s = 0; s < 2; s++) {
+            const float E[3] = {s ? eb.z : eb.x, s ? eb.w : eb.y, s ? ec.y : ec.x};
+            const float Em[3] = {s ? ebx.z : ebx.x, s ? eby.w : eby.y, s ? ecz.y : ecz.x};
             double div = 0.0;
 #pragma unroll
-            for (int i = 0; i < 3; i++)
-                div += ((double)mom[comp_off(4 + 3 * s + i, lin, V)] -
-                        (double)mom[comp_off(4 + 3 * s + i, nb[i], V)]) * k.inv_dx;
-            const double fr = pos[comp_off(2 * s, lin, V)], fi = pos[comp_off(2 * s + 1, lin, V)];
-            const double pr = mom[comp_off(2 * s, lin, V)], pi = mom[comp_off(2 * s + 1, lin, V)];
+            for (int i = 0; i < 3; i++) div += ((double)E[i] - (double)Em[i]) * k.inv_dx;
+            const double fr = s ? a.z : a.x, fi = s ? a.w : a.y;
+            const double pr = s ? ma.z : ma.x, pi = s ? ma.w : ma.y;
             const double e0 = s ? k.e2 : k.e1;
             const double rho = 2.0 * e0 * e0 * k.cG * (fr * pi - fi * pr);
             const double g = div - rho;
@@ -62,67 +66,103 @@ __global__ void __launch_bounds__(RED_BLOCK) gauss_kernel(const float *pos, cons
     block_reduce_store<8>(acc, 6, partials);
 }
 
-// ---------------------------------------------------------------------------------------------
-// Link angle chi_i(x) = arg( conj(f(x)) U_i(x) f(x+i) ) in (-pi, pi], atan2(0,0) = 0.
-// ---------------------------------------------------------------------------------------------
-__device__ inline float link_angle(const float *pos, int f0, int tcomp, size_t V, size_t c, size_t nb)
-{
-    float sn, cs;
-    sincosf(pos[comp_off(tcomp, c, V)], &sn, &cs);
-    const float ar = pos[comp_off(f0, nb, V)], ai = pos[comp_off(f0 + 1, nb, V)];
-    const float hr = cs * ar + sn * ai, hi = cs * ai - sn * ar;
-    const float fr = pos[comp_off(f0, c, V)], fi = pos[comp_off(f0 + 1, c, V)];
-    const float re = fr * hr + fi * hi, im = fr * hi - fi * hr;
-    return (re == 0.f && im == 0.f) ? 0.f : atan2f(im, re);
-}
-
 __device__ inline int near_cut(float chi) { return (3.14159265358979323846 - fabs((double)chi)) < 1e-5; }
 
 // Winding code byte: bits 0..3 = W + 8 (W in [-8, 7]), bit 4 = near-branch-cut flag.
 __device__ inline uint8_t encode_w(int w, int nearflag) { return (uint8_t)(((w + 8) & 15) | (nearflag << 4)); }
 __device__ inline int decode_w(uint8_t code) { return (int)(code & 15) - 8; }
 
-// One thread per site, both sectors, three orientations (xy, yz, zx).  Each thread evaluates the 9
-// link angles its three plaquettes need (3x redundant across neighbours; this sweep runs once per
-// 20-100 steps).  Partials: [sum|W_p|, sum|W_q|, near_p, near_q | max|W|].
-__global__ void __launch_bounds__(RED_BLOCK) winding_kernel(const float *pos, size_t V, int N,
-                                                            uint8_t *codes, double *partials)
+// ---------------------------------------------------------------------------------------------
+// Windings (reading R-12), tiled.  chi_i(x) = arg(conj(f(x)) U_i(x) f(x+i)) is the principal value of
+// v = alpha(x+i) - alpha(x) - theta_i(x) with alpha = arg f, so ONE atan2 per site and sector replaces a
+// sincos + atan2 per link: chi = v - 2 pi rint(v / 2 pi).  A CTA owns a 32 x 8 tile, marches in z, keeps the
+// phases alpha of the tile + its (+x, +y) halo for planes z and z+1 in shared memory, and evaluates the nine
+// link angles each site's three plaquettes need from them.  W = rint((sum of chi + P) / 2 pi) as before;
+// a link whose end point is exactly zero has chi = 0 (atan2(0,0) = 0, R-15).
+// Partials: [sum|W_p|, sum|W_q|, near_p, near_q | max|W|].
+// ---------------------------------------------------------------------------------------------
+constexpr int WTX = 32, WTY = 8, WEX = WTX + 1, WEY = WTY + 1, WNE = WEX * WEY, WZC = 32;
+
+__device__ inline float chi_of(float alpha_a, float alpha_b, float theta)
 {
+    if (isnan(alpha_a) || isnan(alpha_b)) return 0.f;                 // a zero end point
+    const float v = (alpha_b - alpha_a) - theta;
+    const float n = (fmaf(v, 0.15915494309189535f, 12582912.f)) - 12582912.f;      // rint(v / 2 pi), |v| < 2^22
+    float r = fmaf(n, -6.2831854820251465f, v);                        // 2 pi = 6.2831854820251465 - 1.7484556e-7
+    r = fmaf(n, 1.7484556000744883e-7f, r);
+    // the principal value lies in (-pi, pi]; rounding of v / 2 pi at the cut can leave r a hair outside
+    if (r > 3.14159274f) r -= 6.28318548f;
+    if (r <= -3.14159274f) r += 6.28318548f;
+    return r;
+}
+
+__global__ void __launch_bounds__(RED_BLOCK) winding_tiled_kernel(const float *pos, size_t V, int N, uint8_t *codes,
+                                                                  double *partials, int ntx, int nty, int nzc)
+{
+    __shared__ float alpha[2][2][WNE];                // [plane buffer][sector][extended tile site]
     const Wrap w{N};
+    const size_t NN = (size_t)N * N;
+    const float4 *PA = reinterpret_cast<const float4 *>(pos), *PB = reinterpret_cast<const float4 *>(pos + 4 * V);
+    const float2 *PC = reinterpret_cast<const float2 *>(pos + 8 * V);
+    const int tid = threadIdx.x, tx = tid & (WTX - 1), ty = tid / WTX;
     double acc[5] = {0, 0, 0, 0, 0};
-    for (size_t lin = (size_t)blockIdx.x * blockDim.x + threadIdx.x; lin < V;
-         lin += (size_t)gridDim.x * blockDim.x) {
-        int x, y, z;
-        site_xyz(lin, N, x, y, z);
-        const size_t nb[3] = {w.at(w.p(x), y, z), w.at(x, w.p(y), z), w.at(x, y, w.p(z))};
-        // forward neighbours of the forward neighbours: nb2[i][j] = x + i + j
-        const int xs[3] = {w.p(x), x, x}, ys[3] = {y, w.p(y), y}, zs[3] = {z, z, w.p(z)};
-#pragma unroll
-        for (int s = 0; s < 2; s++) {
-            const int f0 = 2 * s, t0 = 4 + 3 * s;
-            float chi0[3];
-#pragma unroll
-            for (int i = 0; i < 3; i++) chi0[i] = link_angle(pos, f0, t0 + i, V, lin, nb[i]);
-#pragma unroll
-            for (int o = 0; o < 3; o++) {
-                const int i = o, j = (o + 1) % 3;              // (xy), (yz), (zx)
-                // x+i+j
-                const size_t nij = w.at(j == 0 ? w.p(xs[i]) : xs[i], j == 1 ? w.p(ys[i]) : ys[i],
-                                        j == 2 ? w.p(zs[i]) : zs[i]);
-                const float c1 = chi0[i];
-                const float c2 = link_angle(pos, f0, t0 + j, V, nb[i], nij);  // chi_j(x+i)
-                const float c3 = link_angle(pos, f0, t0 + i, V, nb[j], nij);  // chi_i(x+j)
-                const float c4 = chi0[j];
-                const float P = pos[comp_off(t0 + i, lin, V)] + pos[comp_off(t0 + j, nb[i], V)] -
-                                pos[comp_off(t0 + i, nb[j], V)] - pos[comp_off(t0 + j, lin, V)];
-                const float sum = c1 + c2 - c3 - c4 + P;
-                const int W = __float2int_rn(sum * 0.15915494309189535f);
-                const int nr = near_cut(c1) | near_cut(c2) | near_cut(c3) | near_cut(c4);
-                codes[(size_t)(3 * s + o) * V + lin] = encode_w(W, nr);
-                acc[s] += (double)abs(W);
-                acc[2 + s] += (double)nr;
-                acc[4] = fmax(acc[4], (double)abs(W));
+    const int items = ntx * nty * nzc;
+    for (int item = blockIdx.x; item < items; item += gridDim.x) {
+        const int bx = item % ntx, by = (item / ntx) % nty, bz = item / (ntx * nty);
+        const int x0 = bx * WTX, y0 = by * WTY, z0 = bz * WZC;
+        const int wx = min(WTX, N - x0), wy = min(WTY, N - y0), nz = min(WZC, N - z0);
+        const bool active = tx < wx && ty < wy;
+        // phases of plane z (periodic) for the tile and its +x / +y halo into buffer b
+        auto fill = [&](int z, int b) {
+            for (int e = tid; e < WNE; e += RED_BLOCK) {
+                const int ey = e / WEX, ex = e - ey * WEX;
+                if (ex > wx || ey > wy) continue;
+                const int x = x0 + ex == N ? 0 : x0 + ex, y = y0 + ey == N ? 0 : y0 + ey;
+                const float4 a = PA[(size_t)z * NN + (size_t)y * N + x];
+                alpha[b][0][e] = (a.x == 0.f && a.y == 0.f) ? __int_as_float(0x7fc00000) : atan2f(a.y, a.x);
+                alpha[b][1][e] = (a.z == 0.f && a.w == 0.f) ? __int_as_float(0x7fc00000) : atan2f(a.w, a.z);
             }
+        };
+        __syncthreads();                               // previous item's readers are done
+        fill(z0, 0);
+        for (int iz = 0; iz < nz; iz++) {
+            const int z = z0 + iz, zp = w.p(z), cur = iz & 1, nxt = cur ^ 1;
+            fill(zp, nxt);
+            __syncthreads();
+            if (active) {
+                const int x = x0 + tx, y = y0 + ty, xp = w.p(x), yp = w.p(y);
+                const size_t lin = w.at(x, y, z), lx = w.at(xp, y, z), ly = w.at(x, yp, z), lz = w.at(x, y, zp);
+                const float4 Bc = PB[lin], Bx = PB[lx], By = PB[ly], Bz = PB[lz];
+                const float2 Cc = PC[lin], Cx = PC[lx], Cy = PC[ly];
+                const int e = ty * WEX + tx;
+#pragma unroll
+                for (int s = 0; s < 2; s++) {
+                    const float *ac = alpha[cur][s], *an = alpha[nxt][s];
+                    const float a0 = ac[e], ax = ac[e + 1], ay = ac[e + WEX], axy = ac[e + WEX + 1];
+                    const float az = an[e], axz = an[e + 1], ayz = an[e + WEX];
+                    const float tx0 = s ? Bc.z : Bc.x, ty0 = s ? Bc.w : Bc.y, tz0 = s ? Cc.y : Cc.x;   // theta_i(x)
+                    const float ty_x = s ? Bx.w : Bx.y, tz_x = s ? Cx.y : Cx.x;                          // theta_{y,z}(x + x)
+                    const float tx_y = s ? By.z : By.x, tz_y = s ? Cy.y : Cy.x;                          // theta_{x,z}(x + y)
+                    const float tx_z = s ? Bz.z : Bz.x, ty_z = s ? Bz.w : Bz.y;                          // theta_{x,y}(x + z)
+                    const float cx = chi_of(a0, ax, tx0), cy = chi_of(a0, ay, ty0), cz = chi_of(a0, az, tz0);
+                    // orientation o = (i, j): chi_i(x) + chi_j(x+i) - chi_i(x+j) - chi_j(x) + P_ij(x)
+                    const float c2[3] = {chi_of(ax, axy, ty_x), chi_of(ay, ayz, tz_y), chi_of(az, axz, tx_z)};
+                    const float c3[3] = {chi_of(ay, axy, tx_y), chi_of(az, ayz, ty_z), chi_of(ax, axz, tz_x)};
+                    const float c1[3] = {cx, cy, cz}, c4[3] = {cy, cz, cx};
+                    const float P[3] = {tx0 + ty_x - tx_y - ty0, ty0 + tz_y - ty_z - tz0, tz0 + tx_z - tz_x - tx0};
+#pragma unroll
+                    for (int o = 0; o < 3; o++) {
+                        const float sum = c1[o] + c2[o] - c3[o] - c4[o] + P[o];
+                        const int W = __float2int_rn(sum * 0.15915494309189535f);
+                        const int nr = near_cut(c1[o]) | near_cut(c2[o]) | near_cut(c3[o]) | near_cut(c4[o]);
+                        codes[(size_t)(3 * s + o) * V + lin] = encode_w(W, nr);
+                        acc[s] += (double)abs(W);
+                        acc[2 + s] += (double)nr;
+                        acc[4] = fmax(acc[4], (double)abs(W));
+                    }
+                }
+            }
+            __syncthreads();                           // buffer `cur` is refilled next iteration
         }
     }
     block_reduce_store<5>(acc, 4, partials);
@@ -161,41 +201,51 @@ __global__ void __launch_bounds__(RED_BLOCK) density_kernel(const float *pos, co
                                                             int N, DiagCoef k, double *partials)
 {
     const Wrap w{N};
+    const float4 *PA = reinterpret_cast<const float4 *>(pos), *PB = reinterpret_cast<const float4 *>(pos + 4 * V);
+    const float2 *PC = reinterpret_cast<const float2 *>(pos + 8 * V);
+    const float4 *MA = reinterpret_cast<const float4 *>(mom), *MB = reinterpret_cast<const float4 *>(mom + 4 * V);
+    const float2 *MC = reinterpret_cast<const float2 *>(mom + 8 * V);
     double acc[11] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
     for (size_t lin = (size_t)blockIdx.x * blockDim.x + threadIdx.x; lin < V;
          lin += (size_t)gridDim.x * blockDim.x) {
         int x, y, z;
         site_xyz(lin, N, x, y, z);
         const size_t nb[3] = {w.at(w.p(x), y, z), w.at(x, w.p(y), z), w.at(x, y, w.p(z))};
+        const float4 Ac = PA[lin], An[3] = {PA[nb[0]], PA[nb[1]], PA[nb[2]]};
+        const float4 Bc = PB[lin], Bn[3] = {PB[nb[0]], PB[nb[1]], PB[nb[2]]};
+        const float2 Cc = PC[lin], Cn[2] = {PC[nb[0]], PC[nb[1]]};
+        const float4 ma = MA[lin], mb = MB[lin];
+        const float2 mc = MC[lin];
         double kin = 0, grad = 0, elec = 0, mag = 0, m2[2];
 #pragma unroll
         for (int s = 0; s < 2; s++) {
-            const int f0 = 2 * s, t0 = 4 + 3 * s;
-            const float fr = pos[comp_off(f0, lin, V)], fi = pos[comp_off(f0 + 1, lin, V)];
-            const float pr = mom[comp_off(f0, lin, V)], pi = mom[comp_off(f0 + 1, lin, V)];
+            const float fr = s ? Ac.z : Ac.x, fi = s ? Ac.w : Ac.y;
+            const float pr = s ? ma.z : ma.x, pi = s ? ma.w : ma.y;
             const double inv2e2 = 1.0 / (2.0 * (s ? k.e2 * k.e2 : k.e1 * k.e1));
             kin += (double)pr * pr + (double)pi * pi;
             m2[s] = (double)fr * fr + (double)fi * fi;
-            float thc[3];
+            const float thc[3] = {s ? Bc.z : Bc.x, s ? Bc.w : Bc.y, s ? Cc.y : Cc.x};
+            const float ev[3] = {s ? mb.z : mb.x, s ? mb.w : mb.y, s ? mc.y : mc.x};
 #pragma unroll
             for (int i = 0; i < 3; i++) {
-                thc[i] = pos[comp_off(t0 + i, lin, V)];
                 float sn, cs;
                 sincosf(thc[i], &sn, &cs);
-                const float ar = pos[comp_off(f0, nb[i], V)], ai = pos[comp_off(f0 + 1, nb[i], V)];
+                const float ar = s ? An[i].z : An[i].x, ai = s ? An[i].w : An[i].y;
                 const float dr = (cs * ar + sn * ai) - fr, di = (cs * ai - sn * ar) - fi;
                 grad += ((double)dr * dr + (double)di * di) * k.inv_dx2;
-                const double e = mom[comp_off(t0 + i, lin, V)];
+                const double e = ev[i];
                 elec += e * e * inv2e2;
             }
+            // theta_j(x + i) for the three plaquettes (i, j) = (x,y), (x,z), (y,z) and theta_i(x + j)
+            const float ty_x = s ? Bn[0].w : Bn[0].y, tx_y = s ? Bn[1].z : Bn[1].x;
+            const float tz_x = s ? Cn[0].y : Cn[0].x, tx_z = s ? Bn[2].z : Bn[2].x;
+            const float tz_y = s ? Cn[1].y : Cn[1].x, ty_z = s ? Bn[2].w : Bn[2].y;
+            const float Pl[3] = {thc[0] + ty_x - tx_y - thc[1], thc[0] + tz_x - tx_z - thc[2], thc[1] + tz_y - ty_z - thc[2]};
 #pragma unroll
-            for (int i = 0; i < 3; i++)
-#pragma unroll
-                for (int j = i + 1; j < 3; j++) {
-                    const float P = thc[i] + pos[comp_off(t0 + j, nb[i], V)] - pos[comp_off(t0 + i, nb[j], V)] - thc[j];
-                    const double F = (double)P * k.inv_dx2;
-                    mag += F * F * inv2e2;
-                }
+            for (int q = 0; q < 3; q++) {
+                const double F = (double)Pl[q] * k.inv_dx2;
+                mag += F * F * inv2e2;
+            }
         }
         const double a2 = m2[0] - k.sig1sq, b2 = m2[1] - k.sig2sq;
         const double vint = k.kappa * a2 * b2;
@@ -271,8 +321,10 @@ cudaError_t launch_windings(const float *pos, size_t V, int N, uint8_t *codes, u
                             double *partials, double *result, cudaStream_t st)
 {
     const int nb = red_blocks(V);
-    winding_kernel<<<nb, RED_BLOCK, 0, st>>>(pos, V, N, codes, partials);
-    fold_kernel<<<1, RED_BLOCK, 0, st>>>(partials, nb, 5, 4, result);
+    const int ntx = (N + WTX - 1) / WTX, nty = (N + WTY - 1) / WTY, nzc = (N + WZC - 1) / WZC;
+    const int nbw = ntx * nty * nzc < RED_MAX_BLOCKS ? ntx * nty * nzc : RED_MAX_BLOCKS;
+    winding_tiled_kernel<<<nbw, RED_BLOCK, 0, st>>>(pos, V, N, codes, partials, ntx, nty, nzc);
+    fold_kernel<<<1, RED_BLOCK, 0, st>>>(partials, nbw, 5, 4, result);
     cells_kernel<<<nb, RED_BLOCK, 0, st>>>(codes, V, N, cells, partials);
     fold_kernel<<<1, RED_BLOCK, 0, st>>>(partials, nb, 3, 3, result + 8);
     return cudaGetLastError();
