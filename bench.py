@@ -232,7 +232,7 @@ def run_ours(args):
         return
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
-        n_s, steps_s = 192, 3
+        n_s, steps_s = 192, 8
         v, cores, dt = oracle_sample(n_s, steps_s)
         cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
                "sample": f"{n_s}^3 sub-lattice of the workload, {steps_s} steps ({dt:.1f} s), fp64 oracle as it stands"}

@@ -66,7 +66,6 @@ __global__ void __launch_bounds__(RED_BLOCK) gauss_kernel(const float *pos, cons
     block_reduce_store<8>(acc, 6, partials);
 }
 
-__device__ inline int near_cut(float chi) { return (3.14159265358979323846 - fabs((double)chi)) < 1e-5; }
 
 // Winding code byte: bits 0..3 = W + 8 (W in [-8, 7]), bit 4 = near-branch-cut flag.
 __device__ inline uint8_t encode_w(int w, int nearflag) { return (uint8_t)(((w + 8) & 15) | (nearflag << 4)); }
@@ -85,16 +84,14 @@ constexpr int WTX = 32, WTY = 8, WEX = WTX + 1, WEY = WTY + 1, WNE = WEX * WEY, 
 
 __device__ inline float chi_of(float alpha_a, float alpha_b, float theta)
 {
-    if (isnan(alpha_a) || isnan(alpha_b)) return 0.f;                 // a zero end point
-    const float v = (alpha_b - alpha_a) - theta;
+    const float v = (alpha_b - alpha_a) - theta;                       // NaN if an end point is exactly zero
     const float n = (fmaf(v, 0.15915494309189535f, 12582912.f)) - 12582912.f;      // rint(v / 2 pi), |v| < 2^22
     float r = fmaf(n, -6.2831854820251465f, v);                        // 2 pi = 6.2831854820251465 - 1.7484556e-7
     r = fmaf(n, 1.7484556000744883e-7f, r);
-    // the principal value lies in (-pi, pi]; rounding of v / 2 pi at the cut can leave r a hair outside
-    if (r > 3.14159274f) r -= 6.28318548f;
-    if (r <= -3.14159274f) r += 6.28318548f;
-    return r;
+    return r != r ? 0.f : r;             // within rounding of (-pi, pi]; anything at the cut is flagged near-cut
 }
+// near-cut flag in fp32: pi - |chi| < 1e-5  <=>  |chi| > 3.14158265...
+__device__ inline int near_cut32(float chi) { return fabsf(chi) > 3.14158265f; }
 
 __global__ void __launch_bounds__(RED_BLOCK) winding_tiled_kernel(const float *pos, size_t V, int N, uint8_t *codes,
                                                                   double *partials, int ntx, int nty, int nzc)
@@ -105,7 +102,7 @@ __global__ void __launch_bounds__(RED_BLOCK) winding_tiled_kernel(const float *p
     const float4 *PA = reinterpret_cast<const float4 *>(pos), *PB = reinterpret_cast<const float4 *>(pos + 4 * V);
     const float2 *PC = reinterpret_cast<const float2 *>(pos + 8 * V);
     const int tid = threadIdx.x, tx = tid & (WTX - 1), ty = tid / WTX;
-    double acc[5] = {0, 0, 0, 0, 0};
+    int sumw[2] = {0, 0}, nnear[2] = {0, 0}, maxw = 0;
     const int items = ntx * nty * nzc;
     for (int item = blockIdx.x; item < items; item += gridDim.x) {
         const int bx = item % ntx, by = (item / ntx) % nty, bz = item / (ntx * nty);
@@ -154,17 +151,18 @@ __global__ void __launch_bounds__(RED_BLOCK) winding_tiled_kernel(const float *p
                     for (int o = 0; o < 3; o++) {
                         const float sum = c1[o] + c2[o] - c3[o] - c4[o] + P[o];
                         const int W = __float2int_rn(sum * 0.15915494309189535f);
-                        const int nr = near_cut(c1[o]) | near_cut(c2[o]) | near_cut(c3[o]) | near_cut(c4[o]);
+                        const int nr = near_cut32(c1[o]) | near_cut32(c2[o]) | near_cut32(c3[o]) | near_cut32(c4[o]);
                         codes[(size_t)(3 * s + o) * V + lin] = encode_w(W, nr);
-                        acc[s] += (double)abs(W);
-                        acc[2 + s] += (double)nr;
-                        acc[4] = fmax(acc[4], (double)abs(W));
+                        sumw[s] += abs(W);
+                        nnear[s] += nr;
+                        maxw = max(maxw, abs(W));
                     }
                 }
             }
             __syncthreads();                           // buffer `cur` is refilled next iteration
         }
     }
+    const double acc[5] = {(double)sumw[0], (double)sumw[1], (double)nnear[0], (double)nnear[1], (double)maxw};
     block_reduce_store<5>(acc, 4, partials);
 }
 
