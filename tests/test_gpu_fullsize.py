@@ -52,3 +52,45 @@ def test_sampled_sites_full_size(N):
     d = lat.diagnostics()
     assert d["maxW"] <= 2 and d["sumW_p"] > 0 and d["sumW_q"] > 0
     assert 0 <= d["cells_pq"] <= min(d["cells_p"], d["cells_q"])
+
+
+def test_sampled_windings_full_size():
+    """Winding parity at 1024^3 on sampled 6^3 blocks: the oracle evaluates the plaquettes whose four corners
+    lie inside the exported block (sites 0..4 of each axis), the GPU values come from the full-size sweep."""
+    import torch
+    from paper_2208_01525_b200 import Lattice, Params, state_bytes, scratch_bytes
+    N = 1024
+    free, _ = torch.cuda.mem_get_info()
+    need = state_bytes(N) + scratch_bytes(N) + 9 * N ** 3 + (1 << 30)
+    if free < need:
+        pytest.skip(f"needs {need / 2**30:.0f} GiB of free HBM, have {free / 2**30:.0f}")
+    lat = Lattice(N)
+    prm = Params(tau_norm=256.0, friction=0.5)
+    lat.init_fields(5, DX, prm)
+    lat.step(12, 1.0, 0.5, 1.0)
+    d = lat.diagnostics()
+    rng = np.random.default_rng(7)
+    corners = [(0, 0, 0), (N - 3, N - 3, N - 3), (N - 2, 5, 700), (30, 6, 62), (1019, 1020, 1021)]
+    corners += [tuple(int(v) for v in rng.integers(0, N, 3)) for _ in range(20)]
+    checked = flagged = nonzero = 0
+    for sec in (0, 1):
+        W, near, cells = lat.export_windings(sec)
+        for (x, y, z) in corners:
+            blk = lat.export_block(x, y, z, 6, 6, 6).cpu().numpy().astype(np.float64)
+            Wr, near_r = O.windings(blk, DX, sec)
+            idx = [(np.arange(c, c + 5) % N) for c in (z, y, x)]
+            Wg = W[:, idx[0]][:, :, idx[1]][:, :, :, idx[2]].cpu().numpy()
+            ng = near[:, idx[0]][:, :, idx[1]][:, :, :, idx[2]].cpu().numpy()
+            excl = (ng > 0) | (near_r[:, :5, :5, :5] > 0)
+            assert np.array_equal(Wg[~excl], Wr[:, :5, :5, :5][~excl].astype(np.int8)), (sec, x, y, z)
+            checked += int((~excl).sum()); flagged += int(excl.sum()); nonzero += int(np.abs(Wg).sum())
+        # cells of the sampled corners from the GPU's own windings (PAPER.md:234): 6 faces of the cell at (x, y, z)
+        Wc = W
+        for (x, y, z) in corners[:8]:
+            xp, yp, zp = (x + 1) % N, (y + 1) % N, (z + 1) % N
+            c = (abs(int(Wc[0, z, y, x])) + abs(int(Wc[0, zp, y, x])) + abs(int(Wc[1, z, y, x])) + abs(int(Wc[1, z, y, xp])) +
+                 abs(int(Wc[2, z, y, x])) + abs(int(Wc[2, z, yp, x])))
+            assert int(cells[z, y, x]) == c
+        assert d["sumW_p" if sec == 0 else "sumW_q"] == float(W.abs().sum(dtype=torch.int64))
+        del W, near, cells
+    assert checked > 15000 and nonzero > 0          # random-phase start: plenty of strings in any block

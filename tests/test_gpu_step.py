@@ -126,3 +126,27 @@ def test_error_paths_on_gpu():
         lat.export_windings(0)
     lat.step(2, 1.0, 0.5, 1.0)
     assert lat.launch_count() == 3
+
+
+@pytest.mark.parametrize("variant", [0, 2, 4, 1])
+def test_degenerate_states(variant):
+    """All-zero fields stay exactly zero (atan2(0,0)=0, no NaN from the phasors); the uniform vacuum
+    |phi|=eta1, |psi|=eta2 with zero links and momenta is an exact fixed point in fp32."""
+    from paper_2208_01525_b200 import Lattice, Params
+    import torch
+    N = 40
+    prm = Params(eta2=1.25, kernel_variant=variant)
+    for kind in ("zero", "vacuum"):
+        s0 = np.zeros((20, N, N, N))
+        if kind == "vacuum":
+            s0[0], s0[5] = 1.0, -1.25
+        lat = Lattice(N)
+        lat.configure(DX, prm)
+        lat.import_state(torch.from_numpy(s0.astype(np.float32)))
+        lat.step(5, 1.0, 0.5, 1.0)
+        out = lat.export_state().cpu().numpy().astype(np.float64)
+        assert np.array_equal(out, s0), kind
+        d = lat.diagnostics()
+        assert d["sumW_p"] == 0 and d["sumW_q"] == 0 and d["cells_pq"] == 0 and d["near_p"] == 0
+        g = lat.gauss_violation()
+        assert g[0] == 0 and g[4] == 0
