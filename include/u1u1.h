@@ -177,6 +177,9 @@ enum {
     U1U1_D_V2_L,
     U1U1_D_V2_PQ,
     U1U1_D_ENERGY,       /* dx^3 (kin+grad+elec+mag+pot): the flat-space Hamiltonian              */
+    U1U1_D_CELLS_PQ_TOL_P, /* fast method with one cell of tolerance: pierced p cells  */
+    U1U1_D_CELLS_PQ_TOL_Q, /* with a pierced q cell in their 3x3x3 neighbourhood; and q cells near p   */
+    U1U1_D_L_PQ_TOL,     /* dx (tol_p + tol_q) / 2: equals L_pq for coincident AND for one-cell-displaced strings */
     U1U1_D_USED          /* number of slots in use; the rest of the 48 are zero                   */
 };
 

@@ -213,6 +213,21 @@ def cells(W, dx=1.0):
     return C
 
 
+def cells_pq_tolerant(Cp, Cq):
+    """Fast method with one cell of tolerance, PAPER.md:234 ("non-zero at the same location, or displaced by one
+    cell in any direction"), reading R-13b: (number of pierced p cells with a pierced q cell in their periodic
+    3x3x3 neighbourhood, number of pierced q cells with a pierced p cell in theirs)."""
+    def dilate(mask):
+        out = np.zeros_like(mask)
+        for dz in (-1, 0, 1):
+            for dy in (-1, 0, 1):
+                for dx_ in (-1, 0, 1):
+                    out |= np.roll(mask, (dz, dy, dx_), axis=(0, 1, 2))
+        return out
+    p, q = Cp > 0, Cq > 0
+    return int(np.sum(p & dilate(q))), int(np.sum(q & dilate(p)))
+
+
 def densities(state, dx, K):
     """dict of per-site arrays kin, grad, elec, mag, pot, vint (no scale-factor weights)."""
     lat, kc = _lat(state, dx), K.c()
@@ -243,6 +258,8 @@ def diagnostics(state, dx, K, c, cut_tol=1e-5):
         out[f"cells_{tag}"] = int(np.sum(C > 0))
         out[f"maxW_{tag}"] = int(np.max(np.abs(W)))
     out["cells_pq"] = int(np.sum((Cs[0] > 0) & (Cs[1] > 0)))
+    out["cells_pq_tol_p"], out["cells_pq_tol_q"] = cells_pq_tolerant(Cs[0], Cs[1])
+    out["L_pq_tol"] = 0.5 * dx * (out["cells_pq_tol_p"] + out["cells_pq_tol_q"])
     d = densities(state, dx, K)
     lag = d["kin"] - d["grad"] + (d["elec"] - d["mag"]) / c - c * d["pot"]
     out["sum_L"] = float(np.sum(lag))

@@ -297,13 +297,13 @@ extern "C" int u1u1_diagnostics(u1u1_ctx *ctx, double *out)
     const size_t V = ctx->V;
     uint8_t *codes = ctx->scratch, *cells = ctx->scratch + 6 * V;
     double *res = result(ctx);
-    // result slots: [0..4] windings, [8..10] cells, [16..26] densities
+    // result slots: [0..4] windings, [8..10] cells, [12..13] tolerant overlap, [16..26] densities
     cudaError_t e = launch_windings(pos_buf(ctx, ctx->cur), V, ctx->N, codes, cells, partials(ctx), res, ctx->stream);
     if (e == cudaSuccess)
         e = launch_densities(pos_buf(ctx, ctx->cur), mom_buf(ctx), V, ctx->N, diag_coef(ctx), partials(ctx),
                              res + 16, ctx->stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "diagnostics kernel launch");
-    ctx->launches += 6;
+    ctx->launches += 8;
     double r[32];
     if (int rc = fetch(ctx, r, 32)) return rc;
     ctx->diag_valid = true;
@@ -340,6 +340,9 @@ extern "C" int u1u1_diagnostics(u1u1_ctx *ctx, double *out)
     out[U1U1_D_V2_L] = 2.0 * RL / (1.0 + RL);
     out[U1U1_D_V2_PQ] = 2.0 * RV / (1.0 + RV);
     out[U1U1_D_ENERGY] = dx * dx * dx * (r[22] + r[23] + r[24] + r[25] + r[26]);
+    out[U1U1_D_CELLS_PQ_TOL_P] = r[12];
+    out[U1U1_D_CELLS_PQ_TOL_Q] = r[13];
+    out[U1U1_D_L_PQ_TOL] = 0.5 * dx * (r[12] + r[13]);
     return U1U1_OK;
 }
 

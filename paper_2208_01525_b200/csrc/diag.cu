@@ -193,6 +193,35 @@ __global__ void __launch_bounds__(RED_BLOCK) cells_kernel(const uint8_t *codes, 
     block_reduce_store<3>(acc, 3, partials);
 }
 
+// Fast method with one cell of tolerance ("non-zero at the same location, or displaced by one cell in
+// any direction"; reading R-13b): a pierced p cell counts if a pierced q cell lies in its 3x3x3 neighbourhood
+// (periodic), and vice versa.  Pierced cells are sparse, so almost every thread stops after two byte loads.
+// Partials: [#p cells with a q cell within one cell, #q cells with a p cell within one cell].
+__global__ void __launch_bounds__(RED_BLOCK) overlap_tol_kernel(const uint8_t *cells, size_t V, int N, double *partials)
+{
+    const Wrap w{N};
+    double acc[2] = {0, 0};
+    for (size_t lin = (size_t)blockIdx.x * blockDim.x + threadIdx.x; lin < V;
+         lin += (size_t)gridDim.x * blockDim.x) {
+        const int cp = cells[lin], cq = cells[V + lin];
+        if ((cp | cq) == 0) continue;
+        int x, y, z;
+        site_xyz(lin, N, x, y, z);
+        const int xs[3] = {w.m(x), x, w.p(x)}, ys[3] = {w.m(y), y, w.p(y)}, zs[3] = {w.m(z), z, w.p(z)};
+        int anyp = 0, anyq = 0;
+        for (int c = 0; c < 3; c++)
+            for (int b = 0; b < 3; b++)
+                for (int a = 0; a < 3; a++) {
+                    const size_t nb = w.at(xs[a], ys[b], zs[c]);
+                    anyp |= cells[nb];
+                    anyq |= cells[V + nb];
+                }
+        acc[0] += (cp > 0 && anyq > 0);
+        acc[1] += (cq > 0 && anyp > 0);
+    }
+    block_reduce_store<2>(acc, 2, partials);
+}
+
 // Lagrangian, velocity-estimator and energy sums.  Partials:
 // [sum L, sum kin L, sum grad L, sum kin V, sum grad V, sum V, sum kin, sum grad, sum elec, sum mag, sum pot]
 __global__ void __launch_bounds__(RED_BLOCK) density_kernel(const float *pos, const float *mom, size_t V,
@@ -325,6 +354,8 @@ cudaError_t launch_windings(const float *pos, size_t V, int N, uint8_t *codes, u
     fold_kernel<<<1, RED_BLOCK, 0, st>>>(partials, nbw, 5, 4, result);
     cells_kernel<<<nb, RED_BLOCK, 0, st>>>(codes, V, N, cells, partials);
     fold_kernel<<<1, RED_BLOCK, 0, st>>>(partials, nb, 3, 3, result + 8);
+    overlap_tol_kernel<<<nb, RED_BLOCK, 0, st>>>(cells, V, N, partials);
+    fold_kernel<<<1, RED_BLOCK, 0, st>>>(partials, nb, 2, 2, result + 12);
     return cudaGetLastError();
 }
 

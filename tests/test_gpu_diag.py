@@ -111,6 +111,12 @@ def test_diagnostics_match_oracle(N, nsteps, kind):
     assert d["cells_pq"] == np.sum((cells_gpu[0] > 0) & (cells_gpu[1] > 0))
     if tot_near == 0:
         assert d["cells_pq"] == ref["cells_pq"]
+    # one-cell-tolerance overlap: from the GPU's own cell arrays through the oracle's rule, bit-exact
+    tol = O.cells_pq_tolerant(cells_gpu[0].astype(np.int32), cells_gpu[1].astype(np.int32))
+    assert (d["cells_pq_tol_p"], d["cells_pq_tol_q"]) == tol and d["L_pq_tol"] == 0.5 * DX * sum(tol)
+    assert tol[0] >= d["cells_pq"] and tol[1] >= d["cells_pq"]
+    if tot_near == 0:
+        assert tol == (ref["cells_pq_tol_p"], ref["cells_pq_tol_q"])
     assert d["maxW"] == max(ref["maxW_p"], ref["maxW_q"]) or tot_near > 0
     # floating-point sums: fp32 per-site terms, fp64 accumulation.  Scale = sum of |terms|.
     scale = ref["sum_kin"] + ref["sum_grad"] + ref["sum_elec"] + ref["sum_mag"] + abs(ref["sum_pot"])
@@ -143,6 +149,7 @@ def test_known_vortex_lines_on_gpu():
     d = lat.diagnostics()
     assert d["sumW_p"] == 2 * N and d["sumW_q"] == 2 * N and d["cells_pq"] == 2 * N and d["maxW"] == 1
     assert d["L_pq"] == 2.0 * N and d["L_p"] == 0.0 and d["f_total"] == 1.0
+    assert d["cells_pq_tol_p"] == 2 * N and d["cells_pq_tol_q"] == 2 * N and d["L_pq_tol"] == 2.0 * N
     W, near, cells = lat.export_windings(0)
     assert int(cells.max()) == 2 and int((cells == 2).sum()) == 2 * N
     assert bool((W[0, :, 7, 3] == 1).all()) and bool((W[0, :, 7, 11] == -1).all())

@@ -2,6 +2,8 @@
 outputs: 5^3 neighbourhoods are exported before a step, the oracle steps each as a tiny periodic
 lattice (only the centre site is free of wrap pollution: the stencil reaches one site, diagonals
 included), and the centre is compared with the GPU's value after the step."""
+import gc
+
 import numpy as np
 import pytest
 
@@ -16,6 +18,7 @@ DX, DTAU = 0.5, 0.1
 def test_sampled_sites_full_size(N):
     import torch
     from paper_2208_01525_b200 import Lattice, Params, state_bytes, scratch_bytes
+    gc.collect(); torch.cuda.empty_cache()              # lattices of earlier tests may still sit in torch's cache
     free, _ = torch.cuda.mem_get_info()
     need = state_bytes(N) + scratch_bytes(N) + (1 << 30)
     if free < need:
@@ -60,6 +63,7 @@ def test_sampled_windings_full_size():
     import torch
     from paper_2208_01525_b200 import Lattice, Params, state_bytes, scratch_bytes
     N = 1024
+    gc.collect(); torch.cuda.empty_cache()
     free, _ = torch.cuda.mem_get_info()
     need = state_bytes(N) + scratch_bytes(N) + 9 * N ** 3 + (1 << 30)
     if free < need:

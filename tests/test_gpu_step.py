@@ -1,6 +1,8 @@
 """GPU parity of the fused leapfrog step (through the C ABI) against the fp64 oracle, element by element
 on identical (fp32-representable) seeded inputs.  Tolerances are north_star's: max relative error per
 field group (max|gpu-oracle| / max|oracle|, reading R-16) 1e-5 after 1 step, 1e-3 after 32."""
+import os
+
 import numpy as np
 import pytest
 
@@ -150,3 +152,34 @@ def test_degenerate_states(variant):
         assert d["sumW_p"] == 0 and d["sumW_q"] == 0 and d["cells_pq"] == 0 and d["near_p"] == 0
         g = lat.gauss_violation()
         assert g[0] == 0 and g[4] == 0
+
+
+def test_growth_then_physical_schedule():
+    """SURVEY 8(f)-4 / PAPER.md:328-339 Table III: a core-growth phase (beta = beta_growth < 0, a normalised to 1 at
+    its start) followed by physical evolution (beta = 1, a normalised to 1 at the end) is a sequence of `step`
+    calls with `set_params` in between; here on a short schedule, against the oracle doing the same."""
+    from paper_2208_01525_b200 import Lattice, Params
+    import torch
+    N, n1, n2 = 48, 12, 12
+    beta_g = float([l.split()[1] for l in open(os.path.join(os.path.dirname(__file__), "golden", "paper_values.txt"))
+                    if l.startswith("table3_beta_growth_rad")][0])
+    tau0, tau_tr = 5.0, 5.0 + n1 * DTAU
+    tau_end = tau_tr + n2 * DTAU
+    s0 = inputs.to_f32_exact(inputs.random_state((N, N, N), seed=77, amp_mom=0.1, amp_theta=0.3))
+    K = O.Couplings()
+    ref = s0.copy()
+    O.step(ref, DX, K, tau0, 0.5, beta_g, DTAU, tau_norm=tau0, n=n1)
+    O.step(ref, DX, K, tau_tr, 0.5, 1.0, DTAU, tau_norm=tau_end, n=n2)
+    lat = Lattice(N)
+    prm = Params(tau_norm=tau0)
+    lat.configure(DX, prm)
+    lat.import_state(torch.from_numpy(s0.astype(np.float32)))
+    lat.step(n1, tau0, 0.5, beta_g)
+    prm.tau_norm = tau_end
+    lat.set_params(prm)
+    lat.step(n2, tau_tr, 0.5, 1.0)
+    gpu = lat.export_state().cpu().numpy().astype(np.float64)
+    err = group_errors(gpu, ref)
+    assert max(err.values()) < 1e-4, err
+    d = lat.diagnostics()
+    assert np.isclose(d["a"], 1.0) and np.isclose(d["tau"], tau_end)     # width normalised to 1 at the end

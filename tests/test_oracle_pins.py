@@ -537,3 +537,30 @@ def test_derived_scalars_definitions():
     assert np.isclose(d["xi_L"], np.sqrt(2 * np.pi * vol / (0.125 * 50)))  # Eq. 33, mu = 2 pi
     assert np.isclose(d["v2_L"], 2 * (1 / 3) / (1 + 1 / 3))                # Eq. 36
     assert np.isclose(d["v2_pq"], 2 * 0.25 / 1.25)
+
+
+def test_tolerant_overlap_count():
+    """PAPER.md:234, reading R-13b: coincident strings and strings displaced by ONE cell (also diagonally) give the
+    same tolerant length, strings two cells apart give none; brute force on random sparse cell arrays."""
+    shape = (8, 8, 8)
+    lines = [((1.5, 3.5), +1), ((5.5, 3.5), -1)]
+    for q_lines, exact, tol in (
+            (lines, 16, 16),
+            ([((2.5, 3.5), +1), ((6.5, 3.5), -1)], 0, 16),          # one cell along x
+            ([((2.5, 4.5), +1), ((6.5, 2.5), -1)], 0, 16),          # one cell along the diagonal
+            ([((3.5, 3.5), +1), ((7.5, 3.5), -1)], 0, 0)):          # two cells: out of reach
+        d = O.diagnostics(line_state(shape, lines, q_lines), 1.0, K0, 1.0)
+        assert d["cells_pq"] == exact
+        assert d["cells_pq_tol_p"] == tol and d["cells_pq_tol_q"] == tol and d["L_pq_tol"] == float(tol)
+    rng = np.random.default_rng(3)
+    n = 6
+    Cp = (rng.random((n, n, n)) < 0.08).astype(np.int32) * 2
+    Cq = (rng.random((n, n, n)) < 0.08).astype(np.int32) * 2
+    want_p = want_q = 0
+    for z in range(n):
+        for y in range(n):
+            for x in range(n):
+                nb = [((z + c) % n, (y + b) % n, (x + a) % n) for c in (-1, 0, 1) for b in (-1, 0, 1) for a in (-1, 0, 1)]
+                want_p += Cp[z, y, x] > 0 and any(Cq[i] > 0 for i in nb)
+                want_q += Cq[z, y, x] > 0 and any(Cp[i] > 0 for i in nb)
+    assert O.cells_pq_tolerant(Cp, Cq) == (want_p, want_q) and want_p + want_q > 0
