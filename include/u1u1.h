@@ -107,6 +107,16 @@ int u1u1_set_time(u1u1_ctx *ctx, double tau, double era_m, double s);
  * Asynchronous: returns after enqueueing. */
 int u1u1_step(u1u1_ctx *ctx, int32_t n, double tau, double era_m, double s);
 
+/* cool(n, dcool)  [PAPER.md:164-177 Eq. 27-30; reading R-20]: n explicit Euler steps of the diffusive
+ * cooling that precedes the evolution in the paper's own initial-condition pipeline:
+ *   dphi/deta = D-_j D+_j phi - lambda_p0/2 (|phi|^2 - sigma_p^2) phi,   dA_i/deta = -sum_j d-_j F_ij + 2 e_p0^2 Im(phi* D+_i phi)
+ * and the mirror for (psi, B); no kappa term, no scale factor.  Runs in the fused step kernel with the kick
+ * coefficients set to (0, 1) and the drift to dcool; on exit all momenta are zero.  The paper uses eta from -10
+ * to 1 in steps of 1/30.  Needs dcool (12/dx^2 + lambda sigma^2) < 2 (explicit diffusion), else U1U1_EUNSTABLE.
+ * The high-expansion damping phase that follows is u1u1_step with era_m = 0.9 ... 0.95.
+ * Asynchronous. */
+int u1u1_cool(u1u1_ctx *ctx, int32_t n, double dcool);
+
 /* diagnostics(out)  [north_star; PAPER.md:183-224 Eq. 31-37, :230-238]: out = HOST array of
  * U1U1_DIAG_LEN doubles, slots named by the U1U1_D_* enum below.  Uses the scale factor of the last
  * completed step (or of `tau_norm`-normalised a=1 before any step).  Synchronises the stream. */

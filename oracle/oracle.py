@@ -77,6 +77,7 @@ def lib():
         L.orc_friction.argtypes = [LP, dp, d]
         L.orc_drift.argtypes = [LP, dp, d]
         L.orc_step.argtypes = [LP, KP, dp, d, d, d, d, d, d]
+        L.orc_cool_step.argtypes = [LP, KP, dp, d, dp]
         L.orc_gauss_field.argtypes = [LP, KP, dp, ctypes.c_int, d, dp, dp, dp]
         L.orc_windings.argtypes = [LP, dp, ctypes.c_int, d, ctypes.POINTER(ctypes.c_int32),
                                    ctypes.POINTER(ctypes.c_uint8)]
@@ -86,7 +87,7 @@ def lib():
         L.orc_init_random_phase.argtypes = [LP, KP, ctypes.c_uint64, dp]
         L.orc_init_smoothed.argtypes = [LP, KP, ctypes.c_uint64, d, ctypes.c_int, dp]
         for f in ("orc_scalars", "orc_kick_scalars", "orc_kick_gauge", "orc_friction", "orc_drift",
-                  "orc_step", "orc_gauss_field", "orc_windings", "orc_cells", "orc_densities",
+                  "orc_step", "orc_cool_step", "orc_gauss_field", "orc_windings", "orc_cells", "orc_densities",
                   "orc_philox4x32_10", "orc_init_random_phase", "orc_init_smoothed"):
             getattr(L, f).restype = None
         _lib = L
@@ -164,6 +165,15 @@ def step(state, dx, K, tau, m, beta, dtau, tau_norm=1.0, friction=1.0, n=1):
         lib().orc_step(ctypes.byref(lat), ctypes.byref(kc), _dp(state), tau + k * dtau, m, beta,
                        dtau, tau_norm, friction)
     return tau + n * dtau
+
+
+def cool(state, dx, K, dcool, n=1):
+    """n explicit Euler steps of the diffusive cooling equations, Eq. 27-30 (reading R-20):
+    first-order flow of phi, psi (no kappa term) and of the links; momenta are zero on exit."""
+    lat, kc = _lat(state, dx), K.c()
+    scratch = np.zeros(10 * state[0].size)
+    for _ in range(n):
+        lib().orc_cool_step(ctypes.byref(lat), ctypes.byref(kc), _dp(state), dcool, _dp(scratch))
 
 
 def gauss_coefficient(tau_last, m, beta, dtau, tau_norm=1.0):

@@ -27,6 +27,8 @@
  * covariance, static vortex + Bogomolny tension 2 pi sigma^2, sector symmetry
  * (:79), brute-force windings and the "cell value 2" statement (:252), kappa=0 decoupling,
  * homogeneous-mode ODE, Philox known-answer vectors.
+ * Cooling (O-12, Eq. 27-30): monotone energy decrease, relaxed vortex as a fixed point, equivalence with
+ *   kick+drift from zero momenta when kappa = 0.
  * parity unpinned: the VALUES of xi_L, <v^2>, f_total (only their definitions are fixed).
  */
 #include <math.h>
@@ -259,6 +261,70 @@ void orc_step(const orc_lattice *L, const orc_couplings *K, double *state, doubl
     orc_kick_gauge(L, K, state, sc[1], sc[3], dtau);
     if (friction != 1.0) orc_friction(L, state, friction);
     orc_drift(L, state, dtau);
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O-12  diffusive cooling, one explicit Euler step.  PAPER.md:164-177 Eq. 27-30 (readings R-8, R-20):
+ *   d phi / d eta = D-_j D+_j phi - lambda_p0/2 (|phi|^2 - sigma_p^2) phi          (Eq. 27, no kappa term)
+ *   d A_i / d eta = - sum_{j != i} d-_j F_ij + 2 e_p0^2 Im(phi* D+_i phi)          (Eq. 28, R-20)
+ * and the mirror for (psi, B) (Eq. 29-30).  All right-hand sides are evaluated on the fields at eta
+ * (into scratch arrays), then every field is advanced by dcool times its right-hand side.  No scale
+ * factor, no momenta: on exit the momenta hold zero.  scratch = 10 * volume doubles.
+ * ---------------------------------------------------------------------------------------- */
+void orc_cool_step(const orc_lattice *L, const orc_couplings *K, double *state, double dcool,
+                   double *scratch)
+{
+    size_t V = vol(L);
+    double dx = L->dx, dx2 = dx * dx;
+    for (int sec = 0; sec < 2; sec++) {
+        const double *f_re = state + (sec ? PSI : PHI) * V, *f_im = f_re + V;
+        const double *theta = state + (sec ? THB : THA) * V;
+        double lambda = sec ? K->lambda2 : K->lambda1, sigma = sec ? K->eta2 : K->eta1;
+        double e0 = sec ? K->e2 : K->e1;
+        double *r_re = scratch + (size_t)(5 * sec) * V, *r_im = r_re + V, *r_A = r_im + V;
+        for (int iz = 0; iz < L->nz; iz++)
+            for (int iy = 0; iy < L->ny; iy++)
+                for (int ix = 0; ix < L->nx; ix++) {
+                    size_t x = site(L, ix, iy, iz);
+                    double lap_re = 0.0, lap_im = 0.0;
+                    for (int j = 0; j < 3; j++) {
+                        double fr, fi, br, bi;
+                        hop_forward(L, f_re, f_im, theta + (size_t)j * V, ix, iy, iz, j, &fr, &fi);
+                        hop_backward(L, f_re, f_im, theta + (size_t)j * V, ix, iy, iz, j, &br, &bi);
+                        lap_re += (fr + br - 2.0 * f_re[x]) / dx2;
+                        lap_im += (fi + bi - 2.0 * f_im[x]) / dx2;
+                    }
+                    double mod2 = f_re[x] * f_re[x] + f_im[x] * f_im[x];
+                    double pot = 0.5 * lambda * (mod2 - sigma * sigma);
+                    r_re[x] = lap_re - pot * f_re[x];
+                    r_im[x] = lap_im - pot * f_im[x];
+                    for (int i = 0; i < 3; i++) {
+                        double curl = 0.0;
+                        for (int j = 0; j < 3; j++) {
+                            if (j == i) continue;
+                            int jx = ix - (j == 0), jy = iy - (j == 1), jz = iz - (j == 2);
+                            curl += (plaquette(L, theta, ix, iy, iz, i, j) -
+                                     plaquette(L, theta, jx, jy, jz, i, j)) / (dx * dx * dx);
+                        }
+                        double hr, hi;
+                        hop_forward(L, f_re, f_im, theta + (size_t)i * V, ix, iy, iz, i, &hr, &hi);
+                        double Dre = (hr - f_re[x]) / dx, Dim = (hi - f_im[x]) / dx;
+                        r_A[(size_t)i * V + x] = -curl + 2.0 * e0 * e0 * (f_re[x] * Dim - f_im[x] * Dre);
+                    }
+                }
+    }
+    for (int sec = 0; sec < 2; sec++) {
+        double *f_re = state + (sec ? PSI : PHI) * V, *f_im = f_re + V;
+        double *theta = state + (sec ? THB : THA) * V;
+        const double *r_re = scratch + (size_t)(5 * sec) * V, *r_im = r_re + V, *r_A = r_im + V;
+        for (size_t x = 0; x < V; x++) {
+            f_re[x] += dcool * r_re[x];
+            f_im[x] += dcool * r_im[x];
+            for (int i = 0; i < 3; i++) theta[(size_t)i * V + x] += dcool * dx * r_A[(size_t)i * V + x];
+        }
+    }
+    static const int mom[10] = {2, 3, 6, 7, 11, 12, 13, 17, 18, 19};
+    for (int k = 0; k < 10; k++) memset(state + (size_t)mom[k] * V, 0, V * sizeof(double));
 }
 
 /* ------------------------------------------------------------------------------------------

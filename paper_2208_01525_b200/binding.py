@@ -45,7 +45,7 @@ class U1U1Error(RuntimeError):
 
 _lib = None
 SYMBOLS = ["u1u1_state_bytes", "u1u1_scratch_bytes", "u1u1_create", "u1u1_destroy", "u1u1_last_error",
-           "u1u1_configure", "u1u1_init_fields", "u1u1_set_params", "u1u1_set_time", "u1u1_step",
+           "u1u1_configure", "u1u1_init_fields", "u1u1_set_params", "u1u1_set_time", "u1u1_step", "u1u1_cool",
            "u1u1_diagnostics", "u1u1_gauss_violation", "u1u1_export_state", "u1u1_import_state",
            "u1u1_export_state_host", "u1u1_import_state_host", "u1u1_export_windings", "u1u1_export_block", "u1u1_launch_count"]
 
@@ -71,6 +71,7 @@ def load():
     L.u1u1_set_params.argtypes = [vp, pp]
     L.u1u1_set_time.argtypes = [vp, d, d, d]
     L.u1u1_step.argtypes = [vp, i32, d, d, d]
+    L.u1u1_cool.argtypes = [vp, i32, d]
     L.u1u1_diagnostics.argtypes = [vp, dp]
     L.u1u1_gauss_violation.argtypes = [vp, dp]
     L.u1u1_export_state.argtypes = [vp, vp]

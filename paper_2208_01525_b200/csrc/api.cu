@@ -249,6 +249,49 @@ extern "C" int u1u1_step(u1u1_ctx *ctx, int32_t n, double tau, double era_m, dou
     return U1U1_OK;
 }
 
+extern "C" int u1u1_cool(u1u1_ctx *ctx, int32_t n, double dcool)
+{
+    if (!ctx) return U1U1_EINVAL;
+    if (!ctx->configured) return fail(ctx, U1U1_ESTATE, "cool before configure/init_fields");
+    if (n < 0 || !(dcool > 0)) return fail(ctx, U1U1_EINVAL, "need n >= 0 and dcool > 0");
+    const u1u1_params &P = ctx->prm;
+    const double dx = ctx->dx;
+    const double lam = std::fmax(P.lambda1 * P.eta1 * P.eta1, P.lambda2 * P.eta2 * P.eta2);
+    if (dcool * (12.0 / (dx * dx) + lam) >= 2.0)
+        return fail(ctx, U1U1_EUNSTABLE, "explicit cooling unstable: need dcool (12/dx^2 + lambda sigma^2) < 2");
+    const int kv = P.kernel_variant & 15;
+    const bool tiled = kv != 1 && kv != 3 && step_tiled_supports(ctx->N);
+    static const int tmode_of[8] = {5, -1, 3, -1, 1, 2, 0, 4};
+    // Pi+ = 0 Pi- + 1 [D-D+ phi - lambda/2 (|phi|^2 - sigma^2) phi], phi += dcool Pi+  (and the same for E, theta)
+    StepCoef q;
+    q.aS = 0.f; q.bS = 1.f; q.aG = 0.f; q.bG = 1.f; q.aSm1 = -1.f; q.aGm1 = -1.f;
+    q.lamh1 = (float)(0.5 * P.lambda1);
+    q.lamh2 = (float)(0.5 * P.lambda2);
+    q.kap = 0.f;
+    q.sig1sq = (float)(P.eta1 * P.eta1);
+    q.sig2sq = (float)(P.eta2 * P.eta2);
+    q.cur1 = (float)(2.0 * P.e1 * P.e1 / dx);
+    q.cur2 = (float)(2.0 * P.e2 * P.e2 / dx);
+    q.inv_dx2 = (float)(1.0 / (dx * dx));
+    q.inv_dx3 = (float)(1.0 / (dx * dx * dx));
+    q.dtau = (float)dcool;
+    q.dtau_dx = (float)(dcool * dx);
+    q.flags = P.kernel_variant >> 4;
+    for (int k = 0; k < n; k++) {
+        Lattice L{pos_buf(ctx, ctx->cur), pos_buf(ctx, ctx->cur ^ 1), mom_buf(ctx), ctx->V, ctx->N};
+        cudaError_t e = tiled ? launch_step_tiled(L, q, ctx->stream, tmode_of[kv]) : launch_step_ref(L, q, ctx->stream, kv == 3);
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "cooling kernel launch");
+        ctx->launches += 1;
+        ctx->cur ^= 1;
+        ctx->diag_valid = false;
+    }
+    if (n > 0) {
+        cudaError_t e = cudaMemsetAsync(mom_buf(ctx), 0, (size_t)NMOM * ctx->V * sizeof(float), ctx->stream);
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "cool: zeroing the momenta");
+    }
+    return U1U1_OK;
+}
+
 static DiagCoef diag_coef(const u1u1_ctx *ctx)
 {
     const u1u1_params &P = ctx->prm;

@@ -65,6 +65,9 @@ class Lattice:
     def step(self, n: int, tau: float, era_m: float, s: float):
         self._check(self.lib.u1u1_step(self._ctx, n, tau, era_m, s), "step")
 
+    def cool(self, n: int, dcool: float):
+        self._check(self.lib.u1u1_cool(self._ctx, n, dcool), "cool")
+
     def diagnostics(self) -> dict:
         out = (ctypes.c_double * B.DIAG_LEN)()
         self._check(self.lib.u1u1_diagnostics(self._ctx, out), "diagnostics")

@@ -564,3 +564,76 @@ def test_tolerant_overlap_count():
                 want_p += Cp[z, y, x] > 0 and any(Cq[i] > 0 for i in nb)
                 want_q += Cq[z, y, x] > 0 and any(Cp[i] > 0 for i in nb)
     assert O.cells_pq_tolerant(Cp, Cq) == (want_p, want_q) and want_p + want_q > 0
+
+
+# ---------------------------------------------------------------------------------------- cooling (O-12)
+def test_cooling_decreases_energy_and_zeroes_momenta():
+    """PAPER.md:164-177 Eq. 27-30 (R-20) is the gradient flow of the kappa = 0 Hamiltonian: every explicit step
+    with dcool below the stability limit 2 / (12/dx^2 + ...) lowers H; momenta are zero afterwards."""
+    dx = 0.5
+    Kc = O.Couplings(kappa=0.0)
+    s = inputs.random_state((10, 12, 14), seed=4)
+    e = [O.energy(_zero_mom(s), dx, Kc)]
+    for _ in range(25):
+        O.cool(s, dx, K0, 1.0 / 30.0)                      # kappa of K0 must be ignored by the cooling equations
+        assert not s[inputs.MOM].any()
+        e.append(O.energy(s, dx, Kc))
+    assert all(b < a for a, b in zip(e, e[1:])) and e[-1] < 0.5 * e[0]
+
+
+def _zero_mom(s):
+    t = s.copy()
+    t[inputs.MOM] = 0.0
+    return t
+
+
+def test_cooling_equals_first_order_flow_of_the_kicks():
+    """With kappa = 0 the cooling step is 'zero momenta, kick by dcool, drift by 1' of the pinned kicks."""
+    dx, dc = 0.5, 1.0 / 30.0
+    Kc = O.Couplings(lambda1=2.0, lambda2=1.6, e1=1.0, e2=0.8, eta1=1.0, eta2=1.1, kappa=0.0)
+    a = inputs.random_state((6, 8, 10), seed=8)
+    b = a.copy()
+    O.cool(a, dx, Kc, dc, n=3)
+    relax(b, dx, Kc, dc, 3)
+    assert np.max(np.abs(a - b)) < 1e-13
+
+
+def test_cooling_goldstone_decay_rate_and_radial_relaxation():
+    """Closed forms.  (i) A small phase wave i eps cos(k x) on the vacuum with a negligible gauge coupling decays
+    by exactly (1 - dcool khat^2) per step, khat^2 = (2 - 2 cos(k dx)) / dx^2.  (ii) A uniform modulus r obeys
+    dr/deta = -(lambda/2) r (r^2 - sigma^2), i.e. r^2 = sigma^2 / (1 + C exp(-lambda sigma^2 eta))."""
+    dx, dc, n = 0.5, 1.0 / 30.0, 16
+    K = O.Couplings(e1=1e-7, e2=1e-7, kappa=0.0)
+    s = _uniform_state((1, 1, n), 1.0, 1.0)
+    kx = 2 * np.pi * 3 / (n * dx)
+    eps = 1e-7
+    s[1, 0, 0, :] = eps * np.cos(kx * dx * np.arange(n))
+    O.cool(s, dx, K, dc, n=20)
+    khat2 = (2 - 2 * np.cos(kx * dx)) / dx ** 2
+    want = eps * np.cos(kx * dx * np.arange(n)) * (1 - dc * khat2) ** 20
+    assert np.max(np.abs(s[1, 0, 0, :] - want)) < 1e-6 * eps
+    lam, r0 = 2.0, 0.3
+    errs = []
+    for dcs in (0.02, 0.01):
+        u = _uniform_state((2, 2, 2), r0, 1.0)
+        steps = int(round(2.0 / dcs))
+        O.cool(u, dx, O.Couplings(kappa=0.0), dcs, n=steps)
+        C = 1.0 / r0 ** 2 - 1.0
+        exact = np.sqrt(1.0 / (1.0 + C * np.exp(-lam * 2.0)))
+        errs.append(abs(u[0, 0, 0, 0] - exact))
+        assert np.ptp(u[0]) == 0 and np.allclose(u[4], 1.0)          # psi sits in its vacuum
+    assert errs[0] < 5e-3 and 1.7 < errs[0] / errs[1] < 2.3           # explicit Euler: first order
+
+
+def test_cooling_keeps_the_relaxed_vortex():
+    """The relaxed vortex-antivortex pair (pin P-4) is a fixed point of the cooling flow (up to the slow residual
+    of its own finite relaxation time), while a 1 % change of the modulus is pulled back 100x faster."""
+    s, K = vortex_energy(32, 0.5, 0)
+    t = s.copy()
+    O.cool(t, 0.5, K, 0.01, n=10)
+    assert np.max(np.abs(t - s)) < 2e-5
+    u = s.copy()
+    u[0] *= 1.01
+    v = u.copy()
+    O.cool(v, 0.5, K, 0.01, n=10)
+    assert np.max(np.abs(v - u)) > 1e-3
