@@ -147,6 +147,25 @@ int u1u1_export_block(u1u1_ctx *ctx, int32_t x0, int32_t y0, int32_t z0, int32_t
  * array uint8 C[N][N][N].  DEVICE destinations; any of them may be NULL. */
 int u1u1_export_windings(u1u1_ctx *ctx, int32_t sector, void *w_dev, void *near_dev, void *cells_dev);
 
+/* pq_segments(min_cells, tolerant, out)  [PAPER.md:240-256, :390-394 "robust method"; reading R-21]:
+ * after u1u1_diagnostics on the current state, label the connected regions (periodic 26-neighbourhood) of the
+ * cells pierced by both string types -- exact overlap (tolerant = 0) or one cell of tolerance
+ * (tolerant = 1, R-13b) -- and reduce them to out = HOST array of U1U1_SEG_LEN doubles:
+ *   [0] N_pq     number of segments with at least min_cells cells          (Eq. 38)
+ *   [1] L_pq     dx * sum over those segments of (N_cells - 1)             (off-by-one corrected)
+ *   [2] l_pq     L_pq / N_pq (0 if there is none)                           (Eq. 38)
+ *   [3] cells in those segments   [4] number of all segments   [5] number of all pq cells
+ *   [6] cells of the largest segment   [7] 0
+ * The paper's production threshold is N_cells > 41 (min_cells = 42, L_pq > 20), Fig. 1 uses l_pq >= 3.5 (min_cells = 8).
+ * Overwrites the winding / cell scratch arrays (u1u1_export_windings needs a new u1u1_diagnostics afterwards).
+ * Synchronises the stream. */
+#define U1U1_SEG_LEN 8
+int u1u1_pq_segments(u1u1_ctx *ctx, int32_t min_cells, int32_t tolerant, double *out_host);
+
+/* After u1u1_pq_segments: int32 label[N][N][N] to a DEVICE buffer: -1 where the cell is not a pq cell, else the
+ * linear index (x + N (y + N z)) of the smallest cell of its segment. */
+int u1u1_export_labels(u1u1_ctx *ctx, void *labels_dev);
+
 /* Number of kernel launches issued by this context so far (for bench.py's gpu_launches). */
 uint64_t u1u1_launch_count(const u1u1_ctx *ctx);
 

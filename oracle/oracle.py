@@ -238,6 +238,53 @@ def cells_pq_tolerant(Cp, Cq):
     return int(np.sum(p & dilate(q))), int(np.sum(q & dilate(p)))
 
 
+def pq_mask(Cp, Cq, tolerant=False):
+    """Cells counted as pierced by a pq string: exact overlap, or with one cell of tolerance (R-13b):
+    a pierced cell of either type with a pierced cell of the other type in its periodic 3x3x3 neighbourhood."""
+    p, q = Cp > 0, Cq > 0
+    if not tolerant:
+        return p & q
+    def dilate(mask):
+        out = np.zeros_like(mask)
+        for dz in (-1, 0, 1):
+            for dy in (-1, 0, 1):
+                for dx_ in (-1, 0, 1):
+                    out |= np.roll(mask, (dz, dy, dx_), axis=(0, 1, 2))
+        return out
+    return (p & dilate(q)) | (q & dilate(p))
+
+
+def pq_segments(Cp, Cq, dx, min_cells=1, tolerant=False):
+    """The robust method's numbers (reading R-21) by plain flood fill: connected regions
+    of pq cells over the periodic 26-neighbourhood; N_pq = regions with >= min_cells cells, L_pq = dx sum (N_cells - 1)
+    over them (:248), l_pq = L_pq / N_pq (Eq. 38).  Returns (dict, sorted list of all region sizes)."""
+    mask = pq_mask(Cp, Cq, tolerant)
+    nz, ny, nx = mask.shape
+    seen = np.zeros(mask.shape, dtype=bool)
+    sizes = []
+    for start in zip(*np.nonzero(mask)):
+        if seen[start]:
+            continue
+        seen[start] = True
+        stack, n = [start], 0
+        while stack:
+            z, y, x = stack.pop()
+            n += 1
+            for dz in (-1, 0, 1):
+                for dy in (-1, 0, 1):
+                    for dx_ in (-1, 0, 1):
+                        c = ((z + dz) % nz, (y + dy) % ny, (x + dx_) % nx)
+                        if mask[c] and not seen[c]:
+                            seen[c] = True
+                            stack.append(c)
+        sizes.append(n)
+    kept = [n for n in sizes if n >= min_cells]
+    L = dx * sum(n - 1 for n in kept)
+    out = {"N_pq": len(kept), "L_pq": L, "l_pq": L / len(kept) if kept else 0.0, "cells_kept": sum(kept),
+           "segments_all": len(sizes), "cells_all": int(mask.sum()), "largest": max(sizes) if sizes else 0}
+    return out, sorted(sizes)
+
+
 def densities(state, dx, K):
     """dict of per-site arrays kin, grad, elec, mag, pot, vint (no scale-factor weights)."""
     lat, kc = _lat(state, dx), K.c()

@@ -14,6 +14,8 @@ LIB_PATH = os.path.join(HERE, "libu1u1.so")
 
 DIAG_LEN = 48
 GAUSS_LEN = 8
+SEG_LEN = 8
+SEG_SLOTS = ["N_pq", "L_pq", "l_pq", "cells_kept", "segments_all", "cells_all", "largest"]
 DIAG_SLOTS = ["tau", "a", "c", "sumW_p", "sumW_q", "cells_p", "cells_q", "cells_pq", "near_p", "near_q",
               "maxW", "sum_L", "sum_kin_L", "sum_grad_L", "sum_kin_V", "sum_grad_V", "sum_vint", "sum_kin",
               "sum_grad", "sum_elec", "sum_mag", "sum_pot", "L_p", "L_q", "L_pq", "xi_p", "xi_q", "xi_pq",
@@ -47,7 +49,7 @@ _lib = None
 SYMBOLS = ["u1u1_state_bytes", "u1u1_scratch_bytes", "u1u1_create", "u1u1_destroy", "u1u1_last_error",
            "u1u1_configure", "u1u1_init_fields", "u1u1_set_params", "u1u1_set_time", "u1u1_step", "u1u1_cool",
            "u1u1_diagnostics", "u1u1_gauss_violation", "u1u1_export_state", "u1u1_import_state",
-           "u1u1_export_state_host", "u1u1_import_state_host", "u1u1_export_windings", "u1u1_export_block", "u1u1_launch_count"]
+           "u1u1_export_state_host", "u1u1_import_state_host", "u1u1_export_windings", "u1u1_export_block", "u1u1_launch_count", "u1u1_pq_segments", "u1u1_export_labels"]
 
 
 def load():
@@ -80,6 +82,8 @@ def load():
     L.u1u1_import_state_host.argtypes = [vp, vp]
     L.u1u1_export_windings.argtypes = [vp, i32, vp, vp, vp]
     L.u1u1_export_block.argtypes = [vp, i32, i32, i32, i32, i32, i32, vp]
+    L.u1u1_pq_segments.argtypes = [vp, i32, i32, dp]
+    L.u1u1_export_labels.argtypes = [vp, vp]
     L.u1u1_launch_count.argtypes = [vp]; L.u1u1_launch_count.restype = u64
     _lib = L
     return L

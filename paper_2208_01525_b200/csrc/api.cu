@@ -29,6 +29,7 @@ struct u1u1_ctx {
     double tau_pos = 0.0;        // conformal time of the positions
     double a = 1.0, c = 1.0, cG = 1.0;
     bool diag_valid = false;     // scratch holds windings of the current state
+    bool labels_valid = false;   // scratch holds segment labels of the current state
     uint64_t launches = 0;
     std::string err;
 };
@@ -131,6 +132,7 @@ extern "C" int u1u1_configure(u1u1_ctx *ctx, int32_t N, double dx, const u1u1_pa
     ctx->tau_pos = params->tau_norm;
     ctx->a = ctx->c = ctx->cG = 1.0;
     ctx->diag_valid = false;
+    ctx->labels_valid = false;
     return U1U1_OK;
 }
 
@@ -245,6 +247,7 @@ extern "C" int u1u1_step(u1u1_ctx *ctx, int32_t n, double tau, double era_m, dou
         ctx->c = c1;
         ctx->cG = c * (1.0 + delta) / (1.0 + omega);
         ctx->diag_valid = false;
+    ctx->labels_valid = false;
     }
     return U1U1_OK;
 }
@@ -284,6 +287,7 @@ extern "C" int u1u1_cool(u1u1_ctx *ctx, int32_t n, double dcool)
         ctx->launches += 1;
         ctx->cur ^= 1;
         ctx->diag_valid = false;
+    ctx->labels_valid = false;
     }
     if (n > 0) {
         cudaError_t e = cudaMemsetAsync(mom_buf(ctx), 0, (size_t)NMOM * ctx->V * sizeof(float), ctx->stream);
@@ -350,6 +354,7 @@ extern "C" int u1u1_diagnostics(u1u1_ctx *ctx, double *out)
     double r[32];
     if (int rc = fetch(ctx, r, 32)) return rc;
     ctx->diag_valid = true;
+    ctx->labels_valid = false;
     memset(out, 0, U1U1_DIAG_LEN * sizeof(double));
     const double dx = ctx->dx, vol = (double)V * dx * dx * dx;
     out[U1U1_D_TAU] = ctx->tau_pos;
@@ -394,7 +399,10 @@ static int relayout(u1u1_ctx *ctx, float *canon, int to_canonical)
     cudaError_t e = launch_relayout(pos_buf(ctx, ctx->cur), mom_buf(ctx), canon, ctx->V, 0, 20, to_canonical, ctx->stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "relayout kernel launch");
     ctx->launches += 1;
-    if (!to_canonical) ctx->diag_valid = false;
+    if (!to_canonical) {
+        ctx->diag_valid = false;
+        ctx->labels_valid = false;
+    }
     return U1U1_OK;
 }
 
@@ -434,6 +442,7 @@ static int host_copy(u1u1_ctx *ctx, void *host, int to_host)
     const size_t V = ctx->V, bytes = V * sizeof(float);
     float *stage = (float *)ctx->scratch;                 // scratch >= 8 V bytes >= one component plane
     ctx->diag_valid = false;
+    ctx->labels_valid = false;
     for (int c = 0; c < 20; c++) {
         float *buf = stage;
         float *h = (float *)host + (size_t)c * V;
@@ -465,6 +474,43 @@ extern "C" int u1u1_import_state_host(u1u1_ctx *ctx, const void *src_host)
     if (!ctx || !src_host) return ctx ? fail(ctx, U1U1_EINVAL, "src is NULL") : U1U1_EINVAL;
     if (!ctx->configured) return fail(ctx, U1U1_ESTATE, "import_state_host before configure");
     return host_copy(ctx, const_cast<void *>(src_host), 0);
+}
+
+extern "C" int u1u1_pq_segments(u1u1_ctx *ctx, int32_t min_cells, int32_t tolerant, double *out)
+{
+    if (!ctx || !out) return ctx ? fail(ctx, U1U1_EINVAL, "out is NULL") : U1U1_EINVAL;
+    if (min_cells < 1 || (tolerant != 0 && tolerant != 1)) return fail(ctx, U1U1_EINVAL, "need min_cells >= 1 and tolerant in {0, 1}");
+    if (!ctx->diag_valid) return fail(ctx, U1U1_ESTATE, "pq_segments needs u1u1_diagnostics on the current state first");
+    const size_t V = ctx->V;
+    // scratch: [codes 6V | cells 2V] -> [labels 4V | sizes 4V] (the sizes overlap the cells: zeroed after the mask is taken)
+    int *label = (int *)ctx->scratch, *size = (int *)(ctx->scratch + 4 * V);
+    cudaError_t e = launch_segments(ctx->scratch + 6 * V, V, ctx->N, tolerant, min_cells, label, size, partials(ctx),
+                                    result(ctx), ctx->stream);
+    ctx->diag_valid = false;
+    ctx->labels_valid = false;
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "pq_segments kernel launch");
+    ctx->launches += 5;
+    double r[6];
+    if (int rc = fetch(ctx, r, 6)) return rc;
+    ctx->labels_valid = true;
+    memset(out, 0, U1U1_SEG_LEN * sizeof(double));
+    out[0] = r[0];
+    out[1] = ctx->dx * r[1];
+    out[2] = r[0] > 0 ? out[1] / r[0] : 0.0;
+    out[3] = r[2];
+    out[4] = r[3];
+    out[5] = r[4];
+    out[6] = r[5];
+    return U1U1_OK;
+}
+
+extern "C" int u1u1_export_labels(u1u1_ctx *ctx, void *labels_dev)
+{
+    if (!ctx || !labels_dev) return ctx ? fail(ctx, U1U1_EINVAL, "dst is NULL") : U1U1_EINVAL;
+    if (!ctx->labels_valid) return fail(ctx, U1U1_ESTATE, "export_labels needs u1u1_pq_segments on the current state first");
+    cudaError_t e = cudaMemcpyAsync(labels_dev, ctx->scratch, ctx->V * sizeof(int), cudaMemcpyDeviceToDevice, ctx->stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "labels copy");
+    return U1U1_OK;
 }
 
 extern "C" int u1u1_export_windings(u1u1_ctx *ctx, int32_t sector, void *w_dev, void *near_dev, void *cells_dev)

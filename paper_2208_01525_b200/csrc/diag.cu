@@ -335,6 +335,12 @@ int red_blocks(size_t V)
 
 }  // namespace
 
+cudaError_t launch_fold(const double *partials, int nblocks, int nval, int n_sum, double *result, cudaStream_t st)
+{
+    fold_kernel<<<1, RED_BLOCK, 0, st>>>(partials, nblocks, nval, n_sum, result);
+    return cudaGetLastError();
+}
+
 cudaError_t launch_gauss(const float *pos, const float *mom, size_t V, int N, const DiagCoef &k,
                          double *partials, double *result, cudaStream_t st)
 {

@@ -19,6 +19,10 @@ cudaError_t launch_densities(const float *pos, const float *mom, size_t V, int N
 cudaError_t launch_decode_windings(const uint8_t *codes, size_t n, int8_t *w_out, uint8_t *near_out,
                                    cudaStream_t st);
 
+// segments.cu: connected components of the pq cells (labels = root site index, -1 = not a pq cell)
+cudaError_t launch_segments(const uint8_t *cells, size_t V, int N, int tolerant, int min_cells, int *label, int *size,
+                            double *partials, double *result, cudaStream_t st);
+
 // init.cu
 cudaError_t launch_init_random_phase(float *pos, size_t V, uint64_t seed, double eta1, double eta2,
                                      cudaStream_t st);

@@ -108,6 +108,17 @@ class Lattice:
         self.stream.synchronize()
         return W, near, cells
 
+    def pq_segments(self, min_cells: int = 1, tolerant: bool = False) -> dict:
+        out = (ctypes.c_double * B.SEG_LEN)()
+        self._check(self.lib.u1u1_pq_segments(self._ctx, min_cells, int(tolerant), out), "pq_segments")
+        return {k: out[i] for i, k in enumerate(B.SEG_SLOTS)}
+
+    def export_labels(self):
+        t = self._torch.empty((self.N, self.N, self.N), dtype=self._torch.int32, device=self.device)
+        self._check(self.lib.u1u1_export_labels(self._ctx, t.data_ptr()), "export_labels")
+        self.stream.synchronize()
+        return t
+
     def export_block(self, x0, y0, z0, bx, by, bz):
         t = self._torch.empty((20, bz, by, bx), dtype=self._torch.float32, device=self.device)
         self._check(self.lib.u1u1_export_block(self._ctx, x0, y0, z0, bx, by, bz, t.data_ptr()), "export_block")

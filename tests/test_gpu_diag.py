@@ -153,3 +153,34 @@ def test_known_vortex_lines_on_gpu():
     W, near, cells = lat.export_windings(0)
     assert int(cells.max()) == 2 and int((cells == 2).sum()) == 2 * N
     assert bool((W[0, :, 7, 3] == 1).all()) and bool((W[0, :, 7, 11] == -1).all())
+
+
+@pytest.mark.parametrize("tolerant", [False, True])
+@pytest.mark.parametrize("N,nsteps,f", [(48, 40, 1.0), (64, 150, 0.5), (96, 200, 0.5)])
+def test_pq_segments_match_oracle(N, nsteps, f, tolerant):
+    """Connected-component labelling of the pq cells (robust method; R-21): integer work, so the
+    GPU must reproduce the oracle's flood fill on the GPU's own cell arrays exactly -- segment count, lengths with
+    and without threshold, and the partition itself (same multiset of region sizes, labels = smallest site index)."""
+    lat, snap = evolved_snapshot(N, 5 + N, nsteps, s=0.0, friction=f)   # f = 1: one giant region; damped: many segments
+    lat.diagnostics()
+    cells = [lat.export_windings(sec)[2].cpu().numpy().astype(np.int32) for sec in (0, 1)]
+    ref_all, sizes = O.pq_segments(cells[0], cells[1], DX, 1, tolerant)
+    seg = lat.pq_segments(1, tolerant)
+    assert {k: seg[k] for k in ref_all} == {k: float(v) for k, v in ref_all.items()}
+    lab = lat.export_labels().cpu().numpy()
+    mask = O.pq_mask(cells[0], cells[1], tolerant)
+    assert np.array_equal(lab >= 0, mask) and len(sizes) >= (1 if f == 1.0 else 4), sizes[-5:]
+    roots, counts = np.unique(lab[lab >= 0], return_counts=True)
+    assert sorted(counts.tolist()) == sizes
+    flat = lab.ravel()
+    assert np.array_equal(flat[roots], roots)                          # a root labels itself ...
+    assert all(r == np.flatnonzero(flat == r)[0] for r in roots[:50])  # ... and is the smallest index of its region
+    # threshold (needs a fresh diagnostics: the labelling reuses the winding scratch)
+    lat.diagnostics()
+    thr = max(2, sizes[len(sizes) // 2])
+    ref_thr, _ = O.pq_segments(cells[0], cells[1], DX, thr, tolerant)
+    seg = lat.pq_segments(thr, tolerant)
+    assert {k: seg[k] for k in ref_thr} == {k: float(v) for k, v in ref_thr.items()}
+    from paper_2208_01525_b200 import U1U1Error
+    with pytest.raises(U1U1Error, match="ESTATE"):
+        lat.pq_segments(1, tolerant)                                   # scratch was consumed

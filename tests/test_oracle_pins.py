@@ -637,3 +637,44 @@ def test_cooling_keeps_the_relaxed_vortex():
     v = u.copy()
     O.cool(v, 0.5, K, 0.01, n=10)
     assert np.max(np.abs(v - u)) > 1e-3
+
+
+# ---------------------------------------------------------------------------------------- pq segments (R-21)
+def test_pq_segments_on_hand_built_regions():
+    """PAPER.md:248 L_pq = (N_cells - 1) dx per region, Eq. 38 l_pq = L_pq / N_pq, threshold on N_cells (:250)."""
+    n = 12
+    Cp = np.zeros((n, n, n), dtype=np.int32)
+    Cq = np.zeros((n, n, n), dtype=np.int32)
+    for z in range(2, 9):                      # a straight 7-cell segment
+        Cp[z, 3, 3] = Cq[z, 3, 3] = 2
+    for k in range(4):                         # a 4-cell diagonal staircase: cells touch only at corners
+        Cp[k + 1, k + 6, k + 6] = Cq[k + 1, k + 6, k + 6] = 2
+    Cp[0, 0, 11] = Cq[0, 0, 11] = 2            # a region that wraps around the periodic box: 3 cells
+    Cp[11, 11, 0] = Cq[11, 11, 0] = 2
+    Cp[0, 11, 0] = Cq[0, 11, 0] = 2
+    Cp[6, 0, 6] = 2                            # pierced by p only: not a pq cell
+    out, sizes = O.pq_segments(Cp, Cq, 0.5)
+    assert sizes == [3, 4, 7] and out["N_pq"] == 3 and out["L_pq"] == 0.5 * (2 + 3 + 6)
+    assert np.isclose(out["l_pq"], 0.5 * 11 / 3) and out["largest"] == 7 and out["cells_all"] == 14
+    out, _ = O.pq_segments(Cp, Cq, 0.5, min_cells=4)
+    assert out["N_pq"] == 2 and out["L_pq"] == 0.5 * (3 + 6) and out["cells_kept"] == 11 and out["segments_all"] == 3
+    # one cell of tolerance: q displaced by one cell from a p line -> both lines' cells form ONE region
+    Cp[:] = 0; Cq[:] = 0
+    Cp[2:9, 3, 3] = 2
+    Cq[2:9, 3, 4] = 2
+    assert O.pq_segments(Cp, Cq, 0.5)[1] == []
+    out, sizes = O.pq_segments(Cp, Cq, 0.5, tolerant=True)
+    assert sizes == [14] and out["N_pq"] == 1
+
+
+def test_pq_segments_against_library_labelling():
+    """Away from the periodic boundary the flood fill must agree with scipy.ndimage.label (26-connectivity)."""
+    from scipy import ndimage
+    rng = np.random.default_rng(12)
+    n = 14
+    m = rng.random((n, n, n)) < 0.07
+    m[0] = m[-1] = False; m[:, 0] = m[:, -1] = False; m[:, :, 0] = m[:, :, -1] = False
+    C = m.astype(np.int32) * 2
+    _, sizes = O.pq_segments(C, C, 1.0)
+    lab, num = ndimage.label(m, structure=np.ones((3, 3, 3)))
+    assert sizes == sorted(np.bincount(lab.ravel())[1:].tolist()) and num == len(sizes) and num > 5
