@@ -183,3 +183,31 @@ def test_growth_then_physical_schedule():
     assert max(err.values()) < 1e-4, err
     d = lat.diagnostics()
     assert np.isclose(d["a"], 1.0) and np.isclose(d["tau"], tau_end)     # width normalised to 1 at the end
+
+
+@pytest.mark.parametrize("config", [2, 3, 4, 5])
+def test_baseline_configs_first_32_steps(config):
+    """BASELINE.json configs 2-5 at 64^3 (their own seeds, initial conditions, eras, s, tau_norm and friction
+    prephase as scheduled by paper_2208_01525_b200.run_config): the first 32 steps against the oracle from the
+    oracle's OWN seeded initial condition (so the generator, the coefficients and the kernel are all in the loop)."""
+    from paper_2208_01525_b200 import Lattice, Params
+    from paper_2208_01525_b200.run_config import CONFIGS, TAU0
+    c = CONFIGS[config]
+    N, n = 64, 32
+    total = c["pre"] + c["steps"]
+    tau_norm = c["tau_norm"] if c["tau_norm"] is not None else TAU0 + total * DTAU
+    f = 0.5 if c["pre"] else 1.0
+    K = O.Couplings()
+    ref = O.init_smoothed(N, config) if c["kind"] == 1 else O.init_random_phase(N, config)
+    ref = inputs.to_f32_exact(ref)
+    lat = Lattice(N)
+    lat.init_fields(config, DX, Params(init_kind=c["kind"], tau_norm=tau_norm, friction=f))
+    g0 = lat.export_state().cpu().numpy().astype(np.float64)
+    assert np.max(np.abs(g0 - ref)) < (2e-4 if c["kind"] == 1 else 2e-7)
+    if c["kind"] == 1:
+        ref = g0.copy()          # smoothed noise: fp32 intermediates on the GPU (tested in test_gpu_diag); same start for the step parity
+    lat.step(n, TAU0, c["m"], c["s"])
+    O.step(ref, DX, K, TAU0, c["m"], c["s"], DTAU, tau_norm=tau_norm, friction=f, n=n)
+    gpu = lat.export_state().cpu().numpy().astype(np.float64)
+    err = group_errors(gpu, ref)
+    assert max(err.values()) < 1e-3, err
