@@ -440,9 +440,11 @@ step_tiled_kernel(Lattice L, StepCoef k, int zchunk, const __grid_constant__ Ste
 
 int pick_zchunk(int N)
 {
-    // enough CTAs to fill 148 SMs x 3 several times over, chunks long enough to amortise the 2-plane prologue
+    // enough CTAs to fill 148 SMs x 3 several times over, chunks long enough to amortise the 2-plane prologue --
+    // but no longer: neighbouring CTAs drift apart while they march, and a halo line that the neighbour fetched
+    // too long ago has left L2 (measured at 1024^3: 16-32 planes 29.8 ms, 64: 30.6, 128: 32.3, 512: 34.6)
     const int tiles = ((N + TX - 1) / TX) * ((N + TY - 1) / TY);
-    int zc = 64;
+    int zc = 32;
     while (zc > 8 && (long)tiles * ((N + zc - 1) / zc) < 148L * 3 * 4) zc >>= 1;
     return zc < N ? zc : N;
 }
