@@ -205,19 +205,23 @@ __global__ void __launch_bounds__(RED_BLOCK) overlap_tol_kernel(const uint8_t *c
          lin += (size_t)gridDim.x * blockDim.x) {
         const int cp = cells[lin], cq = cells[V + lin];
         if ((cp | cq) == 0) continue;
+        if (cp > 0 && cq > 0) {                // exact overlap: both counts, no search
+            acc[0] += 1.0;
+            acc[1] += 1.0;
+            continue;
+        }
+        // pierced by one type only: look for the OTHER type in the 3x3x3 neighbourhood, stop at the first hit
         int x, y, z;
         site_xyz(lin, N, x, y, z);
         const int xs[3] = {w.m(x), x, w.p(x)}, ys[3] = {w.m(y), y, w.p(y)}, zs[3] = {w.m(z), z, w.p(z)};
-        int anyp = 0, anyq = 0;
-        for (int c = 0; c < 3; c++)
-            for (int b = 0; b < 3; b++)
-                for (int a = 0; a < 3; a++) {
-                    const size_t nb = w.at(xs[a], ys[b], zs[c]);
-                    anyp |= cells[nb];
-                    anyq |= cells[V + nb];
-                }
-        acc[0] += (cp > 0 && anyq > 0);
-        acc[1] += (cq > 0 && anyp > 0);
+        const uint8_t *other = cells + (cp > 0 ? V : 0);
+        int found = 0;
+        for (int c = 0; c < 3 && !found; c++)
+            for (int b = 0; b < 3 && !found; b++) {
+                const size_t row = (size_t)N * ((size_t)ys[b] + (size_t)N * zs[c]);
+                found = other[row + xs[0]] | other[row + xs[1]] | other[row + xs[2]];
+            }
+        if (found) acc[cp > 0 ? 0 : 1] += 1.0;
     }
     block_reduce_store<2>(acc, 2, partials);
 }

@@ -512,12 +512,9 @@ bool get_maps(const Lattice &L, StepMaps &out)
 template <bool FAST, typename R, bool DIFF>
 cudaError_t launch_one(const Lattice &L, StepCoef k, cudaStream_t st)
 {
-    static bool configured = false;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(step_tiled_kernel<FAST, R, DIFF>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
-        if (e != cudaSuccess) return e;
-        configured = true;
-    }
+    // per device and cheap: set on every launch rather than caching a per-process flag
+    cudaError_t ea = cudaFuncSetAttribute(step_tiled_kernel<FAST, R, DIFF>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+    if (ea != cudaSuccess) return ea;
     StepMaps maps;
     if (L.N < COLS + 2) {
         memset(&maps, 0, sizeof maps);

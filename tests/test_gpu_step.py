@@ -211,3 +211,18 @@ def test_baseline_configs_first_32_steps(config):
     gpu = lat.export_state().cpu().numpy().astype(np.float64)
     err = group_errors(gpu, ref)
     assert max(err.values()) < 1e-3, err
+
+
+@pytest.mark.parametrize("base", [0, 2, 4])
+def test_staging_paths_bit_identical(base):
+    """The tiled kernel stages interior tiles by TMA boxes and boundary tiles by cp.async, momenta by TMA boxes or
+    ld.global.cs: the arithmetic is the same, so forcing the other staging path (tuning flags 2 and 4 in bits 4.. of
+    kernel_variant) must give the bit-identical state -- on a lattice with interior, boundary and ragged tiles."""
+    from paper_2208_01525_b200 import Params
+    N = 132
+    s0 = inputs.to_f32_exact(inputs.random_state((N, N, N), seed=31))
+    outs = []
+    for flags in (0, 2, 4):
+        out, _ = run_gpu(s0, N, Params(kernel_variant=base + 16 * flags, tau_norm=1.5), [(3, 2.0, 0.5, 1.0)])
+        outs.append(out)
+    assert np.array_equal(outs[0], outs[1]) and np.array_equal(outs[0], outs[2])
