@@ -247,25 +247,27 @@ __global__ void __launch_bounds__(RED_BLOCK) density_kernel(const float *pos, co
         const float2 Cc = PC[lin], Cn[2] = {PC[nb[0]], PC[nb[1]]};
         const float4 ma = MA[lin], mb = MB[lin];
         const float2 mc = MC[lin];
-        double kin = 0, grad = 0, elec = 0, mag = 0, m2[2];
+        // per-site terms in fp32 (each a sum of <= 18 squares), everything that is accumulated over the lattice in fp64
+        float kin = 0.f, grad = 0.f, elec = 0.f, mag = 0.f, m2[2];
+        const float inv_dx2 = (float)k.inv_dx2;
 #pragma unroll
         for (int s = 0; s < 2; s++) {
             const float fr = s ? Ac.z : Ac.x, fi = s ? Ac.w : Ac.y;
             const float pr = s ? ma.z : ma.x, pi = s ? ma.w : ma.y;
-            const double inv2e2 = 1.0 / (2.0 * (s ? k.e2 * k.e2 : k.e1 * k.e1));
-            kin += (double)pr * pr + (double)pi * pi;
-            m2[s] = (double)fr * fr + (double)fi * fi;
+            const float inv2e2 = (float)(1.0 / (2.0 * (s ? k.e2 * k.e2 : k.e1 * k.e1)));
+            kin += pr * pr + pi * pi;
+            m2[s] = fr * fr + fi * fi;
             const float thc[3] = {s ? Bc.z : Bc.x, s ? Bc.w : Bc.y, s ? Cc.y : Cc.x};
             const float ev[3] = {s ? mb.z : mb.x, s ? mb.w : mb.y, s ? mc.y : mc.x};
+            float g2 = 0.f, e2 = 0.f, f2 = 0.f;
 #pragma unroll
             for (int i = 0; i < 3; i++) {
                 float sn, cs;
                 sincosf(thc[i], &sn, &cs);
                 const float ar = s ? An[i].z : An[i].x, ai = s ? An[i].w : An[i].y;
                 const float dr = (cs * ar + sn * ai) - fr, di = (cs * ai - sn * ar) - fi;
-                grad += ((double)dr * dr + (double)di * di) * k.inv_dx2;
-                const double e = ev[i];
-                elec += e * e * inv2e2;
+                g2 += dr * dr + di * di;
+                e2 += ev[i] * ev[i];
             }
             // theta_j(x + i) for the three plaquettes (i, j) = (x,y), (x,z), (y,z) and theta_i(x + j)
             const float ty_x = s ? Bn[0].w : Bn[0].y, tx_y = s ? Bn[1].z : Bn[1].x;
@@ -273,15 +275,15 @@ __global__ void __launch_bounds__(RED_BLOCK) density_kernel(const float *pos, co
             const float tz_y = s ? Cn[1].y : Cn[1].x, ty_z = s ? Bn[2].w : Bn[2].y;
             const float Pl[3] = {thc[0] + ty_x - tx_y - thc[1], thc[0] + tz_x - tx_z - thc[2], thc[1] + tz_y - ty_z - thc[2]};
 #pragma unroll
-            for (int q = 0; q < 3; q++) {
-                const double F = (double)Pl[q] * k.inv_dx2;
-                mag += F * F * inv2e2;
-            }
+            for (int q = 0; q < 3; q++) f2 += Pl[q] * Pl[q];
+            grad += g2 * inv_dx2;
+            elec += e2 * inv2e2;
+            mag += f2 * (inv_dx2 * inv_dx2) * inv2e2;
         }
-        const double a2 = m2[0] - k.sig1sq, b2 = m2[1] - k.sig2sq;
+        const double a2 = (double)m2[0] - k.sig1sq, b2 = (double)m2[1] - k.sig2sq;
         const double vint = k.kappa * a2 * b2;
         const double pot = 0.25 * k.lam1 * a2 * a2 + 0.25 * k.lam2 * b2 * b2 - vint;
-        const double lag = kin - grad + (elec - mag) / k.c - k.c * pot;
+        const double lag = (double)kin - (double)grad + ((double)elec - (double)mag) / k.c - k.c * pot;
         acc[0] += lag;
         acc[1] += kin * lag;
         acc[2] += grad * lag;
