@@ -226,3 +226,18 @@ def test_staging_paths_bit_identical(base):
         out, _ = run_gpu(s0, N, Params(kernel_variant=base + 16 * flags, tau_norm=1.5), [(3, 2.0, 0.5, 1.0)])
         outs.append(out)
     assert np.array_equal(outs[0], outs[1]) and np.array_equal(outs[0], outs[2])
+
+
+@pytest.mark.parametrize("variant,tol", [(0, 2e-5), (7, 1e-5), (4, 2e-5)])
+def test_large_link_phases(variant, tol):
+    """Non-compact links far outside (-pi, pi] (|theta| up to ~40, reading R-9): the SFU phasor's error grows like
+    6e-8 |theta| (documented in step_tiled.cu), the libm variants stay at the 1e-5 bar."""
+    from paper_2208_01525_b200 import Params
+    N = 24
+    s0 = inputs.to_f32_exact(inputs.random_state((N, N, N), seed=3, amp_theta=12.0))
+    assert np.max(np.abs(s0[[8, 9, 10, 14, 15, 16]])) > 30
+    ref = s0.copy()
+    O.step(ref, DX, O.Couplings(), 1.0, 0.5, 1.0, DTAU, n=1)
+    gpu, _ = run_gpu(s0, N, Params(kernel_variant=variant), [(1, 1.0, 0.5, 1.0)])
+    err = group_errors(gpu, ref)
+    assert max(err.values()) < tol, err
