@@ -153,14 +153,20 @@ __device__ inline void set2(float2 &v, int i, float a) { if (i == 0) v.x = a; el
 // storage floor wherever the fields are smooth.
 template <bool FAST, typename R, bool DIFF>
 __global__ void __launch_bounds__(NTHREADS, sizeof(R) == 8 ? 2 : 3)
-step_tiled_kernel(Lattice L, StepCoef k, int zchunk, const __grid_constant__ StepMaps maps)
+step_tiled_kernel(Lattice L, StepCoef k, int zchunk, int band, const __grid_constant__ StepMaps maps)
 {
     extern __shared__ __align__(128) char smem[];
     const unsigned sbase = smem_u32(smem), bars = sbase + OFF_BARS;
     const int N = L.N;
     const size_t V = L.V, NN = (size_t)N * N;
     const int tid = threadIdx.x, tx = tid & (TX - 1), ty = tid / TX;
-    const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY, z0 = blockIdx.z * zchunk;
+    // 1-d grid, launch order = (tile x fastest, tile row within a band of `band` rows, z chunk, band): the CTAs that
+    // are resident together cover one band of tile rows of one z chunk, and the next wave continues with the NEXT
+    // chunk of the same band, whose two boundary planes the previous wave has just read
+    const int ntx = (N + TX - 1) / TX, nty = (N + TY - 1) / TY, nzc = (N + zchunk - 1) / zchunk;
+    const int full = ntx * band * nzc, bnd = blockIdx.x / full, rem = blockIdx.x - bnd * full;
+    const int rows = min(band, nty - bnd * band), bzc = rem / (ntx * rows), tl = rem - bzc * (ntx * rows);
+    const int x0 = (tl % ntx) * TX, y0 = (bnd * band + tl / ntx) * TY, z0 = bzc * zchunk;
     const int wx = min(TX, N - x0), wy = min(TY, N - y0), nz = min(zchunk, N - z0);
     const bool active = tx < wx && ty < wy;
     // TMA boxes cannot wrap: only tiles whose halo lies inside the lattice take the TMA path (CTA-uniform)
@@ -441,10 +447,12 @@ step_tiled_kernel(Lattice L, StepCoef k, int zchunk, const __grid_constant__ Ste
 int pick_zchunk(int N)
 {
     // enough CTAs to fill 148 SMs x 3 several times over, chunks long enough to amortise the 2-plane prologue --
-    // but no longer: neighbouring CTAs drift apart while they march, and a halo line that the neighbour fetched
-    // too long ago has left L2 (measured at 1024^3: 16-32 planes 29.8 ms, 64: 30.6, 128: 32.3, 512: 34.6)
+    // but no longer: neighbouring CTAs drift apart while they march, and a halo line that the neighbour fetched too
+    // long ago has left L2.  With the band launch order below the two boundary planes of a chunk are re-read by the
+    // very next wave, so short chunks cost little (measured at 1024^3, band order: 8 planes 29.65 ms, 12: 29.2,
+    // 16: 29.05, 24: 29.25, 32: 29.45; plain 3-d grid order: 32: 29.8, 64: 30.6, 128: 32.3, 512: 34.6)
     const int tiles = ((N + TX - 1) / TX) * ((N + TY - 1) / TY);
-    int zc = 32;
+    int zc = 16;
     while (zc > 8 && (long)tiles * ((N + zc - 1) / zc) < 148L * 3 * 4) zc >>= 1;
     return zc < N ? zc : N;
 }
@@ -523,8 +531,13 @@ cudaError_t launch_one(const Lattice &L, StepCoef k, cudaStream_t st)
         return cudaErrorNotSupported;       // cuTensorMapEncodeTiled unavailable or rejected the layout: fail loudly
     }
     const int zc = pick_zchunk(L.N);
-    dim3 grid((L.N + TX - 1) / TX, (L.N + TY - 1) / TY, (L.N + zc - 1) / zc);
-    step_tiled_kernel<FAST, R, DIFF><<<grid, NTHREADS, SMEM_BYTES, st>>>(L, k, zc, maps);
+    const int ntx = (L.N + TX - 1) / TX, nty = (L.N + TY - 1) / TY, nzc = (L.N + zc - 1) / zc;
+    // band height = the tile rows one wave of resident CTAs covers (148 SMs x CTAs per SM / tiles per row)
+    const int per_sm = sizeof(R) == 8 ? 2 : 3;
+    int band = (k.flags & 8) ? nty : (148 * per_sm + ntx - 1) / ntx;     // tuning flag 8: the order of a plain 3-d grid
+    if (band > nty) band = nty;
+    const unsigned grid = (unsigned)ntx * nty * nzc;
+    step_tiled_kernel<FAST, R, DIFF><<<grid, NTHREADS, SMEM_BYTES, st>>>(L, k, zc, band, maps);
     return cudaGetLastError();
 }
 
