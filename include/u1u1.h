@@ -72,7 +72,8 @@ typedef struct {
 
 /* Bytes of device memory the caller must provide for an N^3 lattice.
  * state  : 30 fp32 words/site (20 fields + a second copy of the 10 position words, ping-pong).
- * scratch: winding codes (6 B/site), cell arrays (2 B/site), reduction partials. */
+ * scratch: winding codes (6 B/site) and cell arrays (2 B/site) -- reused as int32 segment labels and sizes by
+ *          u1u1_pq_segments and as a staging plane by the *_host copies -- plus the reduction partials. */
 size_t u1u1_state_bytes(int32_t N);
 size_t u1u1_scratch_bytes(int32_t N);
 

@@ -72,7 +72,8 @@ struct StepCoef {
     float dtau;            // drift of the scalars
     float dtau_dx;         // drift of the link phases: theta += dtau dx E
     float aSm1, aGm1;      // aS - 1, aG - 1 (rounded from fp64): Pi+ = Pi- + [(aS-1) Pi- + bS (...)] keeps ONE rounding at |Pi|
-    int flags;             // tuning switches of the tiled kernel (kernel_variant >> 4); 0 in production
+    int flags;             // tuning switches of the tiled kernel (kernel_variant >> 4), 0 in production:
+                           // 2 = no TMA (cp.async staging everywhere), 4 = momenta by ld.global.cs, 8 = plain grid order
 };
 
 // Coefficients of the diagnostic sweeps.
