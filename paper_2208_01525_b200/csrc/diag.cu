@@ -170,25 +170,38 @@ __global__ void __launch_bounds__(RED_BLOCK) winding_tiled_kernel(const float *p
 __global__ void __launch_bounds__(RED_BLOCK) cells_kernel(const uint8_t *codes, size_t V, int N,
                                                           uint8_t *cells, double *partials)
 {
+    // four consecutive x sites per thread (N is a multiple of 4): 32-bit loads of the code bytes
     const Wrap w{N};
     double acc[3] = {0, 0, 0};
-    for (size_t lin = (size_t)blockIdx.x * blockDim.x + threadIdx.x; lin < V;
-         lin += (size_t)gridDim.x * blockDim.x) {
+    auto mag = [](uint32_t word, int k) { return abs((int)((word >> (8 * k)) & 15u) - 8); };   // |W| of byte k
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < V / 4; q += (size_t)gridDim.x * blockDim.x) {
+        const size_t lin = 4 * q;
         int x, y, z;
         site_xyz(lin, N, x, y, z);
-        const size_t nx = w.at(w.p(x), y, z), ny = w.at(x, w.p(y), z), nz = w.at(x, y, w.p(z));
-        int C[2];
+        const size_t ny = w.at(x, w.p(y), z), nz = w.at(x, y, w.p(z)), nx4 = w.at(x + 4 == N ? 0 : x + 4, y, z);
+        uint32_t C[2] = {0, 0};
 #pragma unroll
         for (int s = 0; s < 2; s++) {
             const uint8_t *Wxy = codes + (size_t)(3 * s + 0) * V, *Wyz = codes + (size_t)(3 * s + 1) * V,
                           *Wzx = codes + (size_t)(3 * s + 2) * V;
-            C[s] = abs(decode_w(Wxy[lin])) + abs(decode_w(Wxy[nz])) + abs(decode_w(Wyz[lin])) +
-                   abs(decode_w(Wyz[nx])) + abs(decode_w(Wzx[lin])) + abs(decode_w(Wzx[ny]));
-            cells[(size_t)s * V + lin] = (uint8_t)C[s];
+            const uint32_t xy0 = *reinterpret_cast<const uint32_t *>(Wxy + lin), xy1 = *reinterpret_cast<const uint32_t *>(Wxy + nz);
+            const uint32_t yz0 = *reinterpret_cast<const uint32_t *>(Wyz + lin), zx0 = *reinterpret_cast<const uint32_t *>(Wzx + lin);
+            const uint32_t zx1 = *reinterpret_cast<const uint32_t *>(Wzx + ny);
+            const uint32_t yz1 = (yz0 >> 8) | ((uint32_t)Wyz[nx4] << 24);                    // W_yz at x + 1
+#pragma unroll
+            for (int k = 0; k < 4; k++) {
+                const int c = mag(xy0, k) + mag(xy1, k) + mag(yz0, k) + mag(yz1, k) + mag(zx0, k) + mag(zx1, k);
+                C[s] |= (uint32_t)c << (8 * k);
+            }
+            *reinterpret_cast<uint32_t *>(cells + (size_t)s * V + lin) = C[s];
         }
-        acc[0] += C[0] > 0;
-        acc[1] += C[1] > 0;
-        acc[2] += (C[0] > 0) && (C[1] > 0);
+#pragma unroll
+        for (int k = 0; k < 4; k++) {
+            const int cp = (C[0] >> (8 * k)) & 255, cq = (C[1] >> (8 * k)) & 255;
+            acc[0] += cp > 0;
+            acc[1] += cq > 0;
+            acc[2] += (cp > 0) && (cq > 0);
+        }
     }
     block_reduce_store<3>(acc, 3, partials);
 }
