@@ -136,6 +136,12 @@ int u1u1_import_state(u1u1_ctx *ctx, const void *src_dev);
 int u1u1_export_state_host(u1u1_ctx *ctx, void *dst_host);
 int u1u1_import_state_host(u1u1_ctx *ctx, const void *src_host);
 
+/* Fill the lattice with the periodic tiling of a smaller canonical state float32 [20][n_src][n_src][n_src] (DEVICE;
+ * N must be a multiple of n_src): a relaxed small box as the initial condition of a large one, and -- because a tiled
+ * state evolves as the tiling of the small evolution -- an exact full-size check of every kernel against a lattice
+ * the oracle can afford. */
+int u1u1_import_state_tiled(u1u1_ctx *ctx, const void *src_dev, int32_t n_src);
+
 /* Canonical sub-block float32 [20][bz][by][bx] whose corner is site (x0,y0,z0), periodic wrap, to a
  * DEVICE buffer: lets a caller inspect a 1024^3 state (for which a full canonical copy does not fit
  * beside the state) -- used by the sampled full-size parity test. */

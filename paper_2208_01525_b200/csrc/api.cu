@@ -420,6 +420,19 @@ extern "C" int u1u1_import_state(u1u1_ctx *ctx, const void *src_dev)
     return relayout(ctx, (float *)src_dev, 0);
 }
 
+extern "C" int u1u1_import_state_tiled(u1u1_ctx *ctx, const void *src_dev, int32_t n_src)
+{
+    if (!ctx || !src_dev) return ctx ? fail(ctx, U1U1_EINVAL, "src is NULL") : U1U1_EINVAL;
+    if (!ctx->configured) return fail(ctx, U1U1_ESTATE, "import_state_tiled before configure");
+    if (n_src < 1 || ctx->N % n_src != 0) return fail(ctx, U1U1_ESIZE, "N must be a multiple of n_src");
+    cudaError_t e = launch_import_tiled(pos_buf(ctx, ctx->cur), mom_buf(ctx), (const float *)src_dev, ctx->V, ctx->N, n_src, ctx->stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "import_state_tiled launch");
+    ctx->launches += 1;
+    ctx->diag_valid = false;
+    ctx->labels_valid = false;
+    return U1U1_OK;
+}
+
 extern "C" int u1u1_export_block(u1u1_ctx *ctx, int32_t x0, int32_t y0, int32_t z0, int32_t bx, int32_t by,
                                  int32_t bz, void *dst_dev)
 {

@@ -121,6 +121,20 @@ __global__ void relayout_kernel(float *pos, float *mom, float *canon, size_t V, 
     }
 }
 
+// internal <- periodic tiling of a smaller canonical state [20][n][n][n] (N a multiple of n)
+__global__ void import_tiled_kernel(float *pos, float *mom, const float *canon, size_t V, int N, int n)
+{
+    const size_t v = (size_t)n * n * n;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < 20 * V; i += (size_t)gridDim.x * blockDim.x) {
+        const int c = (int)(i / V);
+        const size_t lin = i % V;
+        const int x = (int)(lin % (size_t)N), y = (int)((lin / (size_t)N) % (size_t)N), z = (int)(lin / ((size_t)N * N));
+        int is_mom, comp;
+        canonical_to_internal(c, is_mom, comp);
+        (is_mom ? mom : pos)[comp_off(comp, lin, V)] = canon[(size_t)c * v + ((size_t)(z % n) * n + (size_t)(y % n)) * n + (size_t)(x % n)];
+    }
+}
+
 // canonical sub-block [20][bz][by][bx] starting at (x0,y0,z0), periodic wrap (for sampled parity checks)
 __global__ void export_block_kernel(const float *pos, const float *mom, size_t V, int N, int x0, int y0,
                                     int z0, int bx, int by, int bz, float *dst)
@@ -171,6 +185,12 @@ cudaError_t launch_export_block(const float *pos, const float *mom, size_t V, in
                                 int bx, int by, int bz, float *dst, cudaStream_t st)
 {
     export_block_kernel<<<64, 256, 0, st>>>(pos, mom, V, N, x0, y0, z0, bx, by, bz, dst);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_import_tiled(float *pos, float *mom, const float *canon, size_t V, int N, int n, cudaStream_t st)
+{
+    import_tiled_kernel<<<GRID, 256, 0, st>>>(pos, mom, canon, V, N, n);
     return cudaGetLastError();
 }
 

@@ -30,6 +30,7 @@ cudaError_t launch_init_smoothed(float *pos, float *tmp_a, float *tmp_b, size_t 
                                  double width, int trunc, double eta1, double eta2, cudaStream_t st);
 cudaError_t launch_export_block(const float *pos, const float *mom, size_t V, int N, int x0, int y0, int z0,
                                 int bx, int by, int bz, float *dst, cudaStream_t st);
+cudaError_t launch_import_tiled(float *pos, float *mom, const float *canon, size_t V, int N, int n, cudaStream_t st);
 cudaError_t launch_relayout(float *pos, float *mom, float *canon, size_t V, int c0, int ncomp, int to_canonical,
                             cudaStream_t st);
 

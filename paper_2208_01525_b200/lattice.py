@@ -91,6 +91,14 @@ class Lattice:
         self._check(self.lib.u1u1_import_state(self._ctx, t.data_ptr()), "import_state")
         self.stream.synchronize()   # `t` may be a temporary
 
+    def import_state_tiled(self, t):
+        """Periodic tiling of a smaller canonical state [20, n, n, n] (N a multiple of n)."""
+        torch = self._torch
+        t = t.to(device=self.device, dtype=torch.float32).contiguous()
+        assert t.shape[0] == 20 and t.shape[1] == t.shape[2] == t.shape[3], t.shape
+        self._check(self.lib.u1u1_import_state_tiled(self._ctx, t.data_ptr(), int(t.shape[1])), "import_state_tiled")
+        self.stream.synchronize()
+
     def export_state_host(self, host_tensor):
         self._check(self.lib.u1u1_export_state_host(self._ctx, host_tensor.data_ptr()), "export_state_host")
 

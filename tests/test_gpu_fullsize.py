@@ -98,3 +98,58 @@ def test_sampled_windings_full_size():
         assert d["sumW_p" if sec == 0 else "sumW_q"] == float(W.abs().sum(dtype=torch.int64))
         del W, near, cells
     assert checked > 15000 and nonzero > 0          # random-phase start: plenty of strings in any block
+
+
+def test_tiled_state_full_size_every_kernel():
+    """A 1024^3 lattice filled with the periodic tiling of a 64^3 state evolves as the tiling of the 64^3 evolution.
+    So EVERY site of the full-size run is checked at once: after the steps the full-size diagnostics (all integer
+    counts, all lattice sums, the Gauss norms, the segment statistics) must equal 16^3 times / sqrt(16^3) times those
+    of the small lattice, whose state is compared element by element with the oracle."""
+    import torch
+    from paper_2208_01525_b200 import Lattice, Params, state_bytes, scratch_bytes
+    N, n, nsteps = 1024, 64, 3
+    reps = (N // n) ** 3
+    gc.collect(); torch.cuda.empty_cache()
+    free, _ = torch.cuda.mem_get_info()
+    need = state_bytes(N) + scratch_bytes(N) + (2 << 30)
+    if free < need:
+        pytest.skip(f"needs {need / 2**30:.0f} GiB of free HBM, have {free / 2**30:.0f}")
+    prm = Params(tau_norm=256.0)
+    small = Lattice(n)
+    small.init_fields(9, DX, Params(tau_norm=256.0, friction=0.5))
+    small.step(40, 1.0, 0.5, 1.0)                      # a damped start: momenta, links and strings all present
+    small.set_params(prm)
+    s0 = small.export_state()
+    big = Lattice(N)
+    big.configure(DX, prm)
+    big.import_state_tiled(s0)
+    tau = 5.0
+    small.step(nsteps, tau, 0.5, 1.0)
+    big.step(nsteps, tau, 0.5, 1.0)
+    # the small lattice against the oracle, element by element
+    ref = s0.cpu().numpy().astype(np.float64)
+    O.step(ref, DX, O.Couplings(), tau, 0.5, 1.0, DTAU, tau_norm=256.0, n=nsteps)
+    sm = small.export_state().cpu().numpy().astype(np.float64)
+    for name, comps in inputs.GROUPS.items():
+        assert np.max(np.abs(sm[comps] - ref[comps])) / np.max(np.abs(ref[comps])) < 3e-5, name
+    # sampled tiles of the big lattice are bit-identical to the small lattice (interior, boundary and wrap tiles)
+    smt = small.export_state()
+    for (x, y, z) in [(0, 0, 0), (960, 960, 960), (320, 0, 704), (992, 512, 64), (64, 1000, 1000)]:
+        blk = big.export_block(x, y, z, 32, 24, 16)
+        ix = (torch.arange(x, x + 32, device=blk.device) % n)
+        iy = (torch.arange(y, y + 24, device=blk.device) % n)
+        iz = (torch.arange(z, z + 16, device=blk.device) % n)
+        assert torch.equal(blk, smt[:, iz][:, :, iy][:, :, :, ix]), (x, y, z)
+    # every site at once: global diagnostics scale exactly with the number of tiles
+    ds, db = small.diagnostics(), big.diagnostics()
+    for k in ("sumW_p", "sumW_q", "cells_p", "cells_q", "cells_pq", "near_p", "near_q", "cells_pq_tol_p", "cells_pq_tol_q"):
+        assert db[k] == reps * ds[k], k
+    assert db["maxW"] == ds["maxW"] and ds["sumW_p"] > 0
+    for k in ("sum_L", "sum_kin_L", "sum_grad_L", "sum_kin_V", "sum_grad_V", "sum_vint", "sum_kin", "sum_grad", "sum_elec",
+              "sum_mag", "sum_pot"):
+        assert np.isclose(db[k], reps * ds[k], rtol=1e-9, atol=1e-9 * reps * abs(ds["sum_grad"])), k
+    gs, gb = small.gauss_violation(), big.gauss_violation()
+    assert np.allclose(gb[[0, 1, 4, 5]], np.sqrt(reps) * gs[[0, 1, 4, 5]], rtol=1e-9)
+    assert np.array_equal(gb[[2, 6]], gs[[2, 6]])                                   # max |g|
+    ss, sb = small.pq_segments(1, True), big.pq_segments(1, True)
+    assert sb["cells_all"] == reps * ss["cells_all"]
