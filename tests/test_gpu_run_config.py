@@ -1,0 +1,41 @@
+"""The config driver (paper_2208_01525_b200.run_config) end to end on small lattices: schedules, prephase switch,
+diagnostic cadence, segment labelling; config 1 at its own size against the oracle's diagnostics at the last step."""
+import json
+
+import numpy as np
+import pytest
+
+from oracle import oracle as O
+
+pytestmark = pytest.mark.gpu
+
+
+def test_config1_diagnostics_at_last_step():
+    from paper_2208_01525_b200.run_config import run
+    rows = []
+    s = run(1, emit=lambda line: rows.append(json.loads(line)))
+    assert s["steps"] == 32 and np.isclose(s["tau_end"], 4.2) and len(rows) == 2 and "summary" in rows[-1]
+    d = rows[0]
+    ref = O.init_random_phase(64, 1)
+    ref = ref.astype(np.float32).astype(np.float64)
+    O.step(ref, 0.5, O.Couplings(), 1.0, 0.5, 1.0, 0.1, tau_norm=1.0, n=32)
+    _, c, _, _ = O.scalars(4.2, 0.5, 1.0, 0.1, 1.0)
+    r = O.diagnostics(ref, 0.5, O.Couplings(), c)
+    # the oracle's own trajectory differs from the GPU's by ~1e-4 after 32 steps: counts agree to a few plaquettes
+    assert abs(d["sumW_p"] - r["sumW_p"]) <= 0.01 * r["sumW_p"] and d["maxW"] == max(r["maxW_p"], r["maxW_q"])
+    assert np.isclose(d["energy"], 0.5 ** 3 * sum(r[k] for k in ("sum_kin", "sum_grad", "sum_elec", "sum_mag", "sum_pot")), rtol=1e-3)
+    assert d["gauss_rel_p"] < 1e-5 and d["gauss_rel_q"] < 1e-5
+
+
+@pytest.mark.parametrize("config", [2, 3, 4, 5])
+def test_schedules_on_small_lattices(config):
+    from paper_2208_01525_b200.run_config import run, CONFIGS
+    rows = []
+    s = run(config, size=96, segments=True, emit=lambda line: rows.append(json.loads(line)))
+    out = [r for r in rows if "summary" not in r]
+    assert s["steps"] == min(CONFIGS[config]["pre"] + CONFIGS[config]["steps"], 230)     # half light-crossing of 96^3
+    assert out[-1]["step"] == s["steps"] and all(r["maxW"] <= 2 for r in out) and out[-1]["maxW"] <= 1
+    assert all(np.isfinite(r["xi_W"]) or r["sumW_p"] == 0 for r in out)
+    assert all("segments" in r and r["segments"]["cells_all"] >= r["cells_pq"] for r in out)
+    if CONFIGS[config]["pre"]:
+        assert out[0]["prephase"] and not out[-1]["prephase"]
