@@ -82,6 +82,27 @@ __device__ inline int decode_w(uint8_t code) { return (int)(code & 15) - 8; }
 // ---------------------------------------------------------------------------------------------
 constexpr int WTX = 32, WTY = 8, WEX = WTX + 1, WEY = WTY + 1, WNE = WEX * WEY, WZC = 32;
 
+// atan2 in ~20 instructions: octant reduction to t = min/max in [0, 1] and the degree-8 (in t^2) polynomial of
+// Abramowitz & Stegun 4.4.49 (|error| <= 2e-8 in exact arithmetic; ~4e-7 in fp32 with the fast division), the same
+// accuracy as libm's atan2f at a fifth of the instructions.  Never called with x = y = 0.
+__device__ inline float atan2_poly(float y, float x)
+{
+    const float ax = fabsf(x), ay = fabsf(y);
+    const float t = __fdividef(fminf(ax, ay), fmaxf(ax, ay)), s = t * t;
+    float p = 0.0028662257f;
+    p = fmaf(p, s, -0.0161657367f);
+    p = fmaf(p, s, 0.0429096138f);
+    p = fmaf(p, s, -0.0752896400f);
+    p = fmaf(p, s, 0.1065626393f);
+    p = fmaf(p, s, -0.1420889944f);
+    p = fmaf(p, s, 0.1999355085f);
+    p = fmaf(p, s, -0.3333314528f);
+    float r = fmaf(p * s, t, t);
+    r = ay > ax ? 1.57079637f - r : r;
+    r = x < 0.f ? 3.14159274f - r : r;
+    return copysignf(r, y);
+}
+
 __device__ inline float chi_of(float alpha_a, float alpha_b, float theta)
 {
     const float v = (alpha_b - alpha_a) - theta;                       // NaN if an end point is exactly zero
@@ -116,8 +137,8 @@ __global__ void __launch_bounds__(RED_BLOCK) winding_tiled_kernel(const float *p
                 if (ex > wx || ey > wy) continue;
                 const int x = x0 + ex == N ? 0 : x0 + ex, y = y0 + ey == N ? 0 : y0 + ey;
                 const float4 a = PA[(size_t)z * NN + (size_t)y * N + x];
-                alpha[b][0][e] = (a.x == 0.f && a.y == 0.f) ? __int_as_float(0x7fc00000) : atan2f(a.y, a.x);
-                alpha[b][1][e] = (a.z == 0.f && a.w == 0.f) ? __int_as_float(0x7fc00000) : atan2f(a.w, a.z);
+                alpha[b][0][e] = (a.x == 0.f && a.y == 0.f) ? __int_as_float(0x7fc00000) : atan2_poly(a.y, a.x);
+                alpha[b][1][e] = (a.z == 0.f && a.w == 0.f) ? __int_as_float(0x7fc00000) : atan2_poly(a.w, a.z);
             }
         };
         __syncthreads();                               // previous item's readers are done
