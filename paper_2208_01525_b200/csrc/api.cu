@@ -189,6 +189,21 @@ extern "C" int u1u1_set_time(u1u1_ctx *ctx, double tau, double era_m, double s)
     return U1U1_OK;
 }
 
+// kernel_variant (low 4 bits, include/u1u1.h) -> template instance of the tiled kernel; -1 = reference kernel
+static int tiled_mode(int kv)
+{
+    static const int mode_of[8] = {5, -1, 3, -1, 1, 2, 0, 4};
+    return mode_of[kv & 7];
+}
+
+static cudaError_t launch_step(u1u1_ctx *ctx, const StepCoef &q)
+{
+    const int kv = ctx->prm.kernel_variant & 15;
+    Lattice L{pos_buf(ctx, ctx->cur), pos_buf(ctx, ctx->cur ^ 1), mom_buf(ctx), ctx->V, ctx->N};
+    const bool tiled = tiled_mode(kv) >= 0 && step_tiled_supports(ctx->N);
+    return tiled ? launch_step_tiled(L, q, ctx->stream, tiled_mode(kv)) : launch_step_ref(L, q, ctx->stream, kv == 3);
+}
+
 extern "C" int u1u1_step(u1u1_ctx *ctx, int32_t n, double tau, double era_m, double s)
 {
     if (!ctx) return U1U1_EINVAL;
@@ -198,12 +213,6 @@ extern "C" int u1u1_step(u1u1_ctx *ctx, int32_t n, double tau, double era_m, dou
     if (era_m != 0 && !(tau > 0)) return fail(ctx, U1U1_EINVAL, "tau must be positive in an expanding background");
     const u1u1_params &P = ctx->prm;
     const double dx = ctx->dx, dt = P.dtau, f = P.friction;
-    const int kv = P.kernel_variant & 15;
-    const bool tiled = kv != 1 && kv != 3 && step_tiled_supports(ctx->N);
-    // variants (include/u1u1.h): 0 tiled fp32 difference form + SFU phasor (default); 2 tiled plain fp32 + SFU;
-    // 4 tiled fp64 chain + SFU; 5 / 6 / 7 = 2 / 4 / 0 with libm sincosf; 1 / 3 reference one-thread-per-site fp32 / fp64
-    static const int tmode_of[8] = {5, -1, 3, -1, 1, 2, 0, 4};
-    const int tmode = tmode_of[kv];
     for (int k = 0; k < n; k++) {
         const double tk = tau + k * dt;
         double a, c, delta, omega;
@@ -234,8 +243,7 @@ extern "C" int u1u1_step(u1u1_ctx *ctx, int32_t n, double tau, double era_m, dou
         q.aSm1 = (float)(f * (1.0 - delta) / (1.0 + delta) - 1.0);
         q.aGm1 = (float)(f * (1.0 - omega) / (1.0 + omega) - 1.0);
         q.flags = P.kernel_variant >> 4;
-        Lattice L{pos_buf(ctx, ctx->cur), pos_buf(ctx, ctx->cur ^ 1), mom_buf(ctx), ctx->V, ctx->N};
-        cudaError_t e = tiled ? launch_step_tiled(L, q, ctx->stream, tmode) : launch_step_ref(L, q, ctx->stream, kv == 3);
+        cudaError_t e = launch_step(ctx, q);
         if (e != cudaSuccess) return cuda_fail(ctx, e, "step kernel launch");
         ctx->launches += 1;
         ctx->cur ^= 1;
@@ -262,9 +270,6 @@ extern "C" int u1u1_cool(u1u1_ctx *ctx, int32_t n, double dcool)
     const double lam = std::fmax(P.lambda1 * P.eta1 * P.eta1, P.lambda2 * P.eta2 * P.eta2);
     if (dcool * (12.0 / (dx * dx) + lam) >= 2.0)
         return fail(ctx, U1U1_EUNSTABLE, "explicit cooling unstable: need dcool (12/dx^2 + lambda sigma^2) < 2");
-    const int kv = P.kernel_variant & 15;
-    const bool tiled = kv != 1 && kv != 3 && step_tiled_supports(ctx->N);
-    static const int tmode_of[8] = {5, -1, 3, -1, 1, 2, 0, 4};
     // Pi+ = 0 Pi- + 1 [D-D+ phi - lambda/2 (|phi|^2 - sigma^2) phi], phi += dcool Pi+  (and the same for E, theta)
     StepCoef q;
     q.aS = 0.f; q.bS = 1.f; q.aG = 0.f; q.bG = 1.f; q.aSm1 = -1.f; q.aGm1 = -1.f;
@@ -281,8 +286,7 @@ extern "C" int u1u1_cool(u1u1_ctx *ctx, int32_t n, double dcool)
     q.dtau_dx = (float)(dcool * dx);
     q.flags = P.kernel_variant >> 4;
     for (int k = 0; k < n; k++) {
-        Lattice L{pos_buf(ctx, ctx->cur), pos_buf(ctx, ctx->cur ^ 1), mom_buf(ctx), ctx->V, ctx->N};
-        cudaError_t e = tiled ? launch_step_tiled(L, q, ctx->stream, tmode_of[kv]) : launch_step_ref(L, q, ctx->stream, kv == 3);
+        cudaError_t e = launch_step(ctx, q);
         if (e != cudaSuccess) return cuda_fail(ctx, e, "cooling kernel launch");
         ctx->launches += 1;
         ctx->cur ^= 1;
