@@ -29,10 +29,6 @@ struct Lattice {
     int N;
 };
 
-__host__ __device__ inline size_t packA_off(size_t V) { (void)V; return 0; }
-__host__ __device__ inline size_t packB_off(size_t V) { return 4 * V; }
-__host__ __device__ inline size_t packC_off(size_t V) { return 8 * V; }
-
 // float offset of logical component c (0..9) of site lin inside a 10 V-float buffer
 __host__ __device__ inline size_t comp_off(int c, size_t lin, size_t V)
 {
