@@ -9,8 +9,11 @@ sums written as plain numpy reductions, and the derived scalars of PAPER.md Eq. 
 (:185-221).  State arrays are float64 numpy arrays of shape (20, nz, ny, nx) (canonical layout, see
 the C header comment).
 
-parity unpinned: the VALUES of xi_L, <v^2>, f_total (their definitions are fixed, nothing in the
-paper fixes their numbers for a given snapshot).
+Pins of the diagnostic combinations (tests/test_oracle_pins_diag.py): the Lagrangian density and its a-weights by
+the variational principle against the pinned kicks (c != 1), virial theorems on the normal modes, the
+Euler-Lagrange damping ratio omega/delta = 1 - beta; xi_L and mu = 2 pi sigma^2 on the Bogomolny vortex; V_int on
+hand-computed sites; f_total / f_p on hand-built lines; the near-cut mask on hand-built links.  Nothing is left
+"parity unpinned".
 """
 from __future__ import annotations
 
@@ -301,6 +304,14 @@ def energy(state, dx, K):
     return dx ** 3 * float(np.sum(d["kin"] + d["grad"] + d["elec"] + d["mag"] + d["pot"]))
 
 
+def lagrangian(state, dx, K, c):
+    """Per-site Lagrangian density L_x of PAPER.md:198 Eq. 33 (reading R-14): Eq. 1 (:43) in the comoving variables of
+    the discretisation, divided by a^2, with the couplings of Eq. 12 (:89) -- kin - grad + (elec - mag)/c - c pot,
+    c = a^{2 beta}.  Returns (L_x, the dict of unweighted densities it was formed from)."""
+    d = densities(state, dx, K)
+    return d["kin"] - d["grad"] + (d["elec"] - d["mag"]) / c - c * d["pot"], d
+
+
 def diagnostics(state, dx, K, c, cut_tol=1e-5):
     """All in-loop diagnostics of PAPER.md Eq. 31-37 from one snapshot, as a dict."""
     out = {}
@@ -317,8 +328,7 @@ def diagnostics(state, dx, K, c, cut_tol=1e-5):
     out["cells_pq"] = int(np.sum((Cs[0] > 0) & (Cs[1] > 0)))
     out["cells_pq_tol_p"], out["cells_pq_tol_q"] = cells_pq_tolerant(Cs[0], Cs[1])
     out["L_pq_tol"] = 0.5 * dx * (out["cells_pq_tol_p"] + out["cells_pq_tol_q"])
-    d = densities(state, dx, K)
-    lag = d["kin"] - d["grad"] + (d["elec"] - d["mag"]) / c - c * d["pot"]
+    lag, d = lagrangian(state, dx, K, c)
     out["sum_L"] = float(np.sum(lag))
     out["sum_kin_L"] = float(np.sum(d["kin"] * lag))
     out["sum_grad_L"] = float(np.sum(d["grad"] * lag))

@@ -29,7 +29,9 @@
  * homogeneous-mode ODE, Philox known-answer vectors.
  * Cooling (O-12, Eq. 27-30): monotone energy decrease, relaxed vortex as a fixed point, equivalence with
  *   kick+drift from zero momenta when kappa = 0.
- * parity unpinned: the VALUES of xi_L, <v^2>, f_total (only their definitions are fixed).
+ * Diagnostic combinations (tests/test_oracle_pins_diag.py): the densities of orc_densities through the variational
+ *   principle (their weighted sum's gradient is the pinned kicks' right-hand side), virial theorems, the Bogomolny
+ *   vortex; V_int on hand-computed sites; the near-cut mask of orc_windings on hand-built links.
  */
 #include <math.h>
 #include <stdint.h>

@@ -468,8 +468,19 @@ def relax(s, dx, K, eps, iters):
     return s
 
 
+_vortex_cache = {}
+
+
 def vortex_energy(n, dx, sector):
-    """Relaxed vortex-antivortex pair (net flux through a periodic plane must vanish), nz = 1."""
+    """Relaxed vortex-antivortex pair (net flux through a periodic plane must vanish), nz = 1.
+    (Cached per process: several pins start from the same relaxed configuration; callers get copies.)"""
+    if (n, dx, sector) not in _vortex_cache:
+        _vortex_cache[(n, dx, sector)] = _vortex_energy(n, dx, sector)
+    s, K = _vortex_cache[(n, dx, sector)]
+    return s.copy(), K
+
+
+def _vortex_energy(n, dx, sector):
     shape = (1, n, n)
     K = O.Couplings(kappa=0.0)                                  # decoupled, critical: lambda = 2 e^2
     centers = [(n / 4 - 0.5, n / 2 - 0.5), (3 * n / 4 - 0.5, n / 2 - 0.5)]
