@@ -259,8 +259,11 @@ def pq_mask(Cp, Cq, tolerant=False):
 
 def pq_segments(Cp, Cq, dx, min_cells=1, tolerant=False):
     """The robust method's numbers (reading R-21) by plain flood fill: connected regions
-    of pq cells over the periodic 26-neighbourhood; N_pq = regions with >= min_cells cells, L_pq = dx sum (N_cells - 1)
-    over them (:248), l_pq = L_pq / N_pq (Eq. 38).  Returns (dict, sorted list of all region sizes)."""
+    of pq cells over the periodic 26-neighbourhood.  A region's cell count is N = (its cells pierced by p + its cells
+    pierced by q) / 2 (reading R-21b): the number of its cells for exact overlap, and for one cell of tolerance the
+    SAME length for a coincident and for a one-cell-displaced pair of lines (as L_pq^tol of R-13b; the plain cell count
+    of the union mask would double for the displaced pair).  N_pq = regions with N >= min_cells, L_pq = dx sum (N - 1)
+    over them (:248), l_pq = L_pq / N_pq (Eq. 38).  Returns (dict, sorted list of all region counts N)."""
     mask = pq_mask(Cp, Cq, tolerant)
     nz, ny, nx = mask.shape
     seen = np.zeros(mask.shape, dtype=bool)
@@ -269,10 +272,10 @@ def pq_segments(Cp, Cq, dx, min_cells=1, tolerant=False):
         if seen[start]:
             continue
         seen[start] = True
-        stack, n = [start], 0
+        stack, n2 = [start], 0
         while stack:
             z, y, x = stack.pop()
-            n += 1
+            n2 += int(Cp[z, y, x] > 0) + int(Cq[z, y, x] > 0)
             for dz in (-1, 0, 1):
                 for dy in (-1, 0, 1):
                     for dx_ in (-1, 0, 1):
@@ -280,11 +283,11 @@ def pq_segments(Cp, Cq, dx, min_cells=1, tolerant=False):
                         if mask[c] and not seen[c]:
                             seen[c] = True
                             stack.append(c)
-        sizes.append(n)
+        sizes.append(n2 / 2 if n2 % 2 else n2 // 2)
     kept = [n for n in sizes if n >= min_cells]
     L = dx * sum(n - 1 for n in kept)
     out = {"N_pq": len(kept), "L_pq": L, "l_pq": L / len(kept) if kept else 0.0, "cells_kept": sum(kept),
-           "segments_all": len(sizes), "cells_all": int(mask.sum()), "largest": max(sizes) if sizes else 0}
+           "segments_all": len(sizes), "cells_all": sum(sizes), "largest": max(sizes) if sizes else 0}
     return out, sorted(sizes)
 
 

@@ -675,7 +675,28 @@ def test_pq_segments_on_hand_built_regions():
     Cq[2:9, 3, 4] = 2
     assert O.pq_segments(Cp, Cq, 0.5)[1] == []
     out, sizes = O.pq_segments(Cp, Cq, 0.5, tolerant=True)
-    assert sizes == [14] and out["N_pq"] == 1
+    assert sizes == [7] and out["N_pq"] == 1 and out["cells_all"] == 7
+    # reading R-21b: the displaced 7-cell pair has the SAME length and the same threshold behaviour as the coincident one
+    Cq2 = np.zeros_like(Cq)
+    Cq2[2:9, 3, 3] = 2
+    for tol in (False, True):
+        co, _ = O.pq_segments(Cp, Cq2, 0.5, tolerant=tol)
+        assert co["L_pq"] == out["L_pq"] == 0.5 * 6 and co["N_pq"] == 1
+    for thr, kept in ((7, 1), (8, 0)):
+        assert O.pq_segments(Cp, Cq, 0.5, min_cells=thr, tolerant=True)[0]["N_pq"] == kept
+        assert O.pq_segments(Cp, Cq2, 0.5, min_cells=thr, tolerant=True)[0]["N_pq"] == kept
+    # a pair that coincides on 3 cells and is displaced on the other 4: still 7 cells of bound string
+    Cq3 = np.zeros_like(Cq)
+    Cq3[2:5, 3, 3] = 2
+    Cq3[5:9, 3, 4] = 2
+    out3, sizes3 = O.pq_segments(Cp, Cq3, 0.5, tolerant=True)
+    assert sizes3 == [7] and out3["L_pq"] == 3.0
+    # a q line one cell LONGER than the p line it shadows: (7 + 8) / 2 cells, consistent with L_pq^tol of R-13b
+    Cq4 = np.zeros_like(Cq)
+    Cq4[2:10, 3, 4] = 2
+    out4, sizes4 = O.pq_segments(Cp, Cq4, 0.5, tolerant=True)
+    assert sizes4 == [7.5] and out4["L_pq"] == 0.5 * 6.5
+    assert 0.5 * sum(O.cells_pq_tolerant(Cp, Cq4)) == out4["cells_all"] == 7.5
 
 
 def test_pq_segments_against_library_labelling():
