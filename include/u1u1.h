@@ -72,8 +72,9 @@ typedef struct {
 
 /* Bytes of device memory the caller must provide for an N^3 lattice.
  * state  : 30 fp32 words/site (20 fields + a second copy of the 10 position words, ping-pong).
- * scratch: winding codes (6 B/site) and cell arrays (2 B/site) -- reused as int32 segment labels and sizes by
- *          u1u1_pq_segments and as a staging plane by the *_host copies -- plus the reduction partials. */
+ * scratch: cell arrays (2 B/site) + a work area of 8 B/site -- winding codes for u1u1_export_windings, int32 segment
+ *          labels and sizes for u1u1_pq_segments, two staging planes for the *_host copies -- plus the reduction
+ *          partials. */
 size_t u1u1_state_bytes(int32_t N);
 size_t u1u1_scratch_bytes(int32_t N);
 
@@ -113,14 +114,17 @@ int u1u1_step(u1u1_ctx *ctx, int32_t n, double tau, double era_m, double s);
  *   dphi/deta = D-_j D+_j phi - lambda_p0/2 (|phi|^2 - sigma_p^2) phi,   dA_i/deta = -sum_j d-_j F_ij + 2 e_p0^2 Im(phi* D+_i phi)
  * and the mirror for (psi, B); no kappa term, no scale factor.  Runs in the fused step kernel with the kick
  * coefficients set to (0, 1) and the drift to dcool; on exit all momenta are zero.  The paper uses eta from -10
- * to 1 in steps of 1/30.  Needs dcool (12/dx^2 + lambda sigma^2) < 2 (explicit diffusion), else U1U1_EUNSTABLE.
+ * to 1 in steps of 1/30.  Needs dcool (12/dx^2 + max(lambda, 2 e^2) sigma^2) < 2 (explicit diffusion of the scalars
+ * and of the links), else U1U1_EUNSTABLE.  Afterwards the diagnostic weights are those of a = 1 (no scale factor).
  * The high-expansion damping phase that follows is u1u1_step with era_m = 0.9 ... 0.95.
  * Asynchronous. */
 int u1u1_cool(u1u1_ctx *ctx, int32_t n, double dcool);
 
 /* diagnostics(out)  [north_star; PAPER.md:183-224 Eq. 31-37, :230-238]: out = HOST array of
  * U1U1_DIAG_LEN doubles, slots named by the U1U1_D_* enum below.  Uses the scale factor of the last
- * completed step (or of `tau_norm`-normalised a=1 before any step).  Synchronises the stream. */
+ * completed step (or of `tau_norm`-normalised a=1 before any step).  ONE read-only sweep over the state computes
+ * everything, including the Gauss-law norms (slots U1U1_D_GAUSS..+7) and the pierced-cell arrays.  Synchronises
+ * the stream. */
 int u1u1_diagnostics(u1u1_ctx *ctx, double *out_host);
 
 /* gauss_violation(out)  [north_star; PAPER.md:73-77 Eq. 9-10, :272]: out = HOST array of 8 doubles,
@@ -148,7 +152,8 @@ int u1u1_import_state_tiled(u1u1_ctx *ctx, const void *src_dev, int32_t n_src);
 int u1u1_export_block(u1u1_ctx *ctx, int32_t x0, int32_t y0, int32_t z0, int32_t bx, int32_t by, int32_t bz,
                       void *dst_dev);
 
-/* After u1u1_diagnostics: copy out the per-plaquette windings of `sector` (0 = p, 1 = q) as
+/* After u1u1_diagnostics (the per-plaquette codes are produced on the first request by a second sweep in export
+ * mode): copy out the per-plaquette windings of `sector` (0 = p, 1 = q) as
  * int8 W[3][N][N][N] (orientation xy, yz, zx) and the near-branch-cut flags uint8 near[3][N][N][N]
  * (1 if any of the plaquette's four link angles lies within 1e-5 of +-pi), and the pierced-cell
  * array uint8 C[N][N][N].  DEVICE destinations; any of them may be NULL. */
@@ -164,8 +169,9 @@ int u1u1_export_windings(u1u1_ctx *ctx, int32_t sector, void *w_dev, void *near_
  *   [3] cells in those segments   [4] number of all segments   [5] number of all pq cells
  *   [6] cells of the largest segment   [7] 0
  * The paper's production threshold is N_cells > 41 (min_cells = 42, L_pq > 20), Fig. 1 uses l_pq >= 3.5 (min_cells = 8).
- * Overwrites the winding / cell scratch arrays (u1u1_export_windings needs a new u1u1_diagnostics afterwards).
- * Synchronises the stream. */
+ * A region's cell count is (its cells pierced by p + its cells pierced by q) / 2 (reading R-21b): the number of cells
+ * for exact overlap, and the same length for a one-cell-displaced pair of lines as for a coincident pair.
+ * Reuses the scratch work area (winding codes); the cell arrays stay valid.  Synchronises the stream. */
 #define U1U1_SEG_LEN 8
 int u1u1_pq_segments(u1u1_ctx *ctx, int32_t min_cells, int32_t tolerant, double *out_host);
 
@@ -216,7 +222,10 @@ enum {
     U1U1_D_CELLS_PQ_TOL_P, /* fast method with one cell of tolerance: pierced p cells  */
     U1U1_D_CELLS_PQ_TOL_Q, /* with a pierced q cell in their 3x3x3 neighbourhood; and q cells near p   */
     U1U1_D_L_PQ_TOL,     /* dx (tol_p + tol_q) / 2: equals L_pq for coincident AND for one-cell-displaced strings */
-    U1U1_D_USED          /* number of slots in use; the rest of the 48 are zero                   */
+    U1U1_D_MAX_THETA,    /* largest |theta| of any link (non-compact phases drift in temporal gauge; the winding
+                            sweep needs |theta| < 180 and u1u1_diagnostics fails with U1U1_ESTATE beyond)  */
+    U1U1_D_GAUSS,        /* 8 slots: the u1u1_gauss_violation array of the same sweep (no second pass needed) */
+    U1U1_D_USED = U1U1_D_GAUSS + 8 /* number of slots in use; the rest of the 48 are zero        */
 };
 
 #ifdef __cplusplus

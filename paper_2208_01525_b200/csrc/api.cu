@@ -10,6 +10,7 @@
 #include "../../include/u1u1.h"
 #include "common.cuh"
 #include "kernels.h"
+#include "stage.cuh"
 
 using namespace u1u1;
 
@@ -28,13 +29,21 @@ struct u1u1_ctx {
     // time bookkeeping for the diagnostic weights
     double tau_pos = 0.0;        // conformal time of the positions
     double a = 1.0, c = 1.0, cG = 1.0;
-    bool diag_valid = false;     // scratch holds windings of the current state
+    bool diag_valid = false;     // scratch holds the cell arrays of the current state
+    bool codes_valid = false;    // scratch holds the winding codes of the current state
     bool labels_valid = false;   // scratch holds segment labels of the current state
     uint64_t launches = 0;
+    // device properties and TMA tensor maps, set up on the first launch (nothing here needs a GPU before that)
+    int sms = 0;
+    bool maps_ready = false;
+    PackMaps pos_halo[2], mom_halo, mom_tile;
+    // second stream and events of the pipelined host copies, created on first use
+    cudaStream_t copy_stream = nullptr;
+    cudaEvent_t ev_kernel[2] = {nullptr, nullptr}, ev_copy[2] = {nullptr, nullptr};
     std::string err;
 };
 
-static std::string g_create_err;
+static thread_local std::string g_create_err;   // message of a failed u1u1_create on this thread
 
 static int fail(u1u1_ctx *ctx, int code, const std::string &msg)
 {
@@ -49,8 +58,10 @@ static int cuda_fail(u1u1_ctx *ctx, cudaError_t e, const char *where)
 
 static bool size_ok(int32_t N) { return N >= 8 && N <= 1024 && (N % 4) == 0; }
 
-// scratch layout: [winding codes 6V][cells 2V] pad-> [partials RED_MAX_BLOCKS*RED_SLOTS doubles][result 64 doubles]
-static size_t scratch_partials_offset(size_t V) { return ((8 * V + 255) / 256) * 256; }
+// scratch layout: [cells 2V][work 8V] pad-> [partials RED_MAX_BLOCKS*RED_SLOTS doubles][result 64 doubles]
+// work = winding codes 6V (export_windings) | segment labels 4V + sizes 4V (pq_segments) | two staging planes 4V + 4V
+// (host copies): the cell arrays survive all of them.
+static size_t scratch_partials_offset(size_t V) { return ((10 * V + 255) / 256) * 256; }
 
 extern "C" size_t u1u1_state_bytes(int32_t N)
 {
@@ -82,7 +93,16 @@ extern "C" int u1u1_create(u1u1_ctx **out, void *state_dev, size_t state_bytes, 
     return U1U1_OK;
 }
 
-extern "C" void u1u1_destroy(u1u1_ctx *ctx) { delete ctx; }
+extern "C" void u1u1_destroy(u1u1_ctx *ctx)
+{
+    if (!ctx) return;
+    for (int b = 0; b < 2; b++) {
+        if (ctx->ev_kernel[b]) cudaEventDestroy(ctx->ev_kernel[b]);
+        if (ctx->ev_copy[b]) cudaEventDestroy(ctx->ev_copy[b]);
+    }
+    if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
+    delete ctx;
+}
 
 extern "C" const char *u1u1_last_error(const u1u1_ctx *ctx)
 {
@@ -112,8 +132,31 @@ static int check_params(u1u1_ctx *ctx, const u1u1_params *p)
 
 static float *pos_buf(u1u1_ctx *ctx, int which) { return ctx->state + (size_t)which * NPOS * ctx->V; }
 static float *mom_buf(u1u1_ctx *ctx) { return ctx->state + (size_t)2 * NPOS * ctx->V; }
+static uint8_t *cells_buf(u1u1_ctx *ctx) { return ctx->scratch; }
+static uint8_t *work_buf(u1u1_ctx *ctx) { return ctx->scratch + 2 * ctx->V; }
 static double *partials(u1u1_ctx *ctx) { return (double *)(ctx->scratch + scratch_partials_offset(ctx->V)); }
 static double *result(u1u1_ctx *ctx) { return partials(ctx) + (size_t)RED_MAX_BLOCKS * RED_SLOTS; }
+
+// SM count of the current device and the tensor maps of this context's buffers, once per configure
+static int prepare_device(u1u1_ctx *ctx)
+{
+    if (!ctx->sms) {
+        int dev = 0, sms = 0;
+        cudaError_t e = cudaGetDevice(&dev);
+        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        if (e != cudaSuccess || sms < 1) return cuda_fail(ctx, e, "querying the SM count");
+        ctx->sms = sms;
+    }
+    if (!ctx->maps_ready && step_tiled_uses_tma(ctx->N)) {
+        const bool ok = encode_halo_maps(&ctx->pos_halo[0], pos_buf(ctx, 0), ctx->V, ctx->N) &&
+                        encode_halo_maps(&ctx->pos_halo[1], pos_buf(ctx, 1), ctx->V, ctx->N) &&
+                        encode_halo_maps(&ctx->mom_halo, mom_buf(ctx), ctx->V, ctx->N) &&
+                        encode_tile_maps(&ctx->mom_tile, mom_buf(ctx), ctx->V, ctx->N);
+        if (!ok) return fail(ctx, U1U1_ECUDA, "cuTensorMapEncodeTiled unavailable or rejected the layout (TMA is required)");
+        ctx->maps_ready = true;
+    }
+    return U1U1_OK;
+}
 
 extern "C" int u1u1_configure(u1u1_ctx *ctx, int32_t N, double dx, const u1u1_params *params)
 {
@@ -131,8 +174,8 @@ extern "C" int u1u1_configure(u1u1_ctx *ctx, int32_t N, double dx, const u1u1_pa
     ctx->cur = 0;
     ctx->tau_pos = params->tau_norm;
     ctx->a = ctx->c = ctx->cG = 1.0;
-    ctx->diag_valid = false;
-    ctx->labels_valid = false;
+    ctx->diag_valid = ctx->codes_valid = ctx->labels_valid = false;
+    ctx->maps_ready = false;
     return U1U1_OK;
 }
 
@@ -201,8 +244,16 @@ static cudaError_t launch_step(u1u1_ctx *ctx, const StepCoef &q)
     const int kv = ctx->prm.kernel_variant & 15;
     Lattice L{pos_buf(ctx, ctx->cur), pos_buf(ctx, ctx->cur ^ 1), mom_buf(ctx), ctx->V, ctx->N};
     const bool tiled = tiled_mode(kv) >= 0 && step_tiled_supports(ctx->N);
-    return tiled ? launch_step_tiled(L, q, ctx->stream, tiled_mode(kv)) : launch_step_ref(L, q, ctx->stream, kv == 3);
+    if (!tiled) return launch_step_ref(L, q, ctx->stream, kv == 3);
+    StepMaps maps;
+    if (ctx->maps_ready) {
+        maps.pos = ctx->pos_halo[ctx->cur];
+        maps.mom = ctx->mom_tile;
+    }
+    return launch_step_tiled(L, q, ctx->stream, tiled_mode(kv), ctx->maps_ready ? &maps : nullptr, ctx->sms);
 }
+
+static void invalidate(u1u1_ctx *ctx) { ctx->diag_valid = ctx->codes_valid = ctx->labels_valid = false; }
 
 extern "C" int u1u1_step(u1u1_ctx *ctx, int32_t n, double tau, double era_m, double s)
 {
@@ -243,6 +294,7 @@ extern "C" int u1u1_step(u1u1_ctx *ctx, int32_t n, double tau, double era_m, dou
         q.aSm1 = (float)(f * (1.0 - delta) / (1.0 + delta) - 1.0);
         q.aGm1 = (float)(f * (1.0 - omega) / (1.0 + omega) - 1.0);
         q.flags = P.kernel_variant >> 4;
+        if (int rc = prepare_device(ctx)) return rc;      // SM count and tensor maps, once per configure
         cudaError_t e = launch_step(ctx, q);
         if (e != cudaSuccess) return cuda_fail(ctx, e, "step kernel launch");
         ctx->launches += 1;
@@ -254,8 +306,7 @@ extern "C" int u1u1_step(u1u1_ctx *ctx, int32_t n, double tau, double era_m, dou
         ctx->a = a1;
         ctx->c = c1;
         ctx->cG = c * (1.0 + delta) / (1.0 + omega);
-        ctx->diag_valid = false;
-    ctx->labels_valid = false;
+        invalidate(ctx);
     }
     return U1U1_OK;
 }
@@ -267,9 +318,13 @@ extern "C" int u1u1_cool(u1u1_ctx *ctx, int32_t n, double dcool)
     if (n < 0 || !(dcool > 0)) return fail(ctx, U1U1_EINVAL, "need n >= 0 and dcool > 0");
     const u1u1_params &P = ctx->prm;
     const double dx = ctx->dx;
-    const double lam = std::fmax(P.lambda1 * P.eta1 * P.eta1, P.lambda2 * P.eta2 * P.eta2);
+    // explicit diffusion: the scalars see 12/dx^2 + lambda sigma^2, the links 12/dx^2 + 2 e^2 sigma^2
+    const double lam = std::fmax(std::fmax(P.lambda1 * P.eta1 * P.eta1, P.lambda2 * P.eta2 * P.eta2),
+                                 std::fmax(2.0 * P.e1 * P.e1 * P.eta1 * P.eta1, 2.0 * P.e2 * P.e2 * P.eta2 * P.eta2));
     if (dcool * (12.0 / (dx * dx) + lam) >= 2.0)
-        return fail(ctx, U1U1_EUNSTABLE, "explicit cooling unstable: need dcool (12/dx^2 + lambda sigma^2) < 2");
+        return fail(ctx, U1U1_EUNSTABLE, "explicit cooling unstable: need dcool (12/dx^2 + max(lambda, 2 e^2) sigma^2) < 2");
+    if (n > 0)
+        if (int rc = prepare_device(ctx)) return rc;
     // Pi+ = 0 Pi- + 1 [D-D+ phi - lambda/2 (|phi|^2 - sigma^2) phi], phi += dcool Pi+  (and the same for E, theta)
     StepCoef q;
     q.aS = 0.f; q.bS = 1.f; q.aG = 0.f; q.bG = 1.f; q.aSm1 = -1.f; q.aGm1 = -1.f;
@@ -290,12 +345,12 @@ extern "C" int u1u1_cool(u1u1_ctx *ctx, int32_t n, double dcool)
         if (e != cudaSuccess) return cuda_fail(ctx, e, "cooling kernel launch");
         ctx->launches += 1;
         ctx->cur ^= 1;
-        ctx->diag_valid = false;
-    ctx->labels_valid = false;
+        invalidate(ctx);
     }
     if (n > 0) {
         cudaError_t e = cudaMemsetAsync(mom_buf(ctx), 0, (size_t)NMOM * ctx->V * sizeof(float), ctx->stream);
         if (e != cudaSuccess) return cuda_fail(ctx, e, "cool: zeroing the momenta");
+        ctx->a = ctx->c = ctx->cG = 1.0;      // the cooling equations carry no scale factor (Eq. 27-30)
     }
     return U1U1_OK;
 }
@@ -313,12 +368,48 @@ static DiagCoef diag_coef(const u1u1_ctx *ctx)
     return k;
 }
 
+static FusedCoef fused_coef(const u1u1_ctx *ctx)
+{
+    const u1u1_params &P = ctx->prm;
+    const double dx = ctx->dx, dx4 = dx * dx * dx * dx;
+    FusedCoef k;
+    k.inv_dx = 1.0 / dx;
+    k.rho1 = 2.0 * P.e1 * P.e1 * ctx->cG;
+    k.rho2 = 2.0 * P.e2 * P.e2 * ctx->cG;
+    k.inv_dx2 = (float)(1.0 / (dx * dx));
+    k.el1 = (float)(1.0 / (2.0 * P.e1 * P.e1));
+    k.el2 = (float)(1.0 / (2.0 * P.e2 * P.e2));
+    k.mg1 = (float)(1.0 / (2.0 * P.e1 * P.e1 * dx4));
+    k.mg2 = (float)(1.0 / (2.0 * P.e2 * P.e2 * dx4));
+    k.lam1q = (float)(0.25 * P.lambda1);
+    k.lam2q = (float)(0.25 * P.lambda2);
+    k.kappa = (float)P.kappa;
+    k.sig1sq = (float)(P.eta1 * P.eta1);
+    k.sig2sq = (float)(P.eta2 * P.eta2);
+    k.c = (float)ctx->c;
+    k.inv_c = (float)(1.0 / ctx->c);
+    k.flags = P.kernel_variant >> 4;
+    return k;
+}
+
 static int fetch(u1u1_ctx *ctx, double *host, int n)
 {
     cudaError_t e = cudaMemcpyAsync(host, result(ctx), n * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "result readback");
     return U1U1_OK;
+}
+
+// per sector: ||g||_2, ||rho||_2, max|g|, ||g||_2 / max(||rho||_2, ||div E||_2, tiny) from [sum g^2, rho^2, div^2] x 2, max|g| x 2
+static void gauss_norms(const double *sums, const double *gmax, double *out)
+{
+    for (int s = 0; s < 2; s++) {
+        const double l2g = std::sqrt(sums[3 * s]), l2r = std::sqrt(sums[3 * s + 1]), l2d = std::sqrt(sums[3 * s + 2]);
+        out[4 * s + 0] = l2g;
+        out[4 * s + 1] = l2r;
+        out[4 * s + 2] = gmax[s];
+        out[4 * s + 3] = l2g / std::fmax(std::fmax(l2r, l2d), 1e-300);
+    }
 }
 
 extern "C" int u1u1_gauss_violation(u1u1_ctx *ctx, double *out)
@@ -331,13 +422,31 @@ extern "C" int u1u1_gauss_violation(u1u1_ctx *ctx, double *out)
     ctx->launches += 2;
     double r[8];
     if (int rc = fetch(ctx, r, 8)) return rc;
-    for (int s = 0; s < 2; s++) {
-        const double l2g = std::sqrt(r[3 * s]), l2r = std::sqrt(r[3 * s + 1]), l2d = std::sqrt(r[3 * s + 2]);
-        out[4 * s + 0] = l2g;
-        out[4 * s + 1] = l2r;
-        out[4 * s + 2] = r[6 + s];
-        out[4 * s + 3] = l2g / std::fmax(std::fmax(l2r, l2d), 1e-300);
+    gauss_norms(r, r + 6, out);
+    return U1U1_OK;
+}
+
+// The fused sweep (diag_fused.cu) + the tolerant overlap count; result slots [0, FUSED_NRES) and [32, 34).
+// with_codes: also write the winding codes (6 B/site) that u1u1_export_windings decodes.
+static int run_sweep(u1u1_ctx *ctx, bool with_codes)
+{
+    if (int rc = prepare_device(ctx)) return rc;
+    DiagMaps maps;
+    if (ctx->maps_ready) {
+        maps.pos = ctx->pos_halo[ctx->cur];
+        maps.mom = ctx->mom_halo;
     }
+    int nb = 0;
+    cudaError_t e = launch_diag_fused(pos_buf(ctx, ctx->cur), mom_buf(ctx), ctx->V, ctx->N, fused_coef(ctx), cells_buf(ctx),
+                                      with_codes ? work_buf(ctx) : nullptr, partials(ctx), &nb, ctx->maps_ready ? &maps : nullptr,
+                                      ctx->sms, ctx->stream);
+    if (e == cudaSuccess) e = launch_fold(partials(ctx), nb, FUSED_NRES, FUSED_NSUM, result(ctx), ctx->stream);
+    if (e == cudaSuccess) e = launch_overlap_tol(cells_buf(ctx), ctx->V, ctx->N, partials(ctx), result(ctx) + 32, ctx->stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "diagnostics kernel launch");
+    ctx->launches += 4;
+    ctx->diag_valid = true;
+    ctx->codes_valid = with_codes;
+    ctx->labels_valid = false;
     return U1U1_OK;
 }
 
@@ -346,35 +455,31 @@ extern "C" int u1u1_diagnostics(u1u1_ctx *ctx, double *out)
     if (!ctx || !out) return ctx ? fail(ctx, U1U1_EINVAL, "out is NULL") : U1U1_EINVAL;
     if (!ctx->configured) return fail(ctx, U1U1_ESTATE, "diagnostics before configure/init_fields");
     const size_t V = ctx->V;
-    uint8_t *codes = ctx->scratch, *cells = ctx->scratch + 6 * V;
-    double *res = result(ctx);
-    // result slots: [0..4] windings, [8..10] cells, [12..13] tolerant overlap, [16..26] densities
-    cudaError_t e = launch_windings(pos_buf(ctx, ctx->cur), V, ctx->N, codes, cells, partials(ctx), res, ctx->stream);
-    if (e == cudaSuccess)
-        e = launch_densities(pos_buf(ctx, ctx->cur), mom_buf(ctx), V, ctx->N, diag_coef(ctx), partials(ctx),
-                             res + 16, ctx->stream);
-    if (e != cudaSuccess) return cuda_fail(ctx, e, "diagnostics kernel launch");
-    ctx->launches += 8;
-    double r[32];
-    if (int rc = fetch(ctx, r, 32)) return rc;
-    ctx->diag_valid = true;
-    ctx->labels_valid = false;
+    if (int rc = run_sweep(ctx, false)) return rc;
+    double r[34];
+    if (int rc = fetch(ctx, r, 34)) return rc;
+    // the byte lanes of the winding sweep hold wrap counts |n| <= 31: fail loudly beyond (non-compact links, reading R-9)
+    if (r[FR_MAXTH] > 180.0) {
+        ctx->diag_valid = false;
+        return fail(ctx, U1U1_ESTATE, "diagnostics: a link phase exceeds |theta| = 180, beyond the range of the winding sweep");
+    }
     memset(out, 0, U1U1_DIAG_LEN * sizeof(double));
     const double dx = ctx->dx, vol = (double)V * dx * dx * dx;
     out[U1U1_D_TAU] = ctx->tau_pos;
     out[U1U1_D_A] = ctx->a;
     out[U1U1_D_C] = ctx->c;
-    out[U1U1_D_SUMW_P] = r[0];
-    out[U1U1_D_SUMW_Q] = r[1];
-    out[U1U1_D_NEAR_P] = r[2];
-    out[U1U1_D_NEAR_Q] = r[3];
-    out[U1U1_D_MAXW] = r[4];
-    out[U1U1_D_CELLS_P] = r[8];
-    out[U1U1_D_CELLS_Q] = r[9];
-    out[U1U1_D_CELLS_PQ] = r[10];
-    for (int k = 0; k < 11; k++) out[U1U1_D_SUM_L + k] = r[16 + k];
+    out[U1U1_D_SUMW_P] = r[FR_SUMW];
+    out[U1U1_D_SUMW_Q] = r[FR_SUMW + 1];
+    out[U1U1_D_NEAR_P] = r[FR_NEAR];
+    out[U1U1_D_NEAR_Q] = r[FR_NEAR + 1];
+    out[U1U1_D_MAXW] = r[FR_MAXW];
+    out[U1U1_D_CELLS_P] = r[FR_CELLS];
+    out[U1U1_D_CELLS_Q] = r[FR_CELLS + 1];
+    out[U1U1_D_CELLS_PQ] = r[FR_CELLS + 2];
+    const double *dn = r + FR_DENS;      // sum L, kin L, grad L, kin V, grad V, V, kin, grad, elec, mag, pot
+    for (int k = 0; k < 11; k++) out[U1U1_D_SUM_L + k] = dn[k];
     // derived scalars, Eq. 31-37; L_pq = dx N_pq, L_p = dx sum|W^p| - L_pq (:188)
-    const double L_pq = dx * r[10], L_p = dx * r[0] - L_pq, L_q = dx * r[1] - L_pq, tot = L_pq + L_p + L_q;
+    const double L_pq = dx * r[FR_CELLS + 2], L_p = dx * r[FR_SUMW] - L_pq, L_q = dx * r[FR_SUMW + 1] - L_pq, tot = L_pq + L_p + L_q;
     const double inf = INFINITY;
     out[U1U1_D_L_P] = L_p;
     out[U1U1_D_L_Q] = L_q;
@@ -384,17 +489,19 @@ extern "C" int u1u1_diagnostics(u1u1_ctx *ctx, double *out)
     out[U1U1_D_XI_PQ] = L_pq > 0 ? std::sqrt(vol / L_pq) : inf;
     out[U1U1_D_XI_W] = tot > 0 ? std::sqrt(vol / tot) : inf;
     const double mu = 2.0 * 3.14159265358979323846 * ctx->prm.eta1 * ctx->prm.eta1;
-    const double sumL = dx * dx * dx * r[16];
+    const double sumL = dx * dx * dx * dn[0];
     out[U1U1_D_XI_L] = sumL < 0 ? std::sqrt(-mu * vol / sumL) : NAN;
     out[U1U1_D_F_TOTAL] = tot > 0 ? L_pq / tot : 0.0;
     out[U1U1_D_F_P] = L_p > 0 ? L_pq / L_p : 0.0;
-    const double RL = r[18] != 0 ? r[17] / r[18] : NAN, RV = r[20] != 0 ? r[19] / r[20] : NAN;
+    const double RL = dn[2] != 0 ? dn[1] / dn[2] : NAN, RV = dn[4] != 0 ? dn[3] / dn[4] : NAN;
     out[U1U1_D_V2_L] = 2.0 * RL / (1.0 + RL);
     out[U1U1_D_V2_PQ] = 2.0 * RV / (1.0 + RV);
-    out[U1U1_D_ENERGY] = dx * dx * dx * (r[22] + r[23] + r[24] + r[25] + r[26]);
-    out[U1U1_D_CELLS_PQ_TOL_P] = r[12];
-    out[U1U1_D_CELLS_PQ_TOL_Q] = r[13];
-    out[U1U1_D_L_PQ_TOL] = 0.5 * dx * (r[12] + r[13]);
+    out[U1U1_D_ENERGY] = dx * dx * dx * (dn[6] + dn[7] + dn[8] + dn[9] + dn[10]);
+    out[U1U1_D_CELLS_PQ_TOL_P] = r[32];
+    out[U1U1_D_CELLS_PQ_TOL_Q] = r[33];
+    out[U1U1_D_L_PQ_TOL] = 0.5 * dx * (r[32] + r[33]);
+    out[U1U1_D_MAX_THETA] = r[FR_MAXTH];
+    gauss_norms(r + FR_GAUSS, r + FR_GMAX, out + U1U1_D_GAUSS);
     return U1U1_OK;
 }
 
@@ -403,10 +510,7 @@ static int relayout(u1u1_ctx *ctx, float *canon, int to_canonical)
     cudaError_t e = launch_relayout(pos_buf(ctx, ctx->cur), mom_buf(ctx), canon, ctx->V, 0, 20, to_canonical, ctx->stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "relayout kernel launch");
     ctx->launches += 1;
-    if (!to_canonical) {
-        ctx->diag_valid = false;
-        ctx->labels_valid = false;
-    }
+    if (!to_canonical) invalidate(ctx);
     return U1U1_OK;
 }
 
@@ -432,8 +536,7 @@ extern "C" int u1u1_import_state_tiled(u1u1_ctx *ctx, const void *src_dev, int32
     cudaError_t e = launch_import_tiled(pos_buf(ctx, ctx->cur), mom_buf(ctx), (const float *)src_dev, ctx->V, ctx->N, n_src, ctx->stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "import_state_tiled launch");
     ctx->launches += 1;
-    ctx->diag_valid = false;
-    ctx->labels_valid = false;
+    invalidate(ctx);
     return U1U1_OK;
 }
 
@@ -451,31 +554,52 @@ extern "C" int u1u1_export_block(u1u1_ctx *ctx, int32_t x0, int32_t y0, int32_t 
     return U1U1_OK;
 }
 
-// Host variants: one canonical component at a time is gathered into (scattered from) the scratch buffer
-// by the relayout kernel and moved with cudaMemcpyAsync, so no second full-size device buffer is needed
-// (a canonical copy of a 1024^3 state would not fit beside the state).  Clobbers the winding scratch.
+// Host variants: one canonical component at a time is gathered into (scattered from) one of two staging planes in
+// the scratch work area by the relayout kernel, and moved by cudaMemcpyAsync on a second stream, so that the kernel
+// of component c+1 overlaps the PCIe copy of component c and no second full-size device buffer is needed (a canonical
+// copy of a 1024^3 state would not fit beside the state).  Clobbers the winding codes / segment labels, not the cells.
 static int host_copy(u1u1_ctx *ctx, void *host, int to_host)
 {
     const size_t V = ctx->V, bytes = V * sizeof(float);
-    float *stage = (float *)ctx->scratch;                 // scratch >= 8 V bytes >= one component plane
-    ctx->diag_valid = false;
-    ctx->labels_valid = false;
-    for (int c = 0; c < 20; c++) {
-        float *buf = stage;
-        float *h = (float *)host + (size_t)c * V;
-        cudaError_t e;
-        if (to_host) {
-            e = launch_relayout(pos_buf(ctx, ctx->cur), mom_buf(ctx), buf, V, c, 1, 1, ctx->stream);
-            if (e == cudaSuccess) e = cudaMemcpyAsync(h, buf, bytes, cudaMemcpyDeviceToHost, ctx->stream);
-        } else {
-            e = cudaMemcpyAsync(buf, h, bytes, cudaMemcpyHostToDevice, ctx->stream);
-            if (e == cudaSuccess) e = launch_relayout(pos_buf(ctx, ctx->cur), mom_buf(ctx), buf, V, c, 1, 0, ctx->stream);
+    cudaError_t e = cudaSuccess;
+    if (!ctx->copy_stream) {
+        e = cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking);
+        for (int b = 0; b < 2 && e == cudaSuccess; b++) {
+            e = cudaEventCreateWithFlags(&ctx->ev_kernel[b], cudaEventDisableTiming);
+            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_copy[b], cudaEventDisableTiming);
         }
-        if (e != cudaSuccess) return cuda_fail(ctx, e, "host<->device state copy");
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "host copy: creating the copy stream");
+    }
+    ctx->codes_valid = ctx->labels_valid = false;
+    if (!to_host) ctx->diag_valid = false;
+    float *stage[2] = {(float *)work_buf(ctx), (float *)work_buf(ctx) + V};
+    cudaStream_t ms = ctx->stream, cs = ctx->copy_stream;
+    // the copy stream starts after everything already queued on the caller's stream
+    e = cudaEventRecord(ctx->ev_kernel[0], ms);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(cs, ctx->ev_kernel[0], 0);
+    for (int c = 0; c < 20 && e == cudaSuccess; c++) {
+        const int b = c & 1;
+        float *h = (float *)host + (size_t)c * V;
+        if (to_host) {
+            if (c >= 2) e = cudaStreamWaitEvent(ms, ctx->ev_copy[b], 0);              // staging plane b is free again
+            if (e == cudaSuccess) e = launch_relayout(pos_buf(ctx, ctx->cur), mom_buf(ctx), stage[b], V, c, 1, 1, ms);
+            if (e == cudaSuccess) e = cudaEventRecord(ctx->ev_kernel[b], ms);
+            if (e == cudaSuccess) e = cudaStreamWaitEvent(cs, ctx->ev_kernel[b], 0);
+            if (e == cudaSuccess) e = cudaMemcpyAsync(h, stage[b], bytes, cudaMemcpyDeviceToHost, cs);
+            if (e == cudaSuccess) e = cudaEventRecord(ctx->ev_copy[b], cs);
+        } else {
+            if (c >= 2) e = cudaStreamWaitEvent(cs, ctx->ev_kernel[b], 0);            // its scatter kernel has run
+            if (e == cudaSuccess) e = cudaMemcpyAsync(stage[b], h, bytes, cudaMemcpyHostToDevice, cs);
+            if (e == cudaSuccess) e = cudaEventRecord(ctx->ev_copy[b], cs);
+            if (e == cudaSuccess) e = cudaStreamWaitEvent(ms, ctx->ev_copy[b], 0);
+            if (e == cudaSuccess) e = launch_relayout(pos_buf(ctx, ctx->cur), mom_buf(ctx), stage[b], V, c, 1, 0, ms);
+            if (e == cudaSuccess) e = cudaEventRecord(ctx->ev_kernel[b], ms);
+        }
         ctx->launches += 1;
     }
-    cudaError_t e = cudaStreamSynchronize(ctx->stream);
-    if (e != cudaSuccess) return cuda_fail(ctx, e, "host<->device state copy (sync)");
+    for (int b = 0; b < 2 && e == cudaSuccess; b++) e = cudaStreamWaitEvent(ms, ctx->ev_copy[b], 0);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ms);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "host<->device state copy");
     return U1U1_OK;
 }
 
@@ -499,11 +623,11 @@ extern "C" int u1u1_pq_segments(u1u1_ctx *ctx, int32_t min_cells, int32_t tolera
     if (min_cells < 1 || (tolerant != 0 && tolerant != 1)) return fail(ctx, U1U1_EINVAL, "need min_cells >= 1 and tolerant in {0, 1}");
     if (!ctx->diag_valid) return fail(ctx, U1U1_ESTATE, "pq_segments needs u1u1_diagnostics on the current state first");
     const size_t V = ctx->V;
-    // scratch: [codes 6V | cells 2V] -> [labels 4V | sizes 4V] (the sizes overlap the cells: zeroed after the mask is taken)
-    int *label = (int *)ctx->scratch, *size = (int *)(ctx->scratch + 4 * V);
-    cudaError_t e = launch_segments(ctx->scratch + 6 * V, V, ctx->N, tolerant, min_cells, label, size, partials(ctx),
-                                    result(ctx), ctx->stream);
-    ctx->diag_valid = false;
+    // scratch work area: [labels 4V | sizes 4V]; the cell arrays in front of it are only read
+    int *label = (int *)work_buf(ctx), *size = (int *)(work_buf(ctx) + 4 * V);
+    cudaError_t e = launch_segments(cells_buf(ctx), V, ctx->N, tolerant, min_cells, label, size, partials(ctx), result(ctx),
+                                    ctx->stream);
+    ctx->codes_valid = false;
     ctx->labels_valid = false;
     if (e != cudaSuccess) return cuda_fail(ctx, e, "pq_segments kernel launch");
     ctx->launches += 5;
@@ -525,7 +649,7 @@ extern "C" int u1u1_export_labels(u1u1_ctx *ctx, void *labels_dev)
 {
     if (!ctx || !labels_dev) return ctx ? fail(ctx, U1U1_EINVAL, "dst is NULL") : U1U1_EINVAL;
     if (!ctx->labels_valid) return fail(ctx, U1U1_ESTATE, "export_labels needs u1u1_pq_segments on the current state first");
-    cudaError_t e = cudaMemcpyAsync(labels_dev, ctx->scratch, ctx->V * sizeof(int), cudaMemcpyDeviceToDevice, ctx->stream);
+    cudaError_t e = cudaMemcpyAsync(labels_dev, work_buf(ctx), ctx->V * sizeof(int), cudaMemcpyDeviceToDevice, ctx->stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "labels copy");
     return U1U1_OK;
 }
@@ -537,14 +661,16 @@ extern "C" int u1u1_export_windings(u1u1_ctx *ctx, int32_t sector, void *w_dev, 
     if (!ctx->diag_valid) return fail(ctx, U1U1_ESTATE, "export_windings needs u1u1_diagnostics on the current state first");
     const size_t V = ctx->V;
     if (w_dev || near_dev) {
-        cudaError_t e = launch_decode_windings(ctx->scratch + (size_t)3 * sector * V, 3 * V, (int8_t *)w_dev,
+        // the sweep writes the per-plaquette codes (6 B/site) only on request: run it again in export mode
+        if (!ctx->codes_valid)
+            if (int rc = run_sweep(ctx, true)) return rc;
+        cudaError_t e = launch_decode_windings(work_buf(ctx) + (size_t)3 * sector * V, 3 * V, (int8_t *)w_dev,
                                                (uint8_t *)near_dev, ctx->stream);
         if (e != cudaSuccess) return cuda_fail(ctx, e, "decode_windings launch");
         ctx->launches += 1;
     }
     if (cells_dev) {
-        cudaError_t e = cudaMemcpyAsync(cells_dev, ctx->scratch + 6 * V + (size_t)sector * V, V,
-                                        cudaMemcpyDeviceToDevice, ctx->stream);
+        cudaError_t e = cudaMemcpyAsync(cells_dev, cells_buf(ctx) + (size_t)sector * V, V, cudaMemcpyDeviceToDevice, ctx->stream);
         if (e != cudaSuccess) return cuda_fail(ctx, e, "cells copy");
     }
     return U1U1_OK;

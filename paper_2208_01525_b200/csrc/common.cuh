@@ -86,7 +86,7 @@ struct DiagCoef {
 // a one-block kernel folds the partials.  No atomics, so results are bit-reproducible run to run.
 // ------------------------------------------------------------------------------------------------
 constexpr int RED_BLOCK = 256;
-constexpr int RED_MAX_BLOCKS = 148 * 8;
+constexpr int RED_MAX_BLOCKS = 1184;     // cap on reduction / grid-stride blocks: sizes the partials buffer, device independent
 constexpr int RED_SLOTS = 32;
 
 __device__ inline double warp_sum(double v)

@@ -154,7 +154,7 @@ __global__ void export_block_kernel(const float *pos, const float *mom, size_t V
     }
 }
 
-constexpr int GRID = 148 * 8;
+constexpr int GRID = RED_MAX_BLOCKS;      // grid-stride kernels: a few blocks per SM on any device
 
 }  // namespace
 

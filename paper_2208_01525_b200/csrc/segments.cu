@@ -88,31 +88,36 @@ __global__ void seg_merge_kernel(int *label, size_t V, int N)
     }
 }
 
-__global__ void seg_flatten_count_kernel(int *label, int *size, size_t V)
+// size[root] counts HALF cells: a cell adds (pierced by p) + (pierced by q), i.e. 2 for an exact-overlap cell and 1 for a
+// cell that belongs to the region by the one-cell tolerance only (reading R-21b: a region's cell count is
+// (its p cells + its q cells) / 2, so a displaced pair of lines is as long as a coincident one)
+__global__ void seg_flatten_count_kernel(int *label, int *size, const uint8_t *cells, size_t V)
 {
     for (size_t lin = (size_t)blockIdx.x * blockDim.x + threadIdx.x; lin < V; lin += (size_t)gridDim.x * blockDim.x) {
         if (label[lin] < 0) continue;
         const int r = find_root(label, (int)lin);
         label[lin] = r;             // roots keep label == index; concurrent readers see either a valid ancestor or the root
-        atomicAdd(&size[r], 1);
+        atomicAdd(&size[r], (cells[lin] > 0) + (cells[V + lin] > 0));
     }
 }
 
-// Partials: [segments >= min_cells, sum (n - 1) over them, cells in them, all segments, all pq cells | largest n]
+// Partials: [segments with n >= min_cells, sum (n - 1) over them, cells n in them, all segments, all pq cells | largest n],
+// n = size / 2 (may be a half-integer for tolerant regions)
 __global__ void __launch_bounds__(RED_BLOCK) seg_reduce_kernel(const int *label, const int *size, size_t V,
                                                                int min_cells, double *partials)
 {
     double acc[6] = {0, 0, 0, 0, 0, 0};
     for (size_t lin = (size_t)blockIdx.x * blockDim.x + threadIdx.x; lin < V; lin += (size_t)gridDim.x * blockDim.x) {
         if (label[lin] != (int)lin) continue;        // roots only
-        const int n = size[lin];
+        const int n2 = size[lin];
+        const double n = 0.5 * (double)n2;
         acc[3] += 1.0;
-        acc[4] += (double)n;
-        acc[5] = fmax(acc[5], (double)n);
-        if (n >= min_cells) {
+        acc[4] += n;
+        acc[5] = fmax(acc[5], n);
+        if (n2 >= 2 * min_cells) {
             acc[0] += 1.0;
-            acc[1] += (double)(n - 1);
-            acc[2] += (double)n;
+            acc[1] += n - 1.0;
+            acc[2] += n;
         }
     }
     block_reduce_store<6>(acc, 5, partials);
@@ -120,18 +125,16 @@ __global__ void __launch_bounds__(RED_BLOCK) seg_reduce_kernel(const int *label,
 
 }  // namespace
 
-cudaError_t launch_fold(const double *partials, int nblocks, int nval, int n_sum, double *result, cudaStream_t st);
-
 cudaError_t launch_segments(const uint8_t *cells, size_t V, int N, int tolerant, int min_cells, int *label, int *size,
                             double *partials, double *result, cudaStream_t st)
 {
     const size_t need = (V + RED_BLOCK - 1) / RED_BLOCK;
     const int nb = (int)(need < (size_t)RED_MAX_BLOCKS ? need : (size_t)RED_MAX_BLOCKS);
     seg_init_kernel<<<nb, RED_BLOCK, 0, st>>>(cells, V, N, tolerant, label);
-    cudaError_t e = cudaMemsetAsync(size, 0, V * sizeof(int), st);        // overlaps the cell arrays: after init
+    cudaError_t e = cudaMemsetAsync(size, 0, V * sizeof(int), st);
     if (e != cudaSuccess) return e;
     seg_merge_kernel<<<nb, RED_BLOCK, 0, st>>>(label, V, N);
-    seg_flatten_count_kernel<<<nb, RED_BLOCK, 0, st>>>(label, size, V);
+    seg_flatten_count_kernel<<<nb, RED_BLOCK, 0, st>>>(label, size, cells, V);
     seg_reduce_kernel<<<nb, RED_BLOCK, 0, st>>>(label, size, V, min_cells, partials);
     e = launch_fold(partials, nb, 6, 5, result, st);
     return e != cudaSuccess ? e : cudaGetLastError();

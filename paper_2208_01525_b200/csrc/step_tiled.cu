@@ -13,101 +13,22 @@
 // Every stencil operand is a vector read from shared memory, and each site's 20 words make one HBM round
 // trip: positions in through the ring (+ halo, served by L2), momenta in, 3 + 3 vector stores out (new
 // positions to the other ping-pong buffer, momenta in place).
-#include <cuda.h>
 #include <cstring>
 
 #include "common.cuh"
 #include "kernels.h"
+#include "stage.cuh"
 
 namespace u1u1 {
 
 namespace {
 
-constexpr int TX = 32;              // tile width  (one warp along x)
-constexpr int TY = 8;               // tile height (one warp per row)
-constexpr int NTHREADS = TX * TY;
-constexpr int ROWS = TY + 2;        // + halo rows y0-1, y0+wy
-constexpr int COLS = TX + 2;        // + halo columns x0-1, x0+wx
-constexpr int NELEM = ROWS * COLS;  // staged sites per plane (340)
-// one ring slot: A float4[NELEM] | B float4[NELEM] | C float2[NELEM], each 128-byte aligned (TMA destination)
-// TMA needs a 16-byte aligned box origin: pack C (8 B per site) is staged from x0-2, i.e. CCOLS = COLS + 2 columns
-// per row with site column c at index c + 1.
-constexpr int CCOLS = COLS + 2;
-constexpr int OFF_B = 5504, OFF_C = 11008, SLOT_BYTES = 13952;
-constexpr int POS_TX_BYTES = NELEM * 32 + ROWS * CCOLS * 8;    // bytes one plane's three boxes deliver
 constexpr int NSLOT = 4;            // ring: z, z+1 in use, z+2 and z+3 in flight
-constexpr int NITEM = (3 * NELEM + NTHREADS - 1) / NTHREADS;   // cp.async copies per thread per plane (4)
 // momentum ring (TMA tiles only): 2 slots of MA float4[NTHREADS] | MB float4[NTHREADS] | MC float2[NTHREADS]
 constexpr int MOFF_B = NTHREADS * 16, MOFF_C = NTHREADS * 32, MSLOT_BYTES = NTHREADS * 40;
 constexpr int OFF_MRING = NSLOT * SLOT_BYTES;
 constexpr int OFF_BARS = OFF_MRING + 2 * MSLOT_BYTES;           // fullP[4], fullM[2]
 constexpr int SMEM_BYTES = OFF_BARS + 64;                       // 76 352 B -> 3 CTAs per SM
-static_assert(NELEM * 16 <= OFF_B && OFF_B + NELEM * 16 <= OFF_C && OFF_C + ROWS * CCOLS * 8 <= SLOT_BYTES, "slot layout");
-
-// Tensor maps of one launch: position packs of the buffer being read (boxes with halo), momentum packs.
-struct alignas(64) StepMaps {
-    CUtensorMap pA, pB, pC, mA, mB, mC;
-};
-
-__device__ inline unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
-
-__device__ inline void cp_async16(unsigned sdst, const void *gsrc)
-{
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(sdst), "l"(gsrc) : "memory");
-}
-__device__ inline void cp_async8(unsigned sdst, const void *gsrc)
-{
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(sdst), "l"(gsrc) : "memory");
-}
-__device__ inline unsigned long long policy_evict_first()
-{
-    unsigned long long pol;
-    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;\n" : "=l"(pol));
-    return pol;
-}
-__device__ inline unsigned long long policy_evict_last()
-{
-    unsigned long long pol;
-    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;\n" : "=l"(pol));
-    return pol;
-}
-__device__ inline void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
-template <int N_>
-__device__ inline void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N_) : "memory"); }
-
-__device__ inline void mbar_init(unsigned bar, unsigned count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(bar), "r"(count) : "memory");
-}
-__device__ inline void mbar_expect_tx(unsigned bar, unsigned bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(bar), "r"(bytes) : "memory");
-}
-__device__ inline void mbar_wait(unsigned bar, unsigned parity)
-{
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "WAIT_LOOP:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra WAIT_DONE;\n"
-        "bra WAIT_LOOP;\n"
-        "WAIT_DONE:\n"
-        "}\n" ::"r"(bar), "r"(parity)
-        : "memory");
-}
-// TMA box load of a 3-d (W x + component, y, z) float tensor with an L2 eviction policy: evict-first for data
-// read exactly once (the momenta), evict-last for the position planes, which the neighbouring tiles re-read as halo
-__device__ inline void tma_load_3d_hint(unsigned sdst, const CUtensorMap *map, int c0, int c1, int c2, unsigned bar,
-                                          unsigned long long pol)
-{
-    asm volatile(
-        "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%2, %3, %4}], [%5], %6;\n" ::
-            "r"(sdst), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(bar), "l"(pol)
-        : "memory");
-}
-
-__device__ inline int wrapi(int v, int N) { return v < 0 ? v + N : (v >= N ? v - N : v); }
 
 // exp(-i theta): libm sincosf (1-2 ulp) or, with FAST, the SFU approximations.  MUFU.SIN/COS take the angle
 // in turns and reduce it themselves (one FMUL by 1/(2 pi) + 2 MUFU); error max(5e-7, 6e-8 |theta|).  The
@@ -170,52 +91,29 @@ step_tiled_kernel(Lattice L, StepCoef k, int zchunk, int band, const __grid_cons
     const int wx = min(TX, N - x0), wy = min(TY, N - y0), nz = min(zchunk, N - z0);
     const bool active = tx < wx && ty < wy;
     // TMA boxes cannot wrap: only tiles whose halo lies inside the lattice take the TMA path (CTA-uniform)
-    const bool tma = !(k.flags & 2) && x0 >= 2 && x0 + TX + 2 <= N && y0 >= 1 && y0 + TY + 1 <= N;
+    const bool tma = !(k.flags & 2) && tile_is_interior(x0, y0, N);
     const bool tmom = tma && !(k.flags & 4);        // momenta by TMA boxes (default on TMA tiles), else ld.global.cs
     const char *pos = reinterpret_cast<const char *>(L.pos_in);
     const unsigned long long pol_stream = policy_evict_first();
     const unsigned long long pol_keep = policy_evict_last();
 
     // ---- staging of relative plane j (z = z0 + j, j = -1 .. nz) into ring slot (j + 1) & 3 ----
-    int plan_lin[NITEM];          // cp.async path: in-plane site index of each of this thread's copies (-1: none)
-    if (!tma) {
-#pragma unroll
-        for (int q = 0; q < NITEM; q++) {
-            const int item = tid + q * NTHREADS;
-            const int pack = item / NELEM, e = item - pack * NELEM, r = e / COLS, c = e - r * COLS;
-            const int y = wrapi(r == wy + 1 ? y0 + wy : y0 - 1 + r, N), x = wrapi(c == wx + 1 ? x0 + wx : x0 - 1 + c, N);
-            plan_lin[q] = (pack < 3 && r <= wy + 1 && c <= wx + 1) ? y * N + x : -1;
-        }
-    }
+    CpPlan plan;                  // cp.async path: this thread's copies of one halo plane
+    if (!tma) make_cp_plan(plan, tid, x0, y0, wx, wy, N);
     auto stage_cp = [&](int j) {          // every thread; caller commits the group
-        const size_t zp = (size_t)wrapi(z0 + j, N) * NN;
-        const unsigned slot = sbase + ((j + 1) & 3) * SLOT_BYTES;
-#pragma unroll
-        for (int q = 0; q < NITEM; q++) {
-            if (plan_lin[q] < 0) continue;
-            const int item = tid + q * NTHREADS;
-            const int pack = item < NELEM ? 0 : item < 2 * NELEM ? 1 : 2, e = item - pack * NELEM;
-            const size_t site = zp + (size_t)plan_lin[q];
-            if (pack == 0) cp_async16(slot + e * 16, pos + site * 16);
-            else if (pack == 1) cp_async16(slot + OFF_B + e * 16, pos + 16 * V + site * 16);
-            else cp_async8(slot + OFF_C + (e + 2 * (e / COLS) + 1) * 8, pos + 32 * V + site * 8);
-        }
+        stage_plane_cp(plan, tid, pos, V, (size_t)wrapi(z0 + j, N) * NN, sbase + ((j + 1) & 3) * SLOT_BYTES);
     };
     auto stage_tma = [&](int j) {         // one thread
-        const int z = wrapi(z0 + j, N);
-        const unsigned slot = sbase + ((j + 1) & 3) * SLOT_BYTES, bar = bars + 8 * ((j + 1) & 3);
-        mbar_expect_tx(bar, POS_TX_BYTES);
         // evict-last: the neighbouring tiles re-read these lines as halo within a few planes (measured: -1 % DRAM reads)
-        tma_load_3d_hint(slot, &maps.pA, 4 * (x0 - 1), y0 - 1, z, bar, pol_keep);
-        tma_load_3d_hint(slot + OFF_B, &maps.pB, 4 * (x0 - 1), y0 - 1, z, bar, pol_keep);
-        tma_load_3d_hint(slot + OFF_C, &maps.pC, 2 * (x0 - 2), y0 - 1, z, bar, pol_keep);
+        stage_plane_tma(maps.pos, x0, y0, wrapi(z0 + j, N), sbase + ((j + 1) & 3) * SLOT_BYTES, bars + 8 * ((j + 1) & 3),
+                        pol_keep);
     };
     auto stage_mom_tma = [&](int m) {     // one thread; momenta of relative plane m into ring slot m & 1
         const unsigned slot = sbase + OFF_MRING + (m & 1) * MSLOT_BYTES, bar = bars + 8 * (4 + (m & 1));
         mbar_expect_tx(bar, MSLOT_BYTES);
-        tma_load_3d_hint(slot, &maps.mA, 4 * x0, y0, z0 + m, bar, pol_stream);
-        tma_load_3d_hint(slot + MOFF_B, &maps.mB, 4 * x0, y0, z0 + m, bar, pol_stream);
-        tma_load_3d_hint(slot + MOFF_C, &maps.mC, 2 * x0, y0, z0 + m, bar, pol_stream);
+        tma_load_3d_hint(slot, &maps.mom.A, 4 * x0, y0, z0 + m, bar, pol_stream);
+        tma_load_3d_hint(slot + MOFF_B, &maps.mom.B, 4 * x0, y0, z0 + m, bar, pol_stream);
+        tma_load_3d_hint(slot + MOFF_C, &maps.mom.C, 2 * x0, y0, z0 + m, bar, pol_stream);
     };
 
     // ---- prologue: planes -1 .. 2 in flight, wait for -1 and 0 ----
@@ -223,7 +121,7 @@ step_tiled_kernel(Lattice L, StepCoef k, int zchunk, int band, const __grid_cons
         if (tid == 0) {
 #pragma unroll
             for (int b = 0; b < 6; b++) mbar_init(bars + 8 * b, 1);
-            asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+            mbar_fence_init();
         }
         __syncthreads();
         if (tid == 0) {
@@ -444,97 +342,37 @@ step_tiled_kernel(Lattice L, StepCoef k, int zchunk, int band, const __grid_cons
     if (!tma) cp_async_wait<0>();
 }
 
-int pick_zchunk(int N)
+int pick_zchunk(int N, int sms)
 {
-    // enough CTAs to fill 148 SMs x 3 several times over, chunks long enough to amortise the 2-plane prologue --
+    // enough CTAs to fill the SMs x 3 several times over, chunks long enough to amortise the 2-plane prologue --
     // but no longer: neighbouring CTAs drift apart while they march, and a halo line that the neighbour fetched too
     // long ago has left L2.  With the band launch order below the two boundary planes of a chunk are re-read by the
     // very next wave, so short chunks cost little (measured at 1024^3, band order: 8 planes 29.65 ms, 12: 29.2,
     // 16: 29.05, 24: 29.25, 32: 29.45; plain 3-d grid order: 32: 29.8, 64: 30.6, 128: 32.3, 512: 34.6)
     const int tiles = ((N + TX - 1) / TX) * ((N + TY - 1) / TY);
     int zc = 16;
-    while (zc > 8 && (long)tiles * ((N + zc - 1) / zc) < 148L * 3 * 4) zc >>= 1;
+    while (zc > 8 && (long)tiles * ((N + zc - 1) / zc) < (long)sms * 3 * 4) zc >>= 1;
     return zc < N ? zc : N;
 }
 
-// ---- tensor maps (host) -------------------------------------------------------------------------------
-typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
-                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
-                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-
-EncodeTiledFn encode_fn()
-{
-    static EncodeTiledFn fn = nullptr;
-    static bool tried = false;
-    if (!tried) {
-        tried = true;
-        void *p = nullptr;
-        cudaDriverEntryPointQueryResult q;
-        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
-            q == cudaDriverEntryPointSuccess)
-            fn = (EncodeTiledFn)p;
-    }
-    return fn;
-}
-
-// A pack of W floats per site at `base`: 3-d float tensor (W x + component, y, z), box (W bx, by, 1): x and the
-// component form ONE contiguous innermost run, so a box row is a single bx*W*4-byte request.  The box origin
-// must be 16-byte aligned, i.e. (W x) a multiple of 4 floats: any x for W = 4, even x for W = 2.
-bool encode_pack(CUtensorMap *m, const float *base, int W, int N, int bx, int by)
-{
-    const cuuint64_t n = (cuuint64_t)N, w = (cuuint64_t)W;
-    const cuuint64_t dims[3] = {w * n, n, n}, strides[2] = {4 * w * n, 4 * w * n * n};
-    const cuuint32_t box[3] = {(cuuint32_t)(W * bx), (cuuint32_t)by, 1}, es[3] = {1, 1, 1};
-    return encode_fn()(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, (void *)base, dims, strides, box, es,
-                       CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
-                       CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
-}
-
-// Maps are pure functions of (buffer addresses, N); a context alternates between two position buffers, so a
-// tiny cache avoids re-encoding on every launch.
-struct MapCacheEntry {
-    const float *pos = nullptr, *mom = nullptr;
-    int N = 0;
-    StepMaps maps;
-};
-
-bool get_maps(const Lattice &L, StepMaps &out)
-{
-    static MapCacheEntry cache[4];
-    static int next = 0;
-    for (auto &c : cache)
-        if (c.pos == L.pos_in && c.mom == L.mom && c.N == L.N) { out = c.maps; return true; }
-    if (!encode_fn()) return false;
-    MapCacheEntry &c = cache[next];
-    next = (next + 1) & 3;
-    const size_t V = L.V;
-    const bool ok = encode_pack(&c.maps.pA, L.pos_in, 4, L.N, COLS, ROWS) && encode_pack(&c.maps.pB, L.pos_in + 4 * V, 4, L.N, COLS, ROWS) &&
-                    encode_pack(&c.maps.pC, L.pos_in + 8 * V, 2, L.N, CCOLS, ROWS) && encode_pack(&c.maps.mA, L.mom, 4, L.N, TX, TY) &&
-                    encode_pack(&c.maps.mB, L.mom + 4 * V, 4, L.N, TX, TY) && encode_pack(&c.maps.mC, L.mom + 8 * V, 2, L.N, TX, TY);
-    if (!ok) { c.pos = nullptr; return false; }
-    c.pos = L.pos_in; c.mom = L.mom; c.N = L.N;
-    out = c.maps;
-    return true;
-}
-
 template <bool FAST, typename R, bool DIFF>
-cudaError_t launch_one(const Lattice &L, StepCoef k, cudaStream_t st)
+cudaError_t launch_one(const Lattice &L, StepCoef k, cudaStream_t st, const StepMaps *m, int sms)
 {
     // per device and cheap: set on every launch rather than caching a per-process flag
     cudaError_t ea = cudaFuncSetAttribute(step_tiled_kernel<FAST, R, DIFF>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
     if (ea != cudaSuccess) return ea;
     StepMaps maps;
-    if (L.N < COLS + 2) {
+    if (!m) {
         memset(&maps, 0, sizeof maps);
         k.flags |= 2;                       // no tile can lie strictly inside such a lattice: cp.async path only
-    } else if (!get_maps(L, maps)) {
-        return cudaErrorNotSupported;       // cuTensorMapEncodeTiled unavailable or rejected the layout: fail loudly
+    } else {
+        maps = *m;
     }
-    const int zc = pick_zchunk(L.N);
+    const int zc = pick_zchunk(L.N, sms);
     const int ntx = (L.N + TX - 1) / TX, nty = (L.N + TY - 1) / TY, nzc = (L.N + zc - 1) / zc;
-    // band height = the tile rows one wave of resident CTAs covers (148 SMs x CTAs per SM / tiles per row)
+    // band height = the tile rows one wave of resident CTAs covers (SMs x CTAs per SM / tiles per row)
     const int per_sm = sizeof(R) == 8 ? 2 : 3;
-    int band = (k.flags & 8) ? nty : (148 * per_sm + ntx - 1) / ntx;     // tuning flag 8: the order of a plain 3-d grid
+    int band = (k.flags & 8) ? nty : (sms * per_sm + ntx - 1) / ntx;     // tuning flag 8: the order of a plain 3-d grid
     if (band > nty) band = nty;
     const unsigned grid = (unsigned)ntx * nty * nzc;
     step_tiled_kernel<FAST, R, DIFF><<<grid, NTHREADS, SMEM_BYTES, st>>>(L, k, zc, band, maps);
@@ -546,16 +384,19 @@ cudaError_t launch_one(const Lattice &L, StepCoef k, cudaStream_t st)
 bool step_tiled_supports(int N) { return N >= 8 && (N % 4) == 0; }
 
 // mode bit 0: SFU sin/cos; bit 1: fp32 kick chain (default is the fp64 chain); 4 / 5: fp32 chain in difference form
-cudaError_t launch_step_tiled(const Lattice &L, const StepCoef &k, cudaStream_t st, int mode)
+// maps: tensor maps of (L.pos_in, L.mom), or NULL for lattices too small for any interior tile; sms = SM count
+cudaError_t launch_step_tiled(const Lattice &L, const StepCoef &k, cudaStream_t st, int mode, const StepMaps *maps, int sms)
 {
     switch (mode) {
-        case 0: return launch_one<false, double, false>(L, k, st);
-        case 1: return launch_one<true, double, false>(L, k, st);
-        case 2: return launch_one<false, float, false>(L, k, st);
-        case 3: return launch_one<true, float, false>(L, k, st);
-        case 4: return launch_one<false, float, true>(L, k, st);
-        default: return launch_one<true, float, true>(L, k, st);
+        case 0: return launch_one<false, double, false>(L, k, st, maps, sms);
+        case 1: return launch_one<true, double, false>(L, k, st, maps, sms);
+        case 2: return launch_one<false, float, false>(L, k, st, maps, sms);
+        case 3: return launch_one<true, float, false>(L, k, st, maps, sms);
+        case 4: return launch_one<false, float, true>(L, k, st, maps, sms);
+        default: return launch_one<true, float, true>(L, k, st, maps, sms);
     }
 }
+
+bool step_tiled_uses_tma(int N) { return N >= COLS + 2; }
 
 }  // namespace u1u1

@@ -56,11 +56,10 @@ def run(config: int, size: int | None = None, variant: int = 0, segments: bool =
         if done % c["every"] == 0 or done == total:
             torch.cuda.synchronize()
             td = time.perf_counter()
-            g = lat.gauss_violation()
-            d = lat.diagnostics()
+            d = lat.diagnostics()                 # one sweep: windings, cells, sums AND the Gauss-law norms
             row = {k: d[k] for k in KEYS}
-            row.update(step=done, prephase=done <= c["pre"] and c["pre"] > 0, gauss_rel_p=g[3], gauss_rel_q=g[7],
-                       gauss_max_p=g[2])
+            row.update(step=done, prephase=done <= c["pre"] and c["pre"] > 0, gauss_rel_p=d["gauss_rel_p"],
+                       gauss_rel_q=d["gauss_rel_q"], gauss_max_p=d["gauss_max_p"], max_theta=d["max_theta"])
             if segments:
                 row["segments"] = lat.pq_segments(8, True)
             t_diag += time.perf_counter() - td

@@ -98,6 +98,9 @@ def test_sampled_windings_full_size():
         assert d["sumW_p" if sec == 0 else "sumW_q"] == float(W.abs().sum(dtype=torch.int64))
         del W, near, cells
     assert checked > 15000 and nonzero > 0          # random-phase start: plenty of strings in any block
+    # near-cut plaquettes are judged, not just excluded: expected 4e-5/pi of all plaquettes per sector
+    assert flagged <= 1e-4 * (checked + flagged) + 3, flagged
+    assert 0 < d["near_p"] <= 1e-4 * 3 * N ** 3 and 0 < d["near_q"] <= 1e-4 * 3 * N ** 3
 
 
 def test_tiled_state_full_size_every_kernel():
