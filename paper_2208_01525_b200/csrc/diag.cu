@@ -72,48 +72,58 @@ __device__ inline int decode_w(uint8_t code) { return (int)(code & 15) - 8; }
 
 // Fast method with one cell of tolerance ("non-zero at the same location, or displaced by one cell in
 // any direction"; reading R-13b): a pierced p cell counts if a pierced q cell lies in its periodic 3x3x3
-// neighbourhood, and vice versa.  Four consecutive x cells per thread as one 32-bit word per type (N is a multiple of
-// 4); a word with no pierced cell of either type (the common case once the network has thinned out) costs two loads.
-// Otherwise the other type's cells are dilated over the neighbourhood with word operations: OR of the 9 (dy, dz)
-// rows, then OR with the row shifted one byte left and right (the bytes at x - 1 and x + 4 shifted in).
-// Partials: [#p cells with a q cell within one cell, #q cells with a p cell within one cell].
+// neighbourhood, and vice versa.  The dilation is separable.  A thread owns four consecutive x cells (one 32-bit word
+// per type; N is a multiple of 4) of one row y and marches through a chunk of z planes: per plane it ORs the words
+// of rows y-1, y, y+1 (plus the bytes at x-1 and x+4) into a bit per cell, spreads that bit one cell left and right,
+// and keeps the results of planes z-1, z, z+1 in registers -- 18 loads per four cells instead of 54, whatever the
+// string density.  Partials: [#p cells with a q cell within one cell, #q cells with a p cell within one cell].
+constexpr int TOL_ZC = 32;
 __global__ void __launch_bounds__(RED_BLOCK) overlap_tol_kernel(const uint8_t *cells, size_t V, int N, double *partials)
 {
     const Wrap w{N};
-    const int nw = N / 4;                                     // words per row
+    const int nw = N / 4, nzc = (N + TOL_ZC - 1) / TOL_ZC;
+    const size_t NN = (size_t)N * N, ncol = (size_t)nw * N * nzc;
     int acc[2] = {0, 0};
     auto nonzero_bytes = [](uint32_t v) {                     // 0x01 in every byte lane of v that is non-zero
         v |= v >> 4; v |= v >> 2; v |= v >> 1;
         return v & 0x01010101u;
     };
-    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < V / 4; q += (size_t)gridDim.x * blockDim.x) {
-        const uint32_t cp = reinterpret_cast<const uint32_t *>(cells)[q], cq = reinterpret_cast<const uint32_t *>(cells + V)[q];
-        if ((cp | cq) == 0) continue;
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < ncol; q += (size_t)gridDim.x * blockDim.x) {
         const int xw = (int)(q % (size_t)nw);
         const size_t r = q / (size_t)nw;
-        const int y = (int)(r % (size_t)N), z = (int)(r / (size_t)N);
+        const int y = (int)(r % (size_t)N), z0 = (int)(r / (size_t)N) * TOL_ZC, nz = min(TOL_ZC, N - z0);
         const int x = 4 * xw, xl = w.m(x), xr = x + 4 == N ? 0 : x + 4;
-        const int ys[3] = {w.m(y), y, w.p(y)}, zs[3] = {w.m(z), z, w.p(z)};
-        uint32_t mid[2] = {0, 0}, lft[2] = {0, 0}, rgt[2] = {0, 0};
-        for (int c = 0; c < 3; c++)
-            for (int b = 0; b < 3; b++) {
-                const size_t row = (size_t)N * ((size_t)ys[b] + (size_t)N * zs[c]);
+        const size_t rows[3] = {(size_t)w.m(y) * N, (size_t)y * N, (size_t)w.p(y) * N};
+        // xy-dilated pierced bits (0x01 per cell) of both types in plane z
+        auto plane = [&](int z, uint32_t &dp, uint32_t &dq, uint32_t &cp, uint32_t &cq) {
+            const size_t zp = (size_t)z * NN;
+            uint32_t mid[2] = {0, 0}, lft[2] = {0, 0}, rgt[2] = {0, 0}, own[2];
 #pragma unroll
-                for (int t = 0; t < 2; t++) {
-                    const uint8_t *src = cells + (size_t)t * V + row;
-                    mid[t] |= *reinterpret_cast<const uint32_t *>(src + x);
+            for (int t = 0; t < 2; t++) {
+#pragma unroll
+                for (int b = 0; b < 3; b++) {
+                    const uint8_t *src = cells + (size_t)t * V + zp + rows[b];
+                    const uint32_t m = *reinterpret_cast<const uint32_t *>(src + x);
+                    if (b == 1) own[t] = m;
+                    mid[t] |= m;
                     lft[t] |= src[xl];
                     rgt[t] |= src[xr];
                 }
+                const uint32_t m = nonzero_bytes(mid[t]);
+                mid[t] = m | (m << 8) | (lft[t] ? 1u : 0u) | (m >> 8) | (rgt[t] ? 0x01000000u : 0u);
             }
-        uint32_t dil[2];
-#pragma unroll
-        for (int t = 0; t < 2; t++) {
-            const uint32_t m = nonzero_bytes(mid[t]), l = lft[t] ? 1u : 0u, g = rgt[t] ? 1u : 0u;
-            dil[t] = m | (m << 8) | l | (m >> 8) | (g << 24);
+            dp = mid[0]; dq = mid[1]; cp = own[0]; cq = own[1];
+        };
+        uint32_t dpm, dqm, dpc, dqc, dpn, dqn, cpc, cqc, cpn, cqn, u0, u1;
+        plane(w.m(z0), dpm, dqm, u0, u1);
+        plane(z0, dpc, dqc, cpc, cqc);
+        for (int iz = 0; iz < nz; iz++) {
+            const int z = z0 + iz;
+            plane(w.p(z), dpn, dqn, cpn, cqn);
+            acc[0] += __popc(nonzero_bytes(cpc) & (dqm | dqc | dqn));
+            acc[1] += __popc(nonzero_bytes(cqc) & (dpm | dpc | dpn));
+            dpm = dpc; dqm = dqc; dpc = dpn; dqc = dqn; cpc = cpn; cqc = cqn;
         }
-        acc[0] += __popc(nonzero_bytes(cp) & dil[1]);
-        acc[1] += __popc(nonzero_bytes(cq) & dil[0]);
     }
     const double a[2] = {(double)acc[0], (double)acc[1]};
     block_reduce_store<2>(a, 2, partials);

@@ -26,29 +26,31 @@ namespace u1u1 {
 
 namespace {
 
-constexpr int NSLOT = 4;                                   // position ring: planes z, z+1 in use, z+2, z+3 in flight
-constexpr int NMSLOT = 2;                                  // momentum ring: plane z in use, z+1 in flight
+constexpr int NSLOT = 3;                                   // position ring: planes z, z+1 in use, z+2 in flight
+constexpr int MSLOT_BYTES = 5504;                          // momentum ring slot: pack B (E_x, E_y, H_x, H_y) with halo
 constexpr int OFF_MRING = NSLOT * SLOT_BYTES;
-constexpr int OFF_ALPHA = OFF_MRING + NMSLOT * SLOT_BYTES; // float [2 planes][2 sectors][NELEM]
+constexpr int OFF_ALPHA = OFF_MRING + 2 * MSLOT_BYTES;     // float [2 planes][2 sectors][NELEM]
 constexpr int OFF_XY = OFF_ALPHA + 2 * 2 * NELEM * 4;      // uint2 [2 planes][NELEM]: wrap counts of the x and y links
 constexpr int OFF_Z = OFF_XY + 2 * NELEM * 8;              // uint  [NELEM]: wrap counts of the z links of plane z
-constexpr int OFF_RED = OFF_Z + NELEM * 4;                 // double [FUSED_NRES][NTHREADS / 32]
+constexpr int OFF_RED = OFF_Z + NELEM * 4;                 // double [FUSED_NRES][NTHREADS / 32]: per-warp accumulators
 constexpr int OFF_BARS = OFF_RED + FUSED_NRES * (NTHREADS / 32) * 8;
-constexpr int SMEM_BYTES = OFF_BARS + 64;
+constexpr int SMEM_BYTES = OFF_BARS + 64;                  // 66.6 KB -> 3 CTAs per SM
+static_assert(NELEM * 16 <= MSLOT_BYTES && MSLOT_BYTES % 128 == 0, "momentum slot");
 static_assert(OFF_ALPHA % 16 == 0 && OFF_XY % 16 == 0 && OFF_RED % 8 == 0 && OFF_BARS % 8 == 0, "alignment");
 
 constexpr float INV_2PI = 0.15915494309189535f;
 constexpr float NEAR_T = 0.5f - 1.5915494e-6f;             // pi - |chi| < 1e-5  <=>  |t - rint t| > 1/2 - 1e-5 / 2 pi
-constexpr unsigned BIAS = 32u;                             // wrap counts are stored as n + 32 in a byte lane
 constexpr unsigned FLAG_LANES = 0xff00ff00u, VAL_LANES = 0x00ff00ffu;   // lanes 0 / 2: p / q values, lanes 1 / 3: their flags
 
 // atan2 in ~20 instructions: octant reduction to t = min/max in [0, 1] and the degree-8 (in t^2) polynomial of
-// Abramowitz & Stegun 4.4.49 (|error| <= 2e-8 in exact arithmetic; ~4e-7 in fp32 with the fast division).
-// Never called with x = y = 0.
-__device__ inline float atan2_poly(float y, float x)
+// Abramowitz & Stegun 4.4.49 (|error| <= 2e-8 in exact arithmetic; ~4e-7 in fp32 with the SFU reciprocal).
+// A field that is exactly zero has no phase: NaN, which marks the links that touch it as degenerate.
+__device__ inline float site_phase(float x, float y)
 {
-    const float ax = fabsf(x), ay = fabsf(y);
-    const float t = __fdividef(fminf(ax, ay), fmaxf(ax, ay)), s = t * t;
+    const float ax = fabsf(x), ay = fabsf(y), mx = fmaxf(ax, ay);
+    float inv;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(inv) : "f"(mx));
+    const float t = fminf(ax, ay) * inv, s = t * t;
     float p = 0.0028662257f;
     p = fmaf(p, s, -0.0161657367f);
     p = fmaf(p, s, 0.0429096138f);
@@ -60,45 +62,29 @@ __device__ inline float atan2_poly(float y, float x)
     float r = fmaf(p * s, t, t);
     r = ay > ax ? 1.57079637f - r : r;
     r = x < 0.f ? 3.14159274f - r : r;
-    return copysignf(r, y);
-}
-// phase of a site, NaN if the field is exactly zero there (the links that touch it are "degenerate")
-__device__ inline float site_phase(float re, float im)
-{
-    return (re == 0.f && im == 0.f) ? __int_as_float(0x7fc00000) : atan2_poly(im, re);
+    r = copysignf(r, y);
+    return mx == 0.f ? __int_as_float(0x7fc00000) : r;
 }
 
-// One link: wrap count n = rint(t) as a biased byte (valid for |n| <= 31, i.e. |theta| < 190; the host checks the
-// largest |theta| of the sweep), flags in the next byte: bit 0 = within 1e-5 of the cut, bit 2 = degenerate.
+// One link as a byte lane: wrap count n = rint(t) stored as n + 32 (|n| <= 31, i.e. |theta| < 190: the host checks the
+// largest |theta| of the sweep), plus 0x100 in the next lane if the link needs the slow path: its angle is within 1e-5
+// of the cut, or an end point is exactly zero (t is NaN, which fails the <=).  rint by the magic-number addition
+// (exact for |t| < 2^22, ties to even like rintf): the low mantissa byte of t + 1.5 * 2^23 + 32 IS (n + 32) & 0xff, so
+// no float <-> int conversion (XU pipe) is needed.
 __device__ inline unsigned link_lane(float alpha_a, float alpha_b, float theta)
 {
-    const float t = ((alpha_b - alpha_a) - theta) * INV_2PI;          // NaN if an end point is exactly zero
-    const float nf = rintf(t);
-    const unsigned near = fabsf(t - nf) > NEAR_T ? 1u : 0u;           // NaN compares false
-    const unsigned deg = t != t ? 4u : 0u;
-    const int n = __float2int_rn(t);                                  // NaN -> 0
-    return ((unsigned)(n + (int)BIAS) & 0x3fu) | ((near | deg) << 8);
-}
-
-// link angle of the printed formula, for the slow path only
-__device__ inline float chi_slow(float alpha_a, float alpha_b, float theta)
-{
+    constexpr float MAGIC = 12582912.f + 32.f;
     const float t = ((alpha_b - alpha_a) - theta) * INV_2PI;
-    const float r = (t - rintf(t)) * 6.2831853071795865f;
-    return r != r ? 0.f : r;                                          // atan2(0, 0) = 0 (reading R-15)
+    const float tm = t + MAGIC;
+    const float d = t - (tm - MAGIC);
+    return (__float_as_uint(tm) & 0xffu) + (fabsf(d) <= NEAR_T ? 0u : 256u);
 }
 
-struct Acc {
-    double g[6];          // sum g^2, rho^2, div^2 per sector
-    double d[11];         // sum L, kin L, grad L, kin V, grad V, V, kin, grad, elec, mag, pot
-    double gmax[2];
-    unsigned wsum;        // sum |W| of this item, lanes p (bits 0..15) and q (16..31)
-    int sumw[2], nnear[2], ncell[3], maxw;
-    float maxth;
-};
-
+#ifndef FUSED_CTAS
+#define FUSED_CTAS 3
+#endif
 template <bool EXPORT>
-__global__ void __launch_bounds__(NTHREADS, 2)
+__global__ void __launch_bounds__(NTHREADS, FUSED_CTAS)
 diag_fused_kernel(const float *__restrict__ posp, const float *__restrict__ momp, size_t V, int N, FusedCoef k, int zchunk,
                   int band, uint8_t *__restrict__ cells, uint8_t *__restrict__ codes, double *__restrict__ partials,
                   const __grid_constant__ DiagMaps maps)
@@ -108,28 +94,23 @@ diag_fused_kernel(const float *__restrict__ posp, const float *__restrict__ momp
     float *alpha = reinterpret_cast<float *>(smem + OFF_ALPHA);
     uint2 *XY = reinterpret_cast<uint2 *>(smem + OFF_XY);
     unsigned *ZW = reinterpret_cast<unsigned *>(smem + OFF_Z);
+    double *red = reinterpret_cast<double *>(smem + OFF_RED);
     const size_t NN = (size_t)N * N;
-    const int tid = threadIdx.x, tx = tid & (TX - 1), ty = tid / TX, warp = tid >> 5;
+    const int tid = threadIdx.x, tx = tid & (TX - 1), ty = tid / TX, warp = tid >> 5, lane = tid & 31;
     const char *pos = reinterpret_cast<const char *>(posp);
     const unsigned long long pol_stream = policy_evict_first(), pol_keep = policy_evict_last();
     const int ntx = (N + TX - 1) / TX, nty = (N + TY - 1) / TY, nzc = (N + zchunk - 1) / zchunk;
     const int items = ntx * nty * nzc;
+    const float4 *gMA = reinterpret_cast<const float4 *>(momp);
+    const float2 *gMC = reinterpret_cast<const float2 *>(momp + 8 * V);
 
     if (tid == 0) {
 #pragma unroll
-        for (int b = 0; b < NSLOT + NMSLOT; b++) mbar_init(bars + 8 * b, 1);
+        for (int b = 0; b < NSLOT + 2; b++) mbar_init(bars + 8 * b, 1);
         mbar_fence_init();
     }
+    for (int i = tid; i < FUSED_NRES * (NTHREADS / 32); i += NTHREADS) red[i] = 0.0;
     __syncthreads();
-
-    Acc acc;
-#pragma unroll
-    for (int i = 0; i < 6; i++) acc.g[i] = 0.0;
-#pragma unroll
-    for (int i = 0; i < 11; i++) acc.d[i] = 0.0;
-    acc.gmax[0] = acc.gmax[1] = 0.0;
-    acc.sumw[0] = acc.sumw[1] = acc.nnear[0] = acc.nnear[1] = acc.ncell[0] = acc.ncell[1] = acc.ncell[2] = acc.maxw = 0;
-    acc.maxth = 0.f;
     unsigned gpos = 0, gmom = 0;          // planes staged by TMA so far (ring slot and mbarrier phase bookkeeping)
 
     for (int item = blockIdx.x; item < items; item += gridDim.x) {
@@ -140,113 +121,150 @@ diag_fused_kernel(const float *__restrict__ posp, const float *__restrict__ momp
         const int wx = min(TX, N - x0), wy = min(TY, N - y0), nz = min(zchunk, N - z0);
         const bool active = tx < wx && ty < wy;
         const bool tma = !(k.flags & 2) && tile_is_interior(x0, y0, N);
-        acc.wsum = 0;
 
-        // ---- staging: relative position plane j = 0 .. nz, momentum plane m = 0 .. nz-1 ----
+        // this item's partial sums in fp32 (at most zchunk terms each), folded into the per-warp fp64 accumulators at its end
+        float gf[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f}, df[11] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+        float gmax[2] = {0.f, 0.f}, maxth = 0.f;
+        unsigned wsum = 0, csum = 0;          // sum |W| (lanes p: bits 0..15, q: 16..31); pierced cells p, q (same lanes)
+        int npq = 0, nnear = 0, maxw = 0;     // cells pierced by both; near-cut plaquettes (p: bits 0..15, q: 16..31)
+
+        // ---- staging: relative position plane j = 0 .. nz (slot = running plane count mod 3), momentum pack B (with
+        // halo) of plane m = 0 .. nz-1 (slot = running count mod 2).  TMA tiles: one thread issues box loads that
+        // complete on mbarriers; boundary tiles: every thread issues its cp.async copies.
         CpPlan plan;
         if (!tma) make_cp_plan(plan, tid, x0, y0, wx, wy, N);
-        auto pslot = [&](int j) { return tma ? (gpos + (unsigned)j) & 3u : (unsigned)j & 3u; };
-        auto stage_pos = [&](int j) {         // TMA: one thread; cp.async: every thread (caller commits)
+        const unsigned pb = tma ? gpos : 0u, mb = tma ? gmom : 0u;
+        auto stage_pos = [&](int j, unsigned slot) {
             const int z = wrapi(z0 + j, N);
-            if (tma) stage_plane_tma(maps.pos, x0, y0, z, sbase + pslot(j) * SLOT_BYTES, bars + 8 * pslot(j), pol_keep);
-            else stage_plane_cp(plan, tid, pos, V, (size_t)z * NN, sbase + pslot(j) * SLOT_BYTES);
+            if (tma) stage_plane_tma(maps.pos, x0, y0, z, sbase + slot * SLOT_BYTES, bars + 8 * slot, pol_keep);
+            else stage_plane_cp(plan, tid, pos, V, (size_t)z * NN, sbase + slot * SLOT_BYTES);
         };
-        auto mslot = [&](int m) { return (gmom + (unsigned)m) & 1u; };
-        auto stage_mom = [&](int m) {         // TMA tiles only, one thread
-            stage_plane_tma(maps.mom, x0, y0, z0 + m, sbase + OFF_MRING + mslot(m) * SLOT_BYTES, bars + 8 * (NSLOT + mslot(m)),
-                            pol_stream);
-        };
-        auto wait_pos = [&](int j) {          // TMA only
-            const unsigned g = gpos + (unsigned)j;
-            mbar_wait(bars + 8 * (g & 3u), (g >> 2) & 1u);
-        };
-        auto wait_mom = [&](int m) {
-            const unsigned g = gmom + (unsigned)m;
-            mbar_wait(bars + 8 * (NSLOT + (g & 1u)), (g >> 1) & 1u);
+        auto stage_mom = [&](int m) {
+            const unsigned sl = (mb + (unsigned)m) & 1u;
+            if (tma) {
+                const unsigned bar = bars + 8 * (NSLOT + sl);
+                mbar_expect_tx(bar, NELEM * 16);
+                tma_load_3d_hint(sbase + OFF_MRING + sl * MSLOT_BYTES, &maps.mom.B, 4 * (x0 - 1), y0 - 1, z0 + m, bar, pol_stream);
+            } else {
+                stage_packB_cp(plan, tid, reinterpret_cast<const char *>(momp), V, (size_t)(z0 + m) * NN, sbase + OFF_MRING + sl * MSLOT_BYTES);
+            }
         };
 
         __syncthreads();                      // the previous item's readers are done with every buffer
-        if (tma) {                            // planes 0, 1 now; plane iz+3 during iteration iz = -1, 0, ...
-            if (tid == 0) {
-                stage_pos(0);
-                stage_pos(1);
+        unsigned s_n = pb % 3u, par_n = (pb / 3u) & 1u;       // ring slot and mbarrier parity of plane iz+1 (here: plane 0)
+        {
+            unsigned sl = s_n;
+            if (!tma || tid == 0) {
+                for (int j = 0; j <= 2; j++) {
+                    if (j <= nz) stage_pos(j, sl);
+                    sl = sl == 2u ? 0u : sl + 1u;
+                }
                 stage_mom(0);
                 if (nz > 1) stage_mom(1);
             }
-        } else {
-            for (int j = 0; j <= 1; j++) {
-                stage_pos(j);
-                cp_async_commit();
-            }
+            if (!tma) cp_async_commit();
         }
 
         // element indices of this thread's own site inside a staged plane
         const int e_own = (ty + 1) * COLS + tx + 1, e_ownC = (ty + 1) * CCOLS + tx + 2;
         const size_t gsite = (size_t)(y0 + ty) * N + (size_t)(x0 + tx);
+        size_t lin = (size_t)z0 * NN + gsite;
         // E_z, H_z of plane z0 - 1 (for div E of the first plane)
         float2 ez_prev = make_float2(0.f, 0.f);
-        if (active) ez_prev = __ldg(reinterpret_cast<const float2 *>(momp + 8 * V) + (size_t)wrapi(z0 - 1, N) * NN + gsite);
-        unsigned Pxy = 0, Qxy = 0, Fxy = 0;   // W_xy of the current plane (and its links' flags), carried from the previous iteration
+        if (active) ez_prev = __ldg(gMC + (size_t)wrapi(z0 - 1, N) * NN + gsite);
 
-        // extended sites: the tile plus its +x column and +y row (needed by the cells of the last column / row).
-        // Pass 1 = own element of every thread; pass 2 = the extra row (one warp) and the extra column (9 lanes of the
-        // next warp), rotated over the warps from plane to plane to spread the load.
-        auto extra_elem = [&](int iz, int &c, int &r) -> bool {
-            const int w0 = (iz + 1) & 7, lane = tid & 31;
-            if (warp == w0 && wy == TY) { c = lane; r = TY; return c <= wx && (c < TX); }
-            if (warp == ((w0 + 1) & 7) && wx == TX) { c = TX; r = lane; return r <= wy && (r <= TY); }
-            return false;
+        // extended sites: the tile plus its +x column and +y row (the cells of the last column / row need their
+        // plaquettes).  Pass 1 = own element of every thread; pass 2 = the extra row (32 lanes of one warp) and the
+        // extra column (9 lanes of the next warp), rotated over the warps from plane to plane to spread the load.
+        const bool own_ext = tx <= wx && ty <= wy;
+        const int e_row = (TY + 1) * COLS + lane + 1, e_col = (lane + 1) * COLS + TX + 1;
+        auto do_alpha = [&](int e, const char *sn, int nxt) {          // phases of one site of plane `sn` into alpha[nxt]
+            const float4 a = *reinterpret_cast<const float4 *>(sn + e * 16);
+            alpha[(nxt * 2 + 0) * NELEM + e] = site_phase(a.x, a.y);
+            alpha[(nxt * 2 + 1) * NELEM + e] = site_phase(a.z, a.w);
+        };
+        // wrap counts of the x and y links of one site of plane `sn` (links that leave the extended tile -- x links of
+        // the extra column, y links of the extra row -- are evaluated on whatever the neighbouring shared-memory words
+        // hold and never read), returns the site's two phases for the z links
+        auto do_links_xy = [&](int e, const char *sn, int nxt, float &a0p, float &a0q) {
+            const float4 Bn = *reinterpret_cast<const float4 *>(sn + OFF_B + e * 16);
+            const float *ap = alpha + (nxt * 2 + 0) * NELEM + e, *aq = alpha + (nxt * 2 + 1) * NELEM + e;
+            a0p = ap[0];
+            a0q = aq[0];
+            const unsigned X = __byte_perm(link_lane(a0p, ap[1], Bn.x), link_lane(a0q, aq[1], Bn.z), 0x5410);
+            const unsigned Y = __byte_perm(link_lane(a0p, ap[COLS], Bn.y), link_lane(a0q, aq[COLS], Bn.w), 0x5410);
+            XY[nxt * NELEM + e] = make_uint2(X, Y);
+        };
+        auto do_links = [&](int e, const char *sc, const char *sn, int cur) {      // + the z links of plane `sc`
+            float a0p, a0q;
+            do_links_xy(e, sn, cur ^ 1, a0p, a0q);
+            const int r = e / COLS;
+            const float2 Cz = *reinterpret_cast<const float2 *>(sc + OFF_C + (e + 2 * r + 1) * 8);
+            ZW[e] = __byte_perm(link_lane(alpha[(cur * 2 + 0) * NELEM + e], a0p, Cz.x), link_lane(alpha[(cur * 2 + 1) * NELEM + e], a0q, Cz.y), 0x5410);
+        };
+        auto wait_plane = [&]() {             // plane iz+1 (slot s_n) has landed
+            if (tma) mbar_wait(bars + 8 * s_n, par_n);
+            else {
+                cp_async_wait<0>();
+                __syncthreads();
+            }
         };
 
-        for (int iz = -1; iz < nz; iz++) {
-            // ---- plane iz+1 must have landed (and the momenta of plane iz) ----
+        // ---- prologue: phases and in-plane links of plane 0, W_xy of plane 0 ----
+        unsigned Pxy = 0, Qxy = 0;            // W_xy of the current plane, carried from one iteration to the next
+        {
+            wait_plane();
+            const char *sn = smem + s_n * SLOT_BYTES;
+            const bool xrow = warp == 0 && wy == TY, xcol = warp == 1 && wx == TX && lane <= TY;
+            if (own_ext) do_alpha(e_own, sn, 0);
+            if (xrow || xcol) do_alpha(xrow ? e_row : e_col, sn, 0);
+            __syncthreads();
+            float u, v;
+            if (own_ext) do_links_xy(e_own, sn, 0, u, v);
+            if (xrow || xcol) do_links_xy(xrow ? e_row : e_col, sn, 0, u, v);
+            __syncthreads();
+            if (active) {
+                const uint2 Ln = XY[e_own], Lnx = XY[e_own + 1], Lny = XY[e_own + COLS];
+                Pxy = Ln.x + Lnx.y;
+                Qxy = Lny.x + Ln.y;
+            }
+        }
+
+        unsigned s_c = s_n;                   // slot of plane iz
+        for (int iz = 0; iz < nz; iz++) {
+            // momenta of this thread's site: the own-site packs straight from global memory (pack B, whose -x / -y
+            // neighbours div E needs, comes through the shared-memory ring)
+            float4 MA = make_float4(0.f, 0.f, 0.f, 0.f);
+            float2 MC = make_float2(0.f, 0.f);
+            if (active) {
+                MA = __ldcs(gMA + lin);
+                MC = __ldcs(gMC + lin);
+            }
+            s_n = s_c == 2u ? 0u : s_c + 1u;
+            par_n ^= s_n == 0u ? 1u : 0u;
+            wait_plane();                     // plane iz+1; on boundary tiles also the momenta of plane iz
             if (tma) {
-                wait_pos(iz + 1);
-                if (iz >= 0) wait_mom(iz);
-            } else {
-                cp_async_wait<1>();
-                __syncthreads();
-                if (iz + 3 <= nz) stage_pos(iz + 3);      // slot of plane iz-1: every thread is past its last read
-                cp_async_commit();
+                const unsigned h = mb + (unsigned)iz;
+                mbar_wait(bars + 8 * (NSLOT + (h & 1u)), (h >> 1) & 1u);
             }
             const int cur = iz & 1, nxt = cur ^ 1;
-            const char *sc = smem + pslot(iz < 0 ? 0 : iz) * SLOT_BYTES;      // plane iz (unused for iz = -1)
-            const char *sn = smem + pslot(iz + 1) * SLOT_BYTES;               // plane iz+1
+            const char *sc = smem + s_c * SLOT_BYTES, *sn = smem + s_n * SLOT_BYTES;
+            const int rot = (warp - iz - 1) & 7;
+            const bool xrow = rot == 0 && wy == TY, xcol = rot == 1 && wx == TX && lane <= TY;
+            const bool has_extra = xrow || xcol;
+            const int e_ext = xrow ? e_row : e_col;
 
             // ---- phase A: phases alpha of plane iz+1 on the extended tile ----
-            auto do_alpha = [&](int c, int r) {
-                const int e = (r + 1) * COLS + c + 1;
-                const float4 a = *reinterpret_cast<const float4 *>(sn + e * 16);
-                alpha[(nxt * 2 + 0) * NELEM + e] = site_phase(a.x, a.y);
-                alpha[(nxt * 2 + 1) * NELEM + e] = site_phase(a.z, a.w);
-            };
-            if (tx <= wx && ty <= wy) do_alpha(tx, ty);
-            {
-                int c, r;
-                if (extra_elem(iz, c, r)) do_alpha(c, r);
-            }
+            if (own_ext) do_alpha(e_own, sn, nxt);
+            if (has_extra) do_alpha(e_ext, sn, nxt);
 
             // ---- Gauss residual and densities of this thread's site in plane iz (independent of the windings) ----
-            if (iz >= 0 && active) {
-                const size_t lin = (size_t)(z0 + iz) * NN + gsite;
+            if (active) {
                 auto A = [&](const char *s, int d) { return *reinterpret_cast<const float4 *>(s + (e_own + d) * 16); };
                 auto B = [&](const char *s, int d) { return *reinterpret_cast<const float4 *>(s + OFF_B + (e_own + d) * 16); };
                 auto C = [&](const char *s, int d) { return *reinterpret_cast<const float2 *>(s + OFF_C + (e_ownC + d) * 8); };
-                float4 MA, MB, MBxm, MBym;
-                float2 MC;
-                if (tma) {
-                    const char *ms = smem + OFF_MRING + mslot(iz) * SLOT_BYTES;
-                    MA = A(ms, 0); MB = B(ms, 0); MBxm = B(ms, -1); MBym = B(ms, -COLS); MC = C(ms, 0);
-                } else {
-                    const float4 *gA = reinterpret_cast<const float4 *>(momp), *gB = reinterpret_cast<const float4 *>(momp + 4 * V);
-                    const size_t zp = (size_t)(z0 + iz) * NN;
-                    const int x = x0 + tx, y = y0 + ty;
-                    MA = __ldcs(gA + lin);
-                    MB = __ldcs(gB + lin);
-                    MBxm = __ldg(gB + zp + (size_t)y * N + wrapi(x - 1, N));
-                    MBym = __ldg(gB + zp + (size_t)wrapi(y - 1, N) * N + x);
-                    MC = __ldcs(reinterpret_cast<const float2 *>(momp + 8 * V) + lin);
-                }
+                const float4 *ms = reinterpret_cast<const float4 *>(smem + OFF_MRING + ((mb + (unsigned)iz) & 1u) * MSLOT_BYTES);
+                const float4 MB = ms[e_own], MBxm = ms[e_own - 1], MBym = ms[e_own - COLS];
                 const float4 Ac = A(sc, 0), Axp = A(sc, 1), Ayp = A(sc, COLS), Azp = A(sn, 0);
                 const float4 Bc = B(sc, 0), Bxp = B(sc, 1), Byp = B(sc, COLS), Bzp = B(sn, 0);
                 const float2 Cc = C(sc, 0), Cxp = C(sc, 1), Cyp = C(sc, CCOLS);
@@ -258,18 +276,16 @@ diag_fused_kernel(const float *__restrict__ posp, const float *__restrict__ momp
                     // Gauss (Eq. 9-10): differences and the charge density in fp64 (g is a 1e-6 cancellation)
                     const float E[3] = {s ? MB.z : MB.x, s ? MB.w : MB.y, s ? MC.y : MC.x};
                     const float Em[3] = {s ? MBxm.z : MBxm.x, s ? MBym.w : MBym.y, s ? ez_prev.y : ez_prev.x};
-                    double div = 0.0;
-#pragma unroll
-                    for (int i = 0; i < 3; i++) div += ((double)E[i] - (double)Em[i]) * k.inv_dx;
+                    const double div = (((double)E[0] - (double)Em[0]) + ((double)E[1] - (double)Em[1]) + ((double)E[2] - (double)Em[2])) * k.inv_dx;
                     const double rho = (s ? k.rho2 : k.rho1) * ((double)fr * (double)pi - (double)fi * (double)pr);
-                    const double g = div - rho;
-                    acc.g[3 * s + 0] += g * g;
-                    acc.g[3 * s + 1] += rho * rho;
-                    acc.g[3 * s + 2] += div * div;
-                    acc.gmax[s] = fmax(acc.gmax[s], fabs(g));
+                    const float gl = (float)(div - rho), rl = (float)rho, dl = (float)div;
+                    gf[3 * s + 0] = fmaf(gl, gl, gf[3 * s + 0]);
+                    gf[3 * s + 1] = fmaf(rl, rl, gf[3 * s + 1]);
+                    gf[3 * s + 2] = fmaf(dl, dl, gf[3 * s + 2]);
+                    gmax[s] = fmaxf(gmax[s], fabsf(gl));
                     // densities (fp32 per-site terms)
-                    kin += pr * pr + pi * pi;
-                    m2[s] = fr * fr + fi * fi;
+                    kin = fmaf(pr, pr, fmaf(pi, pi, kin));
+                    m2[s] = fmaf(fr, fr, fi * fi);
                     const float th[3] = {s ? Bc.z : Bc.x, s ? Bc.w : Bc.y, s ? Cc.y : Cc.x};
                     const float nr[3] = {s ? Axp.z : Axp.x, s ? Ayp.z : Ayp.x, s ? Azp.z : Azp.x};
                     const float ni[3] = {s ? Axp.w : Axp.y, s ? Ayp.w : Ayp.y, s ? Azp.w : Azp.y};
@@ -278,224 +294,203 @@ diag_fused_kernel(const float *__restrict__ posp, const float *__restrict__ momp
                     for (int i = 0; i < 3; i++) {
                         float sn_, cs_;
                         __sincosf(th[i], &sn_, &cs_);               // U = exp(-i theta): SFU phasor (abs. error ~5e-7)
-                        const float dr = (cs_ * nr[i] + sn_ * ni[i]) - fr, di = (cs_ * ni[i] - sn_ * nr[i]) - fi;
-                        g2 += dr * dr + di * di;
-                        e2 += E[i] * E[i];
-                        acc.maxth = fmaxf(acc.maxth, fabsf(th[i]));
+                        const float dr = fmaf(cs_, nr[i], fmaf(sn_, ni[i], -fr)), di = fmaf(cs_, ni[i], fmaf(-sn_, nr[i], -fi));
+                        g2 = fmaf(dr, dr, fmaf(di, di, g2));
+                        e2 = fmaf(E[i], E[i], e2);
+                        maxth = fmaxf(maxth, fabsf(th[i]));
                     }
                     // plaquettes (i, j) = (x,y), (x,z), (y,z)
                     const float ty_x = s ? Bxp.w : Bxp.y, tx_y = s ? Byp.z : Byp.x;
                     const float tz_x = s ? Cxp.y : Cxp.x, tx_z = s ? Bzp.z : Bzp.x;
                     const float tz_y = s ? Cyp.y : Cyp.x, ty_z = s ? Bzp.w : Bzp.y;
                     const float P0 = th[0] + ty_x - tx_y - th[1], P1 = th[0] + tz_x - tx_z - th[2], P2 = th[1] + tz_y - ty_z - th[2];
-                    grad += g2 * k.inv_dx2;
-                    elec += e2 * (s ? k.el2 : k.el1);
-                    mag += (P0 * P0 + P1 * P1 + P2 * P2) * (s ? k.mg2 : k.mg1);
+                    grad = fmaf(g2, k.inv_dx2, grad);
+                    elec = fmaf(e2, s ? k.el2 : k.el1, elec);
+                    mag = fmaf(fmaf(P0, P0, fmaf(P1, P1, P2 * P2)), s ? k.mg2 : k.mg1, mag);
                 }
                 ez_prev = MC;
                 const float a2 = m2[0] - k.sig1sq, b2 = m2[1] - k.sig2sq;
                 const float vint = k.kappa * a2 * b2;
                 const float pot = k.lam1q * a2 * a2 + k.lam2q * b2 * b2 - vint;
                 const float lag = kin - grad + (elec - mag) * k.inv_c - k.c * pot;
-                acc.d[0] += (double)lag;
-                acc.d[1] += (double)(kin * lag);
-                acc.d[2] += (double)(grad * lag);
-                acc.d[3] += (double)(kin * vint);
-                acc.d[4] += (double)(grad * vint);
-                acc.d[5] += (double)vint;
-                acc.d[6] += (double)kin;
-                acc.d[7] += (double)grad;
-                acc.d[8] += (double)elec;
-                acc.d[9] += (double)mag;
-                acc.d[10] += (double)pot;
+                df[0] += lag;
+                df[1] = fmaf(kin, lag, df[1]);
+                df[2] = fmaf(grad, lag, df[2]);
+                df[3] = fmaf(kin, vint, df[3]);
+                df[4] = fmaf(grad, vint, df[4]);
+                df[5] += vint;
+                df[6] += kin;
+                df[7] += grad;
+                df[8] += elec;
+                df[9] += mag;
+                df[10] += pot;
             }
-            __syncthreads();                  // alpha of plane iz+1 complete; momenta of plane iz consumed
-            if (tma && tid == 0) {
-                if (iz + 3 <= nz) stage_pos(iz + 3);          // slot of plane iz-1: every thread is past iteration iz-1
-                if (iz >= 0 && iz + 2 < nz) stage_mom(iz + 2);        // slot of plane iz, consumed in phase A
+            __syncthreads();                  // alpha of plane iz+1 complete; everybody is past iteration iz-1
+            if (!tma || tid == 0) {
+                if (iz >= 1 && iz + 2 <= nz) stage_pos(iz + 2, s_n == 2u ? 0u : s_n + 1u);      // the slot of plane iz-1
+                if (iz + 2 < nz) stage_mom(iz + 2);                                             // the slot of plane iz, consumed in phase A
             }
+            if (!tma) cp_async_commit();
 
             // ---- phase B: wrap counts of the x, y links of plane iz+1 and of the z links of plane iz ----
-            auto do_links = [&](int c, int r) {
-                const int e = (r + 1) * COLS + c + 1;
-                const float4 Bn = *reinterpret_cast<const float4 *>(sn + OFF_B + e * 16);
-                unsigned X = 0, Y = 0, Z = 0;
-#pragma unroll
-                for (int s = 0; s < 2; s++) {
-                    const float *an = alpha + (nxt * 2 + s) * NELEM;
-                    const float a0 = an[e];
-                    X |= (c < wx ? link_lane(a0, an[e + 1], s ? Bn.z : Bn.x) : BIAS) << (16 * s);
-                    Y |= (r < wy ? link_lane(a0, an[e + COLS], s ? Bn.w : Bn.y) : BIAS) << (16 * s);
-                    if (iz >= 0) {
-                        const float2 Cz = *reinterpret_cast<const float2 *>(sc + OFF_C + ((r + 1) * CCOLS + c + 2) * 8);
-                        Z |= link_lane(alpha[(cur * 2 + s) * NELEM + e], a0, s ? Cz.y : Cz.x) << (16 * s);
-                    }
-                }
-                XY[nxt * NELEM + e] = make_uint2(X, Y);
-                if (iz >= 0) ZW[e] = Z;
-            };
-            if (tx <= wx && ty <= wy) do_links(tx, ty);
-            {
-                int c, r;
-                if (extra_elem(iz, c, r)) do_links(c, r);
-            }
+            if (own_ext) do_links(e_own, sc, sn, cur);
+            if (has_extra) do_links(e_ext, sc, sn, cur);
             __syncthreads();
 
             // ---- phase C: windings, cells, counters of this thread's site ----
             if (active) {
                 const uint2 Ln = XY[nxt * NELEM + e_own], Lnx = XY[nxt * NELEM + e_own + 1], Lny = XY[nxt * NELEM + e_own + COLS];
                 // W_xy of plane iz+1: S = n_x(x) + n_y(x+x) - n_x(x+y) - n_y(x);  W = -S
-                const unsigned Pn = Ln.x + Lnx.y, Qn = Lny.x + Ln.y, Fn = (Ln.x | Lnx.y | Lny.x | Ln.y) & FLAG_LANES;
-                if (iz >= 0) {
-                    const size_t lin = (size_t)(z0 + iz) * NN + gsite;
-                    const uint2 Lc = XY[cur * NELEM + e_own], Lcx = XY[cur * NELEM + e_own + 1], Lcy = XY[cur * NELEM + e_own + COLS];
-                    const unsigned Z0 = ZW[e_own], Zx = ZW[e_own + 1], Zy = ZW[e_own + COLS], Zxy = ZW[e_own + COLS + 1];
-                    // W_yz(x): n_y(x) + n_z(x+y) - n_y(x+z) - n_z(x);   W_zx(x): n_z(x) + n_x(x+z) - n_z(x+x) - n_x(x)
-                    unsigned P[5], Q[5];
-                    P[0] = Pxy;            Q[0] = Qxy;                 // xy, plane iz (own)
-                    P[1] = Lc.y + Zy;      Q[1] = Ln.y + Z0;           // yz (own)
-                    P[2] = Z0 + Ln.x;      Q[2] = Zx + Lc.x;           // zx (own)
-                    P[3] = Lcx.y + Zxy;    Q[3] = Lnx.y + Zx;          // yz at x + x
-                    P[4] = Zy + Lny.x;     Q[4] = Zxy + Lcy.x;         // zx at x + y
-                    unsigned Eabs[6], flagged = (Pn | Qn) & FLAG_LANES;
+                const unsigned Pn = Ln.x + Lnx.y, Qn = Lny.x + Ln.y;
+                const uint2 Lc = XY[cur * NELEM + e_own], Lcx = XY[cur * NELEM + e_own + 1], Lcy = XY[cur * NELEM + e_own + COLS];
+                const unsigned Z0 = ZW[e_own], Zx = ZW[e_own + 1], Zy = ZW[e_own + COLS], Zxy = ZW[e_own + COLS + 1];
+                // W_yz(x): n_y(x) + n_z(x+y) - n_y(x+z) - n_z(x);   W_zx(x): n_z(x) + n_x(x+z) - n_z(x+x) - n_x(x)
+                unsigned P[6], Q[6];
+                P[0] = Pxy;            Q[0] = Qxy;                 // xy, plane iz (own)
+                P[1] = Lc.y + Zy;      Q[1] = Ln.y + Z0;           // yz (own)
+                P[2] = Z0 + Ln.x;      Q[2] = Zx + Lc.x;           // zx (own)
+                P[3] = Lcx.y + Zxy;    Q[3] = Lnx.y + Zx;          // yz at x + x
+                P[4] = Zy + Lny.x;     Q[4] = Zxy + Lcy.x;         // zx at x + y
+                P[5] = Pn;             Q[5] = Qn;                  // xy, plane iz+1
+                unsigned Eabs[6], flagged = 0;
 #pragma unroll
-                    for (int q = 0; q < 5; q++) {
-                        Eabs[q] = __vabsdiffu4(P[q], Q[q]) & VAL_LANES;
-                        flagged |= (P[q] | Q[q]) & FLAG_LANES;
-                    }
-                    Eabs[5] = __vabsdiffu4(Pn, Qn) & VAL_LANES;        // xy, plane iz+1
-                    int wsg[2][3];                                      // signed windings of the own plaquettes (EXPORT)
-                    unsigned nearbits = 0;                              // bit 3 s + o
-                    if (EXPORT) {
+                for (int q = 0; q < 6; q++) {
+                    Eabs[q] = __vabsdiffu4(P[q], Q[q]) & VAL_LANES;
+                    flagged |= P[q] | Q[q];
+                }
+                int wsg[2][3];                                      // signed windings of the own plaquettes (EXPORT)
+                unsigned nearbits = 0;                              // bit 3 s + o
+                if (EXPORT) {
 #pragma unroll
-                        for (int o = 0; o < 3; o++) {
-                            wsg[0][o] = (int)(Q[o] & 0xffu) - (int)(P[o] & 0xffu);
-                            wsg[1][o] = (int)((Q[o] >> 16) & 0xffu) - (int)((P[o] >> 16) & 0xffu);
-                        }
+                    for (int o = 0; o < 3; o++) {
+                        wsg[0][o] = (int)(Q[o] & 0xffu) - (int)(P[o] & 0xffu);
+                        wsg[1][o] = (int)((Q[o] >> 16) & 0xffu) - (int)((P[o] >> 16) & 0xffu);
                     }
-                    if (flagged) {
-                        // slow path: near-cut flags of the own plaquettes; plaquettes with a degenerate link by the
-                        // printed formula with chi = 0 on those links
-                        auto Af = [&](const char *s, int e) { return *reinterpret_cast<const float4 *>(s + e * 16); };
-                        auto th_xy = [&](const char *s, int e, int sec, int dir) {
-                            const float4 b = *reinterpret_cast<const float4 *>(s + OFF_B + e * 16);
-                            return dir == 0 ? (sec ? b.z : b.x) : (sec ? b.w : b.y);
-                        };
-                        auto th_z = [&](const char *s, int e, int sec) {
-                            const int r = e / COLS, c = e - r * COLS;
-                            const float2 cz = *reinterpret_cast<const float2 *>(s + OFF_C + (r * CCOLS + c + 1) * 8);
-                            return sec ? cz.y : cz.x;
-                        };
-                        auto ph = [&](const char *s, int e, int sec) {
-                            const float4 a = Af(s, e);
-                            return sec ? site_phase(a.z, a.w) : site_phase(a.x, a.y);
-                        };
-                        // plaquette q (0 xy cur, 1 yz, 2 zx, 3 yz at x+x, 4 zx at x+y, 5 xy nxt) of sector sec by the formula
-                        auto formula = [&](int q, int sec) {
+                }
+                if (flagged & FLAG_LANES) {
+                    // slow path: a plaquette with a flagged link is re-evaluated link by link from the staged fields
+                    // (same arithmetic as phases A and B, so the classification is consistent): near-cut flag of the
+                    // own plaquettes; with a degenerate link (chi = 0 there, reading R-15) the printed formula
+                    auto ph = [&](const char *s, int e, int sec) {
+                        const float4 a = *reinterpret_cast<const float4 *>(s + e * 16);
+                        return sec ? site_phase(a.z, a.w) : site_phase(a.x, a.y);
+                    };
+                    auto th_xy = [&](const char *s, int e, int sec, int dir) {
+                        const float4 b = *reinterpret_cast<const float4 *>(s + OFF_B + e * 16);
+                        return dir == 0 ? (sec ? b.z : b.x) : (sec ? b.w : b.y);
+                    };
+                    auto th_z = [&](const char *s, int e, int sec) {
+                        const int r = e / COLS;
+                        const float2 cz = *reinterpret_cast<const float2 *>(s + OFF_C + (e + 2 * r + 1) * 8);
+                        return sec ? cz.y : cz.x;
+                    };
+                    for (int q = 0; q < 6; q++) {
+                        for (int sec = 0; sec < 2; sec++) {
+                            unsigned fl = 0;                    // (registers only: no dynamic indexing of P, Q)
+#pragma unroll
+                            for (int qq = 0; qq < 6; qq++)
+                                if (qq == q) fl = P[qq] | Q[qq];
+                            if (!((fl >> (8 + 16 * sec)) & 0xffu)) continue;
                             const int eb = e_own + (q == 3 ? 1 : q == 4 ? COLS : 0);
                             const char *s0 = q == 5 ? sn : sc;
-                            float a00, a10, a01, a11, t1, t2, t3, t4;    // corners x, x+i, x+j, x+i+j; links i(x), j(x+i), i(x+j), j(x)
-                            if (q == 0 || q == 5) {                       // (i, j) = (x, y)
+                            float a00, a10, a01, a11, t[4];    // corners x, x+i, x+j, x+i+j; links i(x), j(x+i), i(x+j), j(x)
+                            if (q == 0 || q == 5) {             // (i, j) = (x, y)
                                 a00 = ph(s0, eb, sec); a10 = ph(s0, eb + 1, sec); a01 = ph(s0, eb + COLS, sec); a11 = ph(s0, eb + COLS + 1, sec);
-                                t1 = th_xy(s0, eb, sec, 0); t2 = th_xy(s0, eb + 1, sec, 1); t3 = th_xy(s0, eb + COLS, sec, 0); t4 = th_xy(s0, eb, sec, 1);
-                            } else if (q == 1 || q == 3) {                // (y, z)
+                                t[0] = th_xy(s0, eb, sec, 0); t[1] = th_xy(s0, eb + 1, sec, 1); t[2] = th_xy(s0, eb + COLS, sec, 0); t[3] = th_xy(s0, eb, sec, 1);
+                            } else if (q == 1 || q == 3) {      // (y, z)
                                 a00 = ph(sc, eb, sec); a10 = ph(sc, eb + COLS, sec); a01 = ph(sn, eb, sec); a11 = ph(sn, eb + COLS, sec);
-                                t1 = th_xy(sc, eb, sec, 1); t2 = th_z(sc, eb + COLS, sec); t3 = th_xy(sn, eb, sec, 1); t4 = th_z(sc, eb, sec);
-                            } else {                                      // (z, x)
+                                t[0] = th_xy(sc, eb, sec, 1); t[1] = th_z(sc, eb + COLS, sec); t[2] = th_xy(sn, eb, sec, 1); t[3] = th_z(sc, eb, sec);
+                            } else {                            // (z, x)
                                 a00 = ph(sc, eb, sec); a10 = ph(sn, eb, sec); a01 = ph(sc, eb + 1, sec); a11 = ph(sn, eb + 1, sec);
-                                t1 = th_z(sc, eb, sec); t2 = th_xy(sn, eb, sec, 0); t3 = th_z(sc, eb + 1, sec); t4 = th_xy(sc, eb, sec, 0);
+                                t[0] = th_z(sc, eb, sec); t[1] = th_xy(sn, eb, sec, 0); t[2] = th_z(sc, eb + 1, sec); t[3] = th_xy(sc, eb, sec, 0);
                             }
-                            const float sum = chi_slow(a00, a10, t1) + chi_slow(a10, a11, t2) - chi_slow(a01, a11, t3) - chi_slow(a00, a01, t4) +
-                                              (t1 + t2 - t3 - t4);
-                            return __float2int_rn(sum * INV_2PI);
-                        };
+                            const float da[4] = {a10 - a00, a11 - a10, a11 - a01, a01 - a00};
+                            float chi[4];
+                            bool near = false, deg = false;
 #pragma unroll
-                        for (int q = 0; q < 6; q++) {
-                            // OR of the flags of the plaquette's four links (lane 1: p, lane 3: q)
-                            unsigned orf;
-                            if (q == 0) orf = Fxy;
-                            else if (q == 1) orf = Lc.y | Zy | Ln.y | Z0;
-                            else if (q == 2) orf = Z0 | Ln.x | Zx | Lc.x;
-                            else if (q == 3) orf = Lcx.y | Zxy | Lnx.y | Zx;
-                            else if (q == 4) orf = Zy | Lny.x | Zxy | Lcy.x;
-                            else orf = Fn;
-                            orf &= FLAG_LANES;
-                            if (!orf) continue;
+                            for (int l = 0; l < 4; l++) {
+                                const float tl_ = (da[l] - t[l]) * INV_2PI, d = tl_ - rintf(tl_);
+                                deg |= d != d;
+                                near |= fabsf(d) > NEAR_T;
+                                chi[l] = d != d ? 0.f : d * 6.2831853071795865f;
+                            }
+                            if (deg) {
+                                const float sum = chi[0] + chi[1] - chi[2] - chi[3] + (t[0] + t[1] - t[2] - t[3]);
+                                const unsigned aW = (unsigned)abs(__float2int_rn(sum * INV_2PI));
+                                const int W = __float2int_rn(sum * INV_2PI);
 #pragma unroll
-                            for (int sec = 0; sec < 2; sec++) {
-                                const unsigned fs = (orf >> (8 + 16 * sec)) & 5u;     // bit 0 near, bit 2 degenerate
-                                if (fs & 4u) {
-                                    const int W = formula(q, sec);
-                                    Eabs[q] = (Eabs[q] & ~(0xffu << (16 * sec))) | ((unsigned)abs(W) << (16 * sec));
-                                    if (EXPORT && q < 3) wsg[sec][q] = W;
+                                for (int qq = 0; qq < 6; qq++)
+                                    if (qq == q) Eabs[qq] = (Eabs[qq] & ~(0xffu << (16 * sec))) | (aW << (16 * sec));
+                                if (EXPORT) {
+#pragma unroll
+                                    for (int o = 0; o < 3; o++)
+                                        if (o == q) { if (sec) wsg[1][o] = W; else wsg[0][o] = W; }
                                 }
-                                if ((fs & 1u) && q < 3) nearbits |= 1u << (3 * sec + q);
                             }
+                            if (near && q < 3) nearbits |= 1u << (3 * sec + q);
                         }
                     }
-                    // own plaquettes: length sums, near-cut counts, largest winding
-                    const unsigned own = Eabs[0] + Eabs[1] + Eabs[2];
-                    acc.wsum += own;
-                    acc.nnear[0] += __popc(nearbits & 7u);
-                    acc.nnear[1] += __popc(nearbits & 56u);
-                    if ((Eabs[0] | Eabs[1] | Eabs[2]) & 0x00fe00feu) {
+                }
+                // own plaquettes: length sums, near-cut counts, largest winding
+                const unsigned own = Eabs[0] + Eabs[1] + Eabs[2];
+                wsum += own;
+                nnear += __popc(nearbits & 7u) + (__popc(nearbits & 56u) << 16);
+                if ((Eabs[0] | Eabs[1] | Eabs[2]) & 0x00fe00feu) {
 #pragma unroll
-                        for (int q = 0; q < 3; q++) acc.maxw = max(acc.maxw, (int)max(Eabs[q] & 0xffu, Eabs[q] >> 16));
-                    } else if (own) {
-                        acc.maxw = max(acc.maxw, 1);
-                    }
-                    // pierced cells: the six faces of the cell at x
-                    const unsigned cell = own + Eabs[3] + Eabs[4] + Eabs[5];
-                    const unsigned cp = cell & 0xffu, cq = cell >> 16;
-                    cells[lin] = (uint8_t)cp;
-                    cells[V + lin] = (uint8_t)cq;
-                    acc.ncell[0] += cp > 0;
-                    acc.ncell[1] += cq > 0;
-                    acc.ncell[2] += (cp > 0) && (cq > 0);
-                    if (EXPORT) {
+                    for (int q = 0; q < 3; q++) maxw = max(maxw, (int)max(Eabs[q] & 0xffu, Eabs[q] >> 16));
+                } else if (own) {
+                    maxw = max(maxw, 1);
+                }
+                // pierced cells: the six faces of the cell at x
+                const unsigned cell = own + Eabs[3] + Eabs[4] + Eabs[5];
+                const unsigned cp = cell & 0xffu, cq = cell >> 16;
+                cells[lin] = (uint8_t)cp;
+                cells[V + lin] = (uint8_t)cq;
+                csum += (cp ? 1u : 0u) + (cq ? 0x10000u : 0u);
+                npq += (cp && cq) ? 1 : 0;
+                if (EXPORT) {
 #pragma unroll
-                        for (int sec = 0; sec < 2; sec++)
+                    for (int sec = 0; sec < 2; sec++)
 #pragma unroll
-                            for (int o = 0; o < 3; o++)
-                                codes[(size_t)(3 * sec + o) * V + lin] =
-                                    (uint8_t)(((wsg[sec][o] + 8) & 15) | (((nearbits >> (3 * sec + o)) & 1u) << 4));
-                    }
+                        for (int o = 0; o < 3; o++)
+                            codes[(size_t)(3 * sec + o) * V + lin] =
+                                (uint8_t)(((wsg[sec][o] + 8) & 15) | (((nearbits >> (3 * sec + o)) & 1u) << 4));
                 }
                 Pxy = Pn;
                 Qxy = Qn;
-                Fxy = Fn;
             }
+            s_c = s_n;
+            lin += NN;
         }
         if (!tma) cp_async_wait<0>();
         if (tma) { gpos += (unsigned)(nz + 1); gmom += (unsigned)nz; }
-        acc.sumw[0] += (int)(acc.wsum & 0xffffu);
-        acc.sumw[1] += (int)(acc.wsum >> 16);
+
+        // ---- fold this item's partials into the per-warp fp64 accumulators (fixed order: deterministic) ----
+        auto add = [&](int slot, double v) { if (lane == 0) red[slot * (NTHREADS / 32) + warp] += v; };
+        auto amax = [&](int slot, double v) { if (lane == 0) red[slot * (NTHREADS / 32) + warp] = fmax(red[slot * (NTHREADS / 32) + warp], v); };
+#pragma unroll
+        for (int i = 0; i < 6; i++) add(FR_GAUSS + i, warp_sum((double)gf[i]));
+#pragma unroll
+        for (int i = 0; i < 11; i++) add(FR_DENS + i, warp_sum((double)df[i]));
+        add(FR_SUMW, (double)__reduce_add_sync(0xffffffffu, wsum & 0xffffu));
+        add(FR_SUMW + 1, (double)__reduce_add_sync(0xffffffffu, wsum >> 16));
+        add(FR_NEAR, (double)__reduce_add_sync(0xffffffffu, (unsigned)nnear & 0xffffu));
+        add(FR_NEAR + 1, (double)__reduce_add_sync(0xffffffffu, (unsigned)nnear >> 16));
+        add(FR_CELLS, (double)__reduce_add_sync(0xffffffffu, csum & 0xffffu));
+        add(FR_CELLS + 1, (double)__reduce_add_sync(0xffffffffu, csum >> 16));
+        add(FR_CELLS + 2, (double)__reduce_add_sync(0xffffffffu, (unsigned)npq));
+        amax(FR_GMAX, (double)__uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(gmax[0]))));
+        amax(FR_GMAX + 1, (double)__uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(gmax[1]))));
+        amax(FR_MAXW, (double)__reduce_max_sync(0xffffffffu, (unsigned)maxw));
+        amax(FR_MAXTH, (double)__uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(maxth))));
     }
 
-    // ---- per-CTA partials (deterministic two-stage reduction, common.cuh) ----
-    double v[FUSED_NRES];
-#pragma unroll
-    for (int i = 0; i < 6; i++) v[FR_GAUSS + i] = acc.g[i];
-    v[FR_SUMW] = acc.sumw[0]; v[FR_SUMW + 1] = acc.sumw[1];
-    v[FR_NEAR] = acc.nnear[0]; v[FR_NEAR + 1] = acc.nnear[1];
-    v[FR_CELLS] = acc.ncell[0]; v[FR_CELLS + 1] = acc.ncell[1]; v[FR_CELLS + 2] = acc.ncell[2];
-#pragma unroll
-    for (int i = 0; i < 11; i++) v[FR_DENS + i] = acc.d[i];
-    v[FR_GMAX] = acc.gmax[0]; v[FR_GMAX + 1] = acc.gmax[1];
-    v[FR_MAXW] = acc.maxw;
-    v[FR_MAXTH] = acc.maxth;
-    double *red = reinterpret_cast<double *>(smem + OFF_RED);
-    const int lane = tid & 31;
-    __syncthreads();
-#pragma unroll
-    for (int i = 0; i < FUSED_NRES; i++) {
-        const double r = i < FUSED_NSUM ? warp_sum(v[i]) : warp_max(v[i]);
-        if (lane == 0) red[i * (NTHREADS / 32) + warp] = r;
-    }
+    // ---- per-CTA partials: the 8 warps' accumulators in fixed order ----
     __syncthreads();
     if (tid < FUSED_NRES) {
         double r = red[tid * (NTHREADS / 32)];
-        for (int w = 1; w < NTHREADS / 32; w++) r = tid < FUSED_NSUM ? r + red[tid * (NTHREADS / 32) + w] : fmax(r, red[tid * (NTHREADS / 32) + w]);
+        for (int w = 1; w < NTHREADS / 32; w++)
+            r = tid < FUSED_NSUM ? r + red[tid * (NTHREADS / 32) + w] : fmax(r, red[tid * (NTHREADS / 32) + w]);
         partials[(size_t)blockIdx.x * RED_SLOTS + tid] = r;
     }
 }
@@ -516,7 +511,7 @@ cudaError_t launch_diag_fused(const float *pos, const float *mom, size_t V, int 
     const int zc = fused_zchunk(N);
     const int ntx = (N + TX - 1) / TX, nty = (N + TY - 1) / TY, nzc = (N + zc - 1) / zc;
     const long items = (long)ntx * nty * nzc;
-    long grid = (long)sms * 2;
+    long grid = (long)sms * FUSED_CTAS;
     if (grid > RED_MAX_BLOCKS) grid = RED_MAX_BLOCKS;
     if (grid > items) grid = items;
     int band = (int)((grid + ntx - 1) / ntx);

@@ -140,6 +140,17 @@ __device__ inline void stage_plane_cp(const CpPlan &p, int tid, const char *buf,
     }
 }
 
+// every thread: pack B only (float4 per site with halo, laid out as float4[ROWS][COLS] at `slot`) of a 10 V-float buffer
+__device__ inline void stage_packB_cp(const CpPlan &p, int tid, const char *buf, size_t V, size_t zp, unsigned slot)
+{
+#pragma unroll
+    for (int q = 0; q < NITEM; q++) {
+        const int item = tid + q * NTHREADS;
+        if (p.lin[q] < 0 || item < NELEM || item >= 2 * NELEM) continue;
+        cp_async16(slot + (item - NELEM) * 16, buf + 16 * V + (zp + (size_t)p.lin[q]) * 16);
+    }
+}
+
 // one thread: the three halo boxes of plane z of the tile at (x0, y0) into `slot`, completion on `bar`
 __device__ inline void stage_plane_tma(const PackMaps &m, int x0, int y0, int z, unsigned slot, unsigned bar,
                                        unsigned long long pol)
