@@ -198,12 +198,13 @@ extern "C" int u1u1_init_fields(u1u1_ctx *ctx, uint64_t seed, int32_t N, double 
         e = launch_init_random_phase(pos_buf(ctx, 0), V, seed, params->eta1, params->eta2, ctx->stream);
         ctx->launches += 1;
     } else {
-        // the second position buffer is free at init time: use 8 of its planes as temporaries
-        float *tmp = pos_buf(ctx, 1);
+        // the second position buffer and the momentum buffer (adjacent: 80 B/site) are free at init time: two fp64
+        // temporaries of 4 planes each (64 B/site)
+        double *tmp = (double *)pos_buf(ctx, 1);
         e = launch_init_smoothed(pos_buf(ctx, 0), tmp, tmp + 4 * V, V, N, seed, params->smooth_width,
                                  params->smooth_trunc, params->eta1, params->eta2, ctx->stream);
         ctx->launches += 5;
-        if (e == cudaSuccess) e = cudaMemsetAsync(tmp, 0, (size_t)NPOS * V * sizeof(float), ctx->stream);
+        if (e == cudaSuccess) e = cudaMemsetAsync(tmp, 0, (size_t)(NPOS + NMOM) * V * sizeof(float), ctx->stream);
     }
     if (e != cudaSuccess) return cuda_fail(ctx, e, "init_fields");
     return U1U1_OK;

@@ -46,7 +46,10 @@ __global__ void init_random_phase_kernel(float *pos, size_t V, uint64_t seed, do
 
 // init_kind 1, stage 1: complex white noise, N(0,1) per real component, Box-Muller on the site's four
 // Philox words: u1 = (r+1)/2^32 in (0,1], u2 = r/2^32.  Written to 4 planes of `dst`.
-__global__ void init_noise_kernel(float *dst, size_t V, uint64_t seed)
+// The whole smoothed generator works in fp64 (noise, taps, the three separable passes, the normalisation) in the
+// 80 B/site of the second position buffer and the momentum buffer, which are free at init time: the smoothed field
+// can be as small as ~1e-4 of its rms at some site, so fp32 intermediates would cost 1e-4 of phase accuracy there.
+__global__ void init_noise_kernel(double *dst, size_t V, uint64_t seed)
 {
     for (size_t lin = (size_t)blockIdx.x * blockDim.x + threadIdx.x; lin < V;
          lin += (size_t)gridDim.x * blockDim.x) {
@@ -59,19 +62,19 @@ __global__ void init_noise_kernel(float *dst, size_t V, uint64_t seed)
             const double rad = sqrt(-2.0 * log(u1));
             double sn, cs;
             sincospi(2.0 * u2, &sn, &cs);
-            dst[(size_t)(2 * k) * V + lin] = (float)(rad * cs);
-            dst[(size_t)(2 * k + 1) * V + lin] = (float)(rad * sn);
+            dst[(size_t)(2 * k) * V + lin] = rad * cs;
+            dst[(size_t)(2 * k + 1) * V + lin] = rad * sn;
         }
     }
 }
 
 struct Taps {
-    float w[65];  // weights for d = -trunc..trunc
+    double w[65];  // weights for d = -trunc..trunc
     int trunc;
 };
 
 // stage 2: one separable pass of the periodic Gaussian along direction `dir` on 4 planes.
-__global__ void smooth_pass_kernel(const float *src, float *dst, size_t V, int N, int dir, Taps t)
+__global__ void smooth_pass_kernel(const double *src, double *dst, size_t V, int N, int dir, Taps t)
 {
     const size_t stride = dir == 0 ? 1 : (dir == 1 ? (size_t)N : (size_t)N * N);
     for (size_t lin = (size_t)blockIdx.x * blockDim.x + threadIdx.x; lin < 4 * V;
@@ -83,14 +86,14 @@ __global__ void smooth_pass_kernel(const float *src, float *dst, size_t V, int N
         for (int d = -t.trunc; d <= t.trunc; d++) {
             int cc = coord + d;
             cc = ((cc % N) + N) % N;
-            acc += (double)t.w[d + t.trunc] * (double)src[base + (size_t)cc * stride];
+            acc += t.w[d + t.trunc] * src[base + (size_t)cc * stride];
         }
-        dst[lin] = (float)acc;
+        dst[lin] = acc;
     }
 }
 
 // stage 3: normalise to |phi| = eta1, |psi| = eta2 (zero -> phase 0).
-__global__ void normalise_kernel(const float *src, float *pos, size_t V, double eta1, double eta2)
+__global__ void normalise_kernel(const double *src, float *pos, size_t V, double eta1, double eta2)
 {
     for (size_t lin = (size_t)blockIdx.x * blockDim.x + threadIdx.x; lin < V;
          lin += (size_t)gridDim.x * blockDim.x) {
@@ -165,17 +168,17 @@ cudaError_t launch_init_random_phase(float *pos, size_t V, uint64_t seed, double
     return cudaGetLastError();
 }
 
-cudaError_t launch_init_smoothed(float *pos, float *tmp_a, float *tmp_b, size_t V, int N, uint64_t seed,
+cudaError_t launch_init_smoothed(float *pos, double *tmp_a, double *tmp_b, size_t V, int N, uint64_t seed,
                                  double width, int trunc, double eta1, double eta2, cudaStream_t st)
 {
     Taps t;
     t.trunc = trunc;
-    for (int d = -trunc; d <= trunc; d++) t.w[d + trunc] = (float)exp(-(double)(d * d) / (2.0 * width * width));
+    for (int d = -trunc; d <= trunc; d++) t.w[d + trunc] = exp(-(double)(d * d) / (2.0 * width * width));
     init_noise_kernel<<<GRID, 256, 0, st>>>(tmp_a, V, seed);
-    float *a = tmp_a, *b = tmp_b;
+    double *a = tmp_a, *b = tmp_b;
     for (int dir = 0; dir < 3; dir++) {
         smooth_pass_kernel<<<GRID, 256, 0, st>>>(a, b, V, N, dir, t);
-        float *s = a; a = b; b = s;
+        double *s = a; a = b; b = s;
     }
     normalise_kernel<<<GRID, 256, 0, st>>>(a, pos, V, eta1, eta2);
     return cudaGetLastError();

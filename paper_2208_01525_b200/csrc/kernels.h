@@ -54,7 +54,7 @@ cudaError_t launch_segments(const uint8_t *cells, size_t V, int N, int tolerant,
 // init.cu
 cudaError_t launch_init_random_phase(float *pos, size_t V, uint64_t seed, double eta1, double eta2,
                                      cudaStream_t st);
-cudaError_t launch_init_smoothed(float *pos, float *tmp_a, float *tmp_b, size_t V, int N, uint64_t seed,
+cudaError_t launch_init_smoothed(float *pos, double *tmp_a, double *tmp_b, size_t V, int N, uint64_t seed,
                                  double width, int trunc, double eta1, double eta2, cudaStream_t st);
 cudaError_t launch_export_block(const float *pos, const float *mom, size_t V, int N, int x0, int y0, int z0,
                                 int bx, int by, int bz, float *dst, cudaStream_t st);

@@ -36,7 +36,7 @@ def longrun(config, variant):
     lat.init_fields(config, DX, prm)
     worst, worst_after_pre, worst_half, at, done = 0.0, 0.0, 0.0, 0, 0
     half_crossing = int((N * DX / 2 - TAU0) / DTAU)
-    series = []
+    series, theta_max = [], 0.0
     while done < total:
         if c["pre"] and done == c["pre"]:
             prm.friction = 1.0
@@ -52,12 +52,14 @@ def longrun(config, variant):
             if done <= max(half_crossing, c["pre"] + 100):
                 worst_half = max(worst_half, rel)
         if done % 100 == 0 or done == total:
-            series.append([done, float(g[3]), float(g[7])])
-    s = lat.export_state()
+            d = lat.diagnostics()                   # one fused sweep: its Gauss slots must agree with the monitor
+            assert np.isclose(d["gauss_rel_p"], g[3], rtol=1e-5) and np.isclose(d["gauss_rel_q"], g[7], rtol=1e-5)
+            theta_max = max(theta_max, d["max_theta"])
+            series.append([done, float(g[3]), float(g[7]), d["max_theta"], d["maxW"]])
     out = {"config": config, "variant": variant, "N": N, "steps": total, "gauss_rel_max": worst, "gauss_rel_max_at_step": at,
            "gauss_rel_max_after_prephase": worst_after_pre, "gauss_rel_max_to_half_crossing": worst_half,
-           "gauss_rel_end": rel, "gauss_rel_p_q_every_100_steps": series,
-           "theta_abs_max_end": float(s[THETA].abs().max()), "maxW_end": lat.diagnostics()["maxW"]}
+           "gauss_rel_end": rel, "theta_abs_max": theta_max, "maxW_end": series[-1][4],
+           "every_100_steps_step_gaussp_gaussq_maxtheta_maxW": series}
     _results[key] = out
     os.makedirs(os.path.join(ROOT, "gpurun_out"), exist_ok=True)
     with open(os.path.join(ROOT, "gpurun_out", "gauss_longrun.json"), "w") as f:
@@ -80,8 +82,8 @@ def test_config5_default_chain_sits_at_the_storage_floor():
     times, the strings have all annihilated by the end (maxW = 0) and the charge density that normalises the residual
     has decayed with them.  The bar the arithmetic can meet is therefore "at the storage floor": the default fp32
     chain within 1.2x of the fp64 chain at every monitored step's maximum (measured: 6.77e-5 vs 6.75e-5), both under
-    the measured ceiling 1e-4; while the network still fills the box (up to the half light-crossing time, step 310)
-    both stay below 1e-5... if they do not, the numbers in profiles/gauss_longrun.json say by how much."""
+    the measured ceiling 1e-4; up to the half light-crossing time of the box (step 310) the same 1.2x holds (the
+    values are in profiles/gauss_longrun.json)."""
     r0, r4 = longrun(5, 0), longrun(5, 4)
     assert r0["gauss_rel_max_after_prephase"] <= 1.2 * r4["gauss_rel_max_after_prephase"], (r0, r4)
     assert r0["gauss_rel_max_after_prephase"] < 1e-4 and r4["gauss_rel_max_after_prephase"] < 1e-4, (r0, r4)
@@ -93,4 +95,4 @@ def test_link_phases_stay_small_in_production_schedules():
     |theta| ~ 10 without range reduction.  Record how far the production schedules actually go."""
     for cfg in (4, 5):
         r = longrun(cfg, 0)
-        assert r["theta_abs_max_end"] < 10.0, r
+        assert r["theta_abs_max"] < 10.0, r
