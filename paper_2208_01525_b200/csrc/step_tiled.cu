@@ -48,8 +48,9 @@ __device__ inline void phasor_diff(float th, float &sn, float &c1)
 {
     float sh, ch;
     phasor<FAST>(0.5f * th, sh, ch);
-    sn = 2.f * sh * ch;
-    c1 = 2.f * sh * sh;
+    const float sh2 = sh + sh;          // exact, so sn and c1 are bit-identical to 2 sh ch and 2 sh sh
+    sn = sh2 * ch;
+    c1 = sh2 * sh;
 }
 
 // P = ((a + b) - c) - d, always in this order: a plaquette evaluated at two different sites from the same

@@ -71,3 +71,80 @@ def test_create_validates_without_gpu(lib):
     assert b"unstable" in lib.u1u1_last_error(ctx)
     assert lib.u1u1_launch_count(ctx) == 0
     lib.u1u1_destroy(ctx)
+
+
+C_CLIENT = r"""
+/* A plain C99 client of include/u1u1.h: the header must compile as C, and the error paths must work without a GPU. */
+#include <stdio.h>
+#include <string.h>
+#include "u1u1.h"
+
+int main(void)
+{
+    u1u1_ctx *ctx = NULL;
+    u1u1_params p;
+    double out[U1U1_DIAG_LEN];
+    if (u1u1_state_bytes(64) != (size_t)30 * 64 * 64 * 64 * 4) return 1;
+    if (u1u1_scratch_bytes(64) < (size_t)10 * 64 * 64 * 64) return 2;
+    if (u1u1_state_bytes(66) != 0) return 3;
+    if (u1u1_create(&ctx, NULL, 0, NULL, 0, NULL) != U1U1_EINVAL) return 4;
+    if (!strstr(u1u1_last_error(NULL), "NULL")) return 5;
+    if (u1u1_create(&ctx, (void *)0x10000, (size_t)30 * 512 * 4, (void *)0x20000, (size_t)1 << 20, NULL) != U1U1_OK) return 6;
+    memset(&p, 0, sizeof p);
+    p.struct_size = (uint32_t)sizeof p;
+    p.lambda1 = p.lambda2 = 2.0; p.e1 = p.e2 = 1.0; p.eta1 = p.eta2 = 1.0; p.kappa = 0.9;
+    p.dtau = 0.1; p.tau_norm = 1.0; p.friction = 1.0; p.smooth_width = 5.0; p.smooth_trunc = 20;
+    if (u1u1_step(ctx, 1, 1.0, 0.5, 1.0) != U1U1_ESTATE) return 7;
+    if (u1u1_configure(ctx, 16, 0.5, &p) != U1U1_ESIZE) return 8;
+    p.kappa = 1.0;
+    if (u1u1_configure(ctx, 8, 0.5, &p) != U1U1_EPARAM) return 9;
+    p.kappa = 0.9;
+    if (u1u1_configure(ctx, 8, 0.5, &p) != U1U1_OK) return 10;
+    if (u1u1_step(ctx, 1, 12.0, 0.5, 1.0) != U1U1_EUNSTABLE) return 11;
+    if (u1u1_cool(ctx, 1, 0.05) != U1U1_EUNSTABLE) return 12;
+    if (u1u1_export_windings(ctx, 0, NULL, NULL, NULL) != U1U1_ESTATE) return 13;
+    if (u1u1_pq_segments(ctx, 1, 0, out) != U1U1_ESTATE) return 14;
+    if (u1u1_diagnostics(ctx, NULL) != U1U1_EINVAL) return 15;
+    if (u1u1_launch_count(ctx) != 0) return 16;
+    printf("%s\n", u1u1_last_error(ctx));
+    u1u1_destroy(ctx);
+    return U1U1_D_USED <= U1U1_DIAG_LEN ? 0 : 17;
+}
+"""
+
+
+def test_header_compiles_as_c99_and_links(lib, tmp_path):
+    """include/u1u1.h is a C header: a C99 client built with gcc -std=c99 -Wall -Werror -pedantic links against
+    libu1u1.so and exercises the size queries and every error path that needs no GPU."""
+    import subprocess
+    src = tmp_path / "client.c"
+    src.write_text(C_CLIENT)
+    exe = tmp_path / "client"
+    pkg = os.path.join(ROOT, "paper_2208_01525_b200")
+    subprocess.check_call(["gcc", "-std=c99", "-Wall", "-Wextra", "-Werror", "-pedantic", "-I", os.path.join(ROOT, "include"),
+                           "-o", str(exe), str(src), "-L", pkg, "-l:libu1u1.so", f"-Wl,-rpath,{pkg}"])
+    r = subprocess.run([str(exe)], capture_output=True, text=True)
+    assert r.returncode == 0, (r.returncode, r.stdout, r.stderr)
+    assert "needs u1u1_diagnostics" in r.stdout or "NULL" in r.stdout
+
+
+def test_create_error_is_per_thread(lib):
+    """The message of a failed u1u1_create lives in thread-local storage: two host threads do not race on it."""
+    import threading
+    seen = {}
+
+    def worker(tag, misaligned):
+        ctx = ctypes.c_void_p()
+        if misaligned:
+            rc = lib.u1u1_create(ctypes.byref(ctx), 0x1001, 10, 0x2000, 10, None)
+        else:
+            rc = lib.u1u1_create(ctypes.byref(ctx), None, 0, None, 0, None)
+        seen[tag] = (rc, lib.u1u1_last_error(None))
+
+    ts = [threading.Thread(target=worker, args=("a", True)), threading.Thread(target=worker, args=("b", False))]
+    for t in ts:
+        t.start()
+    for t in ts:
+        t.join()
+    assert seen["a"][0] == -1 and b"aligned" in seen["a"][1]
+    assert seen["b"][0] == -1 and b"NULL" in seen["b"][1]
