@@ -67,7 +67,9 @@ typedef struct {
                                 4 = tiled, fp64 kick chain, SFU phasor (Gauss residual AT the storage floor);
                                 5 / 6 / 7 = 2 / 4 / 0 with libm sincosf instead of the SFU phasor;
                                 1 / 3 = reference one-thread-per-site kernel in fp32 / fp64.
-                                Bits 4.. are tuning switches of the tiled kernel (0 in production).        */
+                                Bits 4.. are tuning switches (0 in production): 16*2 = cp.async staging everywhere
+                                (no TMA), 16*4 = momenta by ld.global.cs, 16*8 = plain grid order (step kernel);
+                                16*16 / 16*32 = L2 policies, 16*64 / 16*128 = 16 / 32-plane chunks (diagnostics).  */
 } u1u1_params;
 
 /* Bytes of device memory the caller must provide for an N^3 lattice.

@@ -125,7 +125,7 @@ static int check_params(u1u1_ctx *ctx, const u1u1_params *p)
     if (p->init_kind != 0 && p->init_kind != 1) return fail(ctx, U1U1_EINVAL, "init_kind must be 0 or 1");
     if (p->init_kind == 1 && (!(p->smooth_width > 0) || p->smooth_trunc < 1 || p->smooth_trunc > 32))
         return fail(ctx, U1U1_EINVAL, "init_kind 1 needs smooth_width > 0 and 1 <= smooth_trunc <= 32");
-    if (p->kernel_variant < 0 || (p->kernel_variant & 15) > 7 || p->kernel_variant > 255)
+    if (p->kernel_variant < 0 || (p->kernel_variant & 15) > 7 || p->kernel_variant > 4095)
         return fail(ctx, U1U1_EINVAL, "kernel_variant must be 0..7 (+16*tuning flags)");
     return U1U1_OK;
 }

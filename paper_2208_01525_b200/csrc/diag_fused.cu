@@ -98,7 +98,8 @@ diag_fused_kernel(const float *__restrict__ posp, const float *__restrict__ momp
     const size_t NN = (size_t)N * N;
     const int tid = threadIdx.x, tx = tid & (TX - 1), ty = tid / TX, warp = tid >> 5, lane = tid & 31;
     const char *pos = reinterpret_cast<const char *>(posp);
-    const unsigned long long pol_stream = policy_evict_first(), pol_keep = policy_evict_last();
+    const unsigned long long pol_stream = (k.flags & 32) ? policy_evict_last() : policy_evict_first();
+    const unsigned long long pol_keep = (k.flags & 16) ? policy_evict_first() : policy_evict_last();
     const int ntx = (N + TX - 1) / TX, nty = (N + TY - 1) / TY, nzc = (N + zchunk - 1) / zchunk;
     const int items = ntx * nty * nzc;
     const float4 *gMA = reinterpret_cast<const float4 *>(momp);
@@ -127,6 +128,7 @@ diag_fused_kernel(const float *__restrict__ posp, const float *__restrict__ momp
         float gmax[2] = {0.f, 0.f}, maxth = 0.f;
         unsigned wsum = 0, csum = 0;          // sum |W| (lanes p: bits 0..15, q: 16..31); pierced cells p, q (same lanes)
         int npq = 0, nnear = 0, maxw = 0;     // cells pierced by both; near-cut plaquettes (p: bits 0..15, q: 16..31)
+        unsigned wany = 0;                    // OR of all |W| lanes: tells max|W| = 0 from 1
 
         // ---- staging: relative position plane j = 0 .. nz (slot = running plane count mod 3), momentum pack B (with
         // halo) of plane m = 0 .. nz-1 (slot = running count mod 2).  TMA tiles: one thread issues box loads that
@@ -355,7 +357,7 @@ diag_fused_kernel(const float *__restrict__ posp, const float *__restrict__ momp
                 unsigned Eabs[6], flagged = 0;
 #pragma unroll
                 for (int q = 0; q < 6; q++) {
-                    Eabs[q] = __vabsdiffu4(P[q], Q[q]) & VAL_LANES;
+                    Eabs[q] = __vabsdiffu4(P[q], Q[q]);             // lanes 1 / 3 (flags) hold rubbish: masked after summing
                     flagged |= P[q] | Q[q];
                 }
                 int wsg[2][3];                                      // signed windings of the own plaquettes (EXPORT)
@@ -420,7 +422,7 @@ diag_fused_kernel(const float *__restrict__ posp, const float *__restrict__ momp
                                 const int W = __float2int_rn(sum * INV_2PI);
 #pragma unroll
                                 for (int qq = 0; qq < 6; qq++)
-                                    if (qq == q) Eabs[qq] = (Eabs[qq] & ~(0xffu << (16 * sec))) | (aW << (16 * sec));
+                                    if (qq == q) Eabs[qq] = (Eabs[qq] & VAL_LANES & ~(0xffu << (16 * sec))) | (aW << (16 * sec));
                                 if (EXPORT) {
 #pragma unroll
                                     for (int o = 0; o < 3; o++)
@@ -430,24 +432,23 @@ diag_fused_kernel(const float *__restrict__ posp, const float *__restrict__ momp
                             if (near && q < 3) nearbits |= 1u << (3 * sec + q);
                         }
                     }
+                    nnear += __popc(nearbits & 7u) + (__popc(nearbits & 56u) << 16);
                 }
-                // own plaquettes: length sums, near-cut counts, largest winding
-                const unsigned own = Eabs[0] + Eabs[1] + Eabs[2];
+                // own plaquettes: length sums, largest winding (|W| >= 2 is rare: exact maximum only then)
+                const unsigned own = (Eabs[0] + Eabs[1] + Eabs[2]) & VAL_LANES;
                 wsum += own;
-                nnear += __popc(nearbits & 7u) + (__popc(nearbits & 56u) << 16);
-                if ((Eabs[0] | Eabs[1] | Eabs[2]) & 0x00fe00feu) {
+                wany |= own;
+                if (own & 0x00fe00feu) {                            // a lane sum >= 2: maybe a |W| >= 2
 #pragma unroll
-                    for (int q = 0; q < 3; q++) maxw = max(maxw, (int)max(Eabs[q] & 0xffu, Eabs[q] >> 16));
-                } else if (own) {
-                    maxw = max(maxw, 1);
+                    for (int q = 0; q < 3; q++) maxw = max(maxw, (int)max(Eabs[q] & 0xffu, (Eabs[q] >> 16) & 0xffu));
                 }
                 // pierced cells: the six faces of the cell at x
-                const unsigned cell = own + Eabs[3] + Eabs[4] + Eabs[5];
-                const unsigned cp = cell & 0xffu, cq = cell >> 16;
-                cells[lin] = (uint8_t)cp;
-                cells[V + lin] = (uint8_t)cq;
-                csum += (cp ? 1u : 0u) + (cq ? 0x10000u : 0u);
-                npq += (cp && cq) ? 1 : 0;
+                const unsigned cell = (own + Eabs[3] + Eabs[4] + Eabs[5]) & VAL_LANES;
+                cells[lin] = (uint8_t)cell;
+                cells[V + lin] = (uint8_t)(cell >> 16);
+                const unsigned nzl = ((cell + 0x00ff00ffu) >> 8) & 0x00010001u;      // 1 per lane whose cell is pierced
+                csum += nzl;
+                npq += (int)(nzl & (nzl >> 16));
                 if (EXPORT) {
 #pragma unroll
                     for (int sec = 0; sec < 2; sec++)
@@ -481,7 +482,7 @@ diag_fused_kernel(const float *__restrict__ posp, const float *__restrict__ momp
         add(FR_CELLS + 2, (double)__reduce_add_sync(0xffffffffu, (unsigned)npq));
         amax(FR_GMAX, (double)__uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(gmax[0]))));
         amax(FR_GMAX + 1, (double)__uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(gmax[1]))));
-        amax(FR_MAXW, (double)__reduce_max_sync(0xffffffffu, (unsigned)maxw));
+        amax(FR_MAXW, (double)__reduce_max_sync(0xffffffffu, (unsigned)max(maxw, wany ? 1 : 0)));
         amax(FR_MAXTH, (double)__uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(maxth))));
     }
 
@@ -497,7 +498,10 @@ diag_fused_kernel(const float *__restrict__ posp, const float *__restrict__ momp
 
 }  // namespace
 
-int fused_zchunk(int N) { return N >= 32 ? 32 : N; }
+// z planes per work item.  Longer chunks amortise the prologue (phases and in-plane links of the chunk's first plane)
+// and the extra boundary plane: measured at 1024^3, 16 planes 30.2 ms, 32: 28.8, 64: 28.3.  The per-item fp32 partial
+// sums hold at most this many terms.
+int fused_zchunk(int N) { return N >= 64 ? 64 : N; }
 
 cudaError_t launch_diag_fused(const float *pos, const float *mom, size_t V, int N, FusedCoef k, uint8_t *cells, uint8_t *codes,
                               double *partials, int *nblocks, const DiagMaps *maps, int sms, cudaStream_t st)
@@ -508,7 +512,7 @@ cudaError_t launch_diag_fused(const float *pos, const float *mom, size_t V, int 
         memset(&m, 0, sizeof m);
         k.flags |= 2;
     }
-    const int zc = fused_zchunk(N);
+    const int zc = (k.flags & 64) ? (N >= 16 ? 16 : N) : (k.flags & 128) ? (N >= 32 ? 32 : N) : fused_zchunk(N);   // tuning flags
     const int ntx = (N + TX - 1) / TX, nty = (N + TY - 1) / TY, nzc = (N + zc - 1) / zc;
     const long items = (long)ntx * nty * nzc;
     long grid = (long)sms * FUSED_CTAS;

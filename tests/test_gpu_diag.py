@@ -107,6 +107,35 @@ def test_diagnostics_gauss_slots_match_the_monitor():
         assert np.isclose(d["max_theta"], np.max(np.abs(s0[[8, 9, 10, 14, 15, 16]])), rtol=1e-7)
 
 
+def test_fused_sweep_staging_paths_bit_identical():
+    """The fused sweep stages interior tiles by TMA boxes and boundary tiles by cp.async; forcing cp.async everywhere
+    (tuning flag 2) or other z-chunk lengths (flags 64, 128: different work items, same per-site arithmetic) must give
+    identical integer results and windings, and sums equal up to the order of the fp64 additions -- on a lattice with
+    interior, boundary and ragged tiles."""
+    from paper_2208_01525_b200 import Lattice, Params
+    import torch
+    N = 132
+    s0 = inputs.to_f32_exact(inputs.random_state((N, N, N), seed=17, amp_theta=1.5))
+    outs = []
+    for flags in (0, 2, 64, 128 + 2):
+        lat = Lattice(N)
+        lat.configure(DX, Params(kernel_variant=16 * flags, tau_norm=1.5))
+        lat.import_state(torch.from_numpy(s0.astype(np.float32)))
+        lat.set_time(2.0, 0.5, 1.0)
+        d = lat.diagnostics()
+        W = [t.cpu().numpy() for sec in (0, 1) for t in lat.export_windings(sec)]
+        outs.append((d, W))
+    ints = ("sumW_p", "sumW_q", "cells_p", "cells_q", "cells_pq", "near_p", "near_q", "maxW", "cells_pq_tol_p", "cells_pq_tol_q",
+            "max_theta", "gauss_max_p", "gauss_max_q")
+    for d, W in outs[1:]:
+        assert all(d[k] == outs[0][0][k] for k in ints), {k: (d[k], outs[0][0][k]) for k in ints}
+        assert all(np.array_equal(a, b) for a, b in zip(W, outs[0][1]))
+    assert outs[1][0] == outs[0][0]                      # same work items, other staging path: every digit
+    for k in ("sum_L", "sum_kin", "sum_grad", "sum_elec", "sum_mag", "sum_pot", "gauss_l2_p", "gauss_rho_q"):
+        assert all(np.isclose(d[k], outs[0][0][k], rtol=1e-6) for d, _ in outs[2:]), k
+    assert outs[0][0]["sumW_p"] > 0 and outs[0][0]["cells_pq"] > 0
+
+
 def test_windings_with_exactly_zero_sites():
     """Reading R-15: atan2(0, 0) = 0, i.e. a link with an end point where the field is exactly zero has chi = 0 in the
     printed formula.  Zero sites sprinkled over a state with strings (vortex cores put exactly ON lattice sites do
