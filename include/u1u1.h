@@ -181,6 +181,31 @@ int u1u1_pq_segments(u1u1_ctx *ctx, int32_t min_cells, int32_t tolerant, double 
  * linear index (x + N (y + N z)) of the smallest cell of its segment. */
 int u1u1_export_labels(u1u1_ctx *ctx, void *labels_dev);
 
+/* ---- z slabs: ONE lattice split over several GPUs.  Not the default: the
+ * benchmark workload fits one GPU and runs there (north_star); this is the path to lattices that do not (PAPER.md:31:
+ * 4096^3).  The global lattice is N x N x NZ_global, periodic; a rank's context owns nz_own consecutive z planes starting
+ * at global plane z_first, stored with one halo plane below and above (buffer planes 0 .. nz_own + 1).  u1u1_step on a
+ * slab advances the own planes by ONE step with the fused kernel and stores its top / bottom plane of the new positions
+ * straight into the halo planes of the neighbouring slabs (plain stores through peer memory: NVLink when the neighbour
+ * lives on another GPU), so there is no separate exchange pass.  Between two steps the caller must make sure that every
+ * rank has finished the previous one (stream-ordered barrier / torch.distributed).  All slabs must have the same nz_own.
+ * Available on a slab: set_params, step (n = 1, kernel_variant 0), init_slab, import_slab / export_slab, push_halos,
+ * launch_count; the diagnostics calls need a cubic lattice (U1U1_ESTATE). */
+size_t u1u1_slab_state_bytes(int32_t N, int32_t nz_own);
+int u1u1_configure_slab(u1u1_ctx *ctx, int32_t N, int32_t nz_own, int64_t z_first, double dx, const u1u1_params *params);
+/* DEVICE pointers to the STATE buffers (as given to u1u1_create) of the slabs above and below (periodic: the top
+ * slab's upper neighbour is the bottom slab; with a single slab both are its own buffer). */
+int u1u1_set_slab_peers(u1u1_ctx *ctx, void *up_state_dev, void *dn_state_dev);
+/* The random-phase initial condition of the GLOBAL lattice (same Philox counters = global site indices as
+ * u1u1_init_fields) restricted to this slab's own planes; halo planes via u1u1_push_halos. */
+int u1u1_init_slab(u1u1_ctx *ctx, uint64_t seed);
+/* Canonical float32 [20][nz_own][N][N] (own planes only), DEVICE. */
+int u1u1_export_slab(u1u1_ctx *ctx, void *dst_dev);
+int u1u1_import_slab(u1u1_ctx *ctx, const void *src_dev);
+/* Copy this slab's boundary planes of the current positions into the neighbours' halo planes (once, after init_slab /
+ * import_slab on every rank; afterwards every step does it itself). */
+int u1u1_push_halos(u1u1_ctx *ctx);
+
 /* Number of kernel launches issued by this context so far (for bench.py's gpu_launches). */
 uint64_t u1u1_launch_count(const u1u1_ctx *ctx);
 

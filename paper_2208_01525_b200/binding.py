@@ -51,7 +51,9 @@ _lib = None
 SYMBOLS = ["u1u1_state_bytes", "u1u1_scratch_bytes", "u1u1_create", "u1u1_destroy", "u1u1_last_error",
            "u1u1_configure", "u1u1_init_fields", "u1u1_set_params", "u1u1_set_time", "u1u1_step", "u1u1_cool",
            "u1u1_diagnostics", "u1u1_gauss_violation", "u1u1_export_state", "u1u1_import_state",
-           "u1u1_export_state_host", "u1u1_import_state_host", "u1u1_export_windings", "u1u1_export_block", "u1u1_launch_count", "u1u1_pq_segments", "u1u1_export_labels", "u1u1_import_state_tiled"]
+           "u1u1_export_state_host", "u1u1_import_state_host", "u1u1_export_windings", "u1u1_export_block", "u1u1_launch_count", "u1u1_pq_segments", "u1u1_export_labels", "u1u1_import_state_tiled",
+           "u1u1_slab_state_bytes", "u1u1_configure_slab", "u1u1_set_slab_peers", "u1u1_init_slab", "u1u1_export_slab",
+           "u1u1_import_slab", "u1u1_push_halos"]
 
 
 def load():
@@ -88,6 +90,13 @@ def load():
     L.u1u1_export_labels.argtypes = [vp, vp]
     L.u1u1_import_state_tiled.argtypes = [vp, vp, i32]
     L.u1u1_launch_count.argtypes = [vp]; L.u1u1_launch_count.restype = u64
+    L.u1u1_slab_state_bytes.argtypes = [i32, i32]; L.u1u1_slab_state_bytes.restype = ctypes.c_size_t
+    L.u1u1_configure_slab.argtypes = [vp, i32, i32, ctypes.c_int64, d, pp]
+    L.u1u1_set_slab_peers.argtypes = [vp, vp, vp]
+    L.u1u1_init_slab.argtypes = [vp, u64]
+    L.u1u1_export_slab.argtypes = [vp, vp]
+    L.u1u1_import_slab.argtypes = [vp, vp]
+    L.u1u1_push_halos.argtypes = [vp]
     _lib = L
     return L
 

@@ -21,7 +21,11 @@ struct u1u1_ctx {
     size_t scratch_bytes = 0;
     cudaStream_t stream = nullptr;
     int N = 0;
-    size_t V = 0;
+    size_t V = 0;                // sites in one buffer (N^3; N * N * (nz_own + 2) for a z slab)
+    // z slab of a lattice split over several GPUs (u1u1_configure_slab; 0 = ordinary cubic lattice)
+    int nz_own = 0;
+    int64_t z_first = 0;         // global index of the slab's first own plane
+    float *peer_up = nullptr, *peer_dn = nullptr;   // state buffers of the slabs above / below
     double dx = 0;
     u1u1_params prm{};
     bool configured = false;
@@ -148,10 +152,11 @@ static int prepare_device(u1u1_ctx *ctx)
         ctx->sms = sms;
     }
     if (!ctx->maps_ready && step_tiled_uses_tma(ctx->N)) {
-        const bool ok = encode_halo_maps(&ctx->pos_halo[0], pos_buf(ctx, 0), ctx->V, ctx->N) &&
-                        encode_halo_maps(&ctx->pos_halo[1], pos_buf(ctx, 1), ctx->V, ctx->N) &&
-                        encode_halo_maps(&ctx->mom_halo, mom_buf(ctx), ctx->V, ctx->N) &&
-                        encode_tile_maps(&ctx->mom_tile, mom_buf(ctx), ctx->V, ctx->N);
+        const int NZ = ctx->nz_own ? ctx->nz_own + 2 : ctx->N;
+        const bool ok = encode_halo_maps(&ctx->pos_halo[0], pos_buf(ctx, 0), ctx->V, ctx->N, NZ) &&
+                        encode_halo_maps(&ctx->pos_halo[1], pos_buf(ctx, 1), ctx->V, ctx->N, NZ) &&
+                        encode_halo_maps(&ctx->mom_halo, mom_buf(ctx), ctx->V, ctx->N, NZ) &&
+                        encode_tile_maps(&ctx->mom_tile, mom_buf(ctx), ctx->V, ctx->N, NZ);
         if (!ok) return fail(ctx, U1U1_ECUDA, "cuTensorMapEncodeTiled unavailable or rejected the layout (TMA is required)");
         ctx->maps_ready = true;
     }
@@ -168,6 +173,9 @@ extern "C" int u1u1_configure(u1u1_ctx *ctx, int32_t N, double dx, const u1u1_pa
     if (ctx->scratch_bytes < u1u1_scratch_bytes(N)) return fail(ctx, U1U1_ESIZE, "scratch buffer smaller than u1u1_scratch_bytes(N)");
     ctx->N = N;
     ctx->V = (size_t)N * N * N;
+    ctx->nz_own = 0;
+    ctx->z_first = 0;
+    ctx->peer_up = ctx->peer_dn = nullptr;
     ctx->dx = dx;
     ctx->prm = *params;
     ctx->configured = true;
@@ -195,7 +203,7 @@ extern "C" int u1u1_init_fields(u1u1_ctx *ctx, uint64_t seed, int32_t N, double 
     cudaError_t e = cudaMemsetAsync(ctx->state, 0, u1u1_state_bytes(N), ctx->stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "init_fields memset");
     if (params->init_kind == 0) {
-        e = launch_init_random_phase(pos_buf(ctx, 0), V, seed, params->eta1, params->eta2, ctx->stream);
+        e = launch_init_random_phase(pos_buf(ctx, 0), V, 0, 0, seed, params->eta1, params->eta2, ctx->stream);
         ctx->launches += 1;
     } else {
         // the second position buffer and the momentum buffer (adjacent: 80 B/site) are free at init time: two fp64
@@ -243,7 +251,19 @@ static int tiled_mode(int kv)
 static cudaError_t launch_step(u1u1_ctx *ctx, const StepCoef &q)
 {
     const int kv = ctx->prm.kernel_variant & 15;
-    Lattice L{pos_buf(ctx, ctx->cur), pos_buf(ctx, ctx->cur ^ 1), mom_buf(ctx), ctx->V, ctx->N};
+    Lattice L{};
+    L.pos_in = pos_buf(ctx, ctx->cur);
+    L.pos_out = pos_buf(ctx, ctx->cur ^ 1);
+    L.mom = mom_buf(ctx);
+    L.V = ctx->V;
+    L.N = ctx->N;
+    if (ctx->nz_own) {                       // z slab: neighbours have the same shape, their pos_out is the same ping-pong index
+        L.nz_own = ctx->nz_own;
+        L.peer_up_out = ctx->peer_up + (size_t)(ctx->cur ^ 1) * NPOS * ctx->V;
+        L.peer_dn_out = ctx->peer_dn + (size_t)(ctx->cur ^ 1) * NPOS * ctx->V;
+        L.peer_dn_plane = (size_t)ctx->nz_own + 1;
+        L.peer_up_V = L.peer_dn_V = ctx->V;
+    }
     const bool tiled = tiled_mode(kv) >= 0 && step_tiled_supports(ctx->N);
     if (!tiled) return launch_step_ref(L, q, ctx->stream, kv == 3);
     StepMaps maps;
@@ -252,6 +272,13 @@ static cudaError_t launch_step(u1u1_ctx *ctx, const StepCoef &q)
         maps.mom = ctx->mom_tile;
     }
     return launch_step_tiled(L, q, ctx->stream, tiled_mode(kv), ctx->maps_ready ? &maps : nullptr, ctx->sms);
+}
+
+// calls that read z neighbours through the periodic wrap of a cubic buffer are not available on a z slab
+static int cubic_only(u1u1_ctx *ctx, const char *what)
+{
+    if (!ctx->nz_own) return U1U1_OK;
+    return fail(ctx, U1U1_ESTATE, std::string(what) + " is not available on a z slab (u1u1_configure_slab)");
 }
 
 static void invalidate(u1u1_ctx *ctx) { ctx->diag_valid = ctx->codes_valid = ctx->labels_valid = false; }
@@ -263,6 +290,9 @@ extern "C" int u1u1_step(u1u1_ctx *ctx, int32_t n, double tau, double era_m, dou
     if (n < 0) return fail(ctx, U1U1_EINVAL, "n must be >= 0");
     if (!(era_m >= 0 && era_m < 1)) return fail(ctx, U1U1_EINVAL, "era_m must satisfy 0 <= m < 1");
     if (era_m != 0 && !(tau > 0)) return fail(ctx, U1U1_EINVAL, "tau must be positive in an expanding background");
+    if (ctx->nz_own && (!ctx->peer_up || !ctx->peer_dn)) return fail(ctx, U1U1_ESTATE, "step on a z slab needs u1u1_set_slab_peers first");
+    if (ctx->nz_own && (n > 1 || (ctx->prm.kernel_variant & 15) != 0))
+        return fail(ctx, U1U1_EINVAL, "a z slab steps one step per call (the ranks synchronise in between) with kernel_variant 0");
     const u1u1_params &P = ctx->prm;
     const double dx = ctx->dx, dt = P.dtau, f = P.friction;
     for (int k = 0; k < n; k++) {
@@ -316,6 +346,7 @@ extern "C" int u1u1_cool(u1u1_ctx *ctx, int32_t n, double dcool)
 {
     if (!ctx) return U1U1_EINVAL;
     if (!ctx->configured) return fail(ctx, U1U1_ESTATE, "cool before configure/init_fields");
+    if (int rc = cubic_only(ctx, "cool")) return rc;
     if (n < 0 || !(dcool > 0)) return fail(ctx, U1U1_EINVAL, "need n >= 0 and dcool > 0");
     const u1u1_params &P = ctx->prm;
     const double dx = ctx->dx;
@@ -417,6 +448,7 @@ extern "C" int u1u1_gauss_violation(u1u1_ctx *ctx, double *out)
 {
     if (!ctx || !out) return ctx ? fail(ctx, U1U1_EINVAL, "out is NULL") : U1U1_EINVAL;
     if (!ctx->configured) return fail(ctx, U1U1_ESTATE, "gauss_violation before configure/init_fields");
+    if (int rc = cubic_only(ctx, "gauss_violation")) return rc;
     cudaError_t e = launch_gauss(pos_buf(ctx, ctx->cur), mom_buf(ctx), ctx->V, ctx->N, diag_coef(ctx),
                                  partials(ctx), result(ctx), ctx->stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "gauss kernel launch");
@@ -455,6 +487,7 @@ extern "C" int u1u1_diagnostics(u1u1_ctx *ctx, double *out)
 {
     if (!ctx || !out) return ctx ? fail(ctx, U1U1_EINVAL, "out is NULL") : U1U1_EINVAL;
     if (!ctx->configured) return fail(ctx, U1U1_ESTATE, "diagnostics before configure/init_fields");
+    if (int rc = cubic_only(ctx, "diagnostics")) return rc;
     const size_t V = ctx->V;
     if (int rc = run_sweep(ctx, false)) return rc;
     double r[34];
@@ -508,7 +541,7 @@ extern "C" int u1u1_diagnostics(u1u1_ctx *ctx, double *out)
 
 static int relayout(u1u1_ctx *ctx, float *canon, int to_canonical)
 {
-    cudaError_t e = launch_relayout(pos_buf(ctx, ctx->cur), mom_buf(ctx), canon, ctx->V, 0, 20, to_canonical, ctx->stream);
+    cudaError_t e = launch_relayout(pos_buf(ctx, ctx->cur), mom_buf(ctx), canon, ctx->V, ctx->V, 0, 0, 20, to_canonical, ctx->stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "relayout kernel launch");
     ctx->launches += 1;
     if (!to_canonical) invalidate(ctx);
@@ -519,6 +552,7 @@ extern "C" int u1u1_export_state(u1u1_ctx *ctx, void *dst_dev)
 {
     if (!ctx || !dst_dev) return ctx ? fail(ctx, U1U1_EINVAL, "dst is NULL") : U1U1_EINVAL;
     if (!ctx->configured) return fail(ctx, U1U1_ESTATE, "export_state before configure/init_fields");
+    if (int rc = cubic_only(ctx, "export_state")) return rc;
     return relayout(ctx, (float *)dst_dev, 1);
 }
 
@@ -526,6 +560,7 @@ extern "C" int u1u1_import_state(u1u1_ctx *ctx, const void *src_dev)
 {
     if (!ctx || !src_dev) return ctx ? fail(ctx, U1U1_EINVAL, "src is NULL") : U1U1_EINVAL;
     if (!ctx->configured) return fail(ctx, U1U1_ESTATE, "import_state before configure");
+    if (int rc = cubic_only(ctx, "import_state")) return rc;
     return relayout(ctx, (float *)src_dev, 0);
 }
 
@@ -533,6 +568,7 @@ extern "C" int u1u1_import_state_tiled(u1u1_ctx *ctx, const void *src_dev, int32
 {
     if (!ctx || !src_dev) return ctx ? fail(ctx, U1U1_EINVAL, "src is NULL") : U1U1_EINVAL;
     if (!ctx->configured) return fail(ctx, U1U1_ESTATE, "import_state_tiled before configure");
+    if (int rc = cubic_only(ctx, "import_state_tiled")) return rc;
     if (n_src < 1 || ctx->N % n_src != 0) return fail(ctx, U1U1_ESIZE, "N must be a multiple of n_src");
     cudaError_t e = launch_import_tiled(pos_buf(ctx, ctx->cur), mom_buf(ctx), (const float *)src_dev, ctx->V, ctx->N, n_src, ctx->stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "import_state_tiled launch");
@@ -546,6 +582,7 @@ extern "C" int u1u1_export_block(u1u1_ctx *ctx, int32_t x0, int32_t y0, int32_t 
 {
     if (!ctx || !dst_dev) return ctx ? fail(ctx, U1U1_EINVAL, "dst is NULL") : U1U1_EINVAL;
     if (!ctx->configured) return fail(ctx, U1U1_ESTATE, "export_block before configure/init_fields");
+    if (int rc = cubic_only(ctx, "export_block")) return rc;
     if (bx < 1 || by < 1 || bz < 1 || bx > ctx->N || by > ctx->N || bz > ctx->N)
         return fail(ctx, U1U1_EINVAL, "block extents must lie in [1, N]");
     cudaError_t e = launch_export_block(pos_buf(ctx, ctx->cur), mom_buf(ctx), ctx->V, ctx->N, x0, y0, z0, bx, by,
@@ -583,7 +620,7 @@ static int host_copy(u1u1_ctx *ctx, void *host, int to_host)
         float *h = (float *)host + (size_t)c * V;
         if (to_host) {
             if (c >= 2) e = cudaStreamWaitEvent(ms, ctx->ev_copy[b], 0);              // staging plane b is free again
-            if (e == cudaSuccess) e = launch_relayout(pos_buf(ctx, ctx->cur), mom_buf(ctx), stage[b], V, c, 1, 1, ms);
+            if (e == cudaSuccess) e = launch_relayout(pos_buf(ctx, ctx->cur), mom_buf(ctx), stage[b], V, V, 0, c, 1, 1, ms);
             if (e == cudaSuccess) e = cudaEventRecord(ctx->ev_kernel[b], ms);
             if (e == cudaSuccess) e = cudaStreamWaitEvent(cs, ctx->ev_kernel[b], 0);
             if (e == cudaSuccess) e = cudaMemcpyAsync(h, stage[b], bytes, cudaMemcpyDeviceToHost, cs);
@@ -593,7 +630,7 @@ static int host_copy(u1u1_ctx *ctx, void *host, int to_host)
             if (e == cudaSuccess) e = cudaMemcpyAsync(stage[b], h, bytes, cudaMemcpyHostToDevice, cs);
             if (e == cudaSuccess) e = cudaEventRecord(ctx->ev_copy[b], cs);
             if (e == cudaSuccess) e = cudaStreamWaitEvent(ms, ctx->ev_copy[b], 0);
-            if (e == cudaSuccess) e = launch_relayout(pos_buf(ctx, ctx->cur), mom_buf(ctx), stage[b], V, c, 1, 0, ms);
+            if (e == cudaSuccess) e = launch_relayout(pos_buf(ctx, ctx->cur), mom_buf(ctx), stage[b], V, V, 0, c, 1, 0, ms);
             if (e == cudaSuccess) e = cudaEventRecord(ctx->ev_kernel[b], ms);
         }
         ctx->launches += 1;
@@ -608,6 +645,7 @@ extern "C" int u1u1_export_state_host(u1u1_ctx *ctx, void *dst_host)
 {
     if (!ctx || !dst_host) return ctx ? fail(ctx, U1U1_EINVAL, "dst is NULL") : U1U1_EINVAL;
     if (!ctx->configured) return fail(ctx, U1U1_ESTATE, "export_state_host before configure/init_fields");
+    if (int rc = cubic_only(ctx, "export_state_host")) return rc;
     return host_copy(ctx, dst_host, 1);
 }
 
@@ -615,6 +653,7 @@ extern "C" int u1u1_import_state_host(u1u1_ctx *ctx, const void *src_host)
 {
     if (!ctx || !src_host) return ctx ? fail(ctx, U1U1_EINVAL, "src is NULL") : U1U1_EINVAL;
     if (!ctx->configured) return fail(ctx, U1U1_ESTATE, "import_state_host before configure");
+    if (int rc = cubic_only(ctx, "import_state_host")) return rc;
     return host_copy(ctx, const_cast<void *>(src_host), 0);
 }
 
@@ -674,5 +713,108 @@ extern "C" int u1u1_export_windings(u1u1_ctx *ctx, int32_t sector, void *w_dev, 
         cudaError_t e = cudaMemcpyAsync(cells_dev, cells_buf(ctx) + (size_t)sector * V, V, cudaMemcpyDeviceToDevice, ctx->stream);
         if (e != cudaSuccess) return cuda_fail(ctx, e, "cells copy");
     }
+    return U1U1_OK;
+}
+
+// ---- z slabs: one lattice split over several GPUs (SURVEY.md 8(f)-4 "then z-slab multi-GPU") -------
+static bool slab_ok(int32_t N, int32_t nz_own) { return N >= 8 && N <= 8192 && (N % 4) == 0 && nz_own >= 1 && nz_own <= 8192; }
+
+extern "C" size_t u1u1_slab_state_bytes(int32_t N, int32_t nz_own)
+{
+    if (!slab_ok(N, nz_own)) return 0;
+    return (size_t)(2 * NPOS + NMOM) * (size_t)N * N * (size_t)(nz_own + 2) * sizeof(float);
+}
+
+extern "C" int u1u1_configure_slab(u1u1_ctx *ctx, int32_t N, int32_t nz_own, int64_t z_first, double dx, const u1u1_params *params)
+{
+    if (!ctx) return U1U1_EINVAL;
+    if (!slab_ok(N, nz_own) || z_first < 0) return fail(ctx, U1U1_ESIZE, "slab: N a multiple of 4 in [8, 8192], 1 <= nz_own <= 8192, z_first >= 0");
+    if (!(dx > 0)) return fail(ctx, U1U1_EINVAL, "dx must be positive");
+    if (int rc = check_params(ctx, params)) return rc;
+    if (ctx->state_bytes < u1u1_slab_state_bytes(N, nz_own)) return fail(ctx, U1U1_ESIZE, "state buffer smaller than u1u1_slab_state_bytes(N, nz_own)");
+    ctx->N = N;
+    ctx->V = (size_t)N * N * (size_t)(nz_own + 2);
+    ctx->nz_own = nz_own;
+    ctx->z_first = z_first;
+    ctx->peer_up = ctx->peer_dn = nullptr;
+    ctx->dx = dx;
+    ctx->prm = *params;
+    ctx->configured = true;
+    ctx->cur = 0;
+    ctx->tau_pos = params->tau_norm;
+    ctx->a = ctx->c = ctx->cG = 1.0;
+    invalidate(ctx);
+    ctx->maps_ready = false;
+    return U1U1_OK;
+}
+
+extern "C" int u1u1_set_slab_peers(u1u1_ctx *ctx, void *up_state_dev, void *dn_state_dev)
+{
+    if (!ctx) return U1U1_EINVAL;
+    if (!ctx->nz_own) return fail(ctx, U1U1_ESTATE, "set_slab_peers needs u1u1_configure_slab first");
+    if (!up_state_dev || !dn_state_dev) return fail(ctx, U1U1_EINVAL, "peer state buffers must not be NULL");
+    ctx->peer_up = (float *)up_state_dev;
+    ctx->peer_dn = (float *)dn_state_dev;
+    return U1U1_OK;
+}
+
+extern "C" int u1u1_init_slab(u1u1_ctx *ctx, uint64_t seed)
+{
+    if (!ctx) return U1U1_EINVAL;
+    if (!ctx->nz_own) return fail(ctx, U1U1_ESTATE, "init_slab needs u1u1_configure_slab first");
+    if (ctx->prm.init_kind != 0) return fail(ctx, U1U1_EINVAL, "init_slab generates the random-phase initial condition only (init_kind 0)");
+    const size_t NN = (size_t)ctx->N * ctx->N;
+    cudaError_t e = cudaMemsetAsync(ctx->state, 0, u1u1_slab_state_bytes(ctx->N, ctx->nz_own), ctx->stream);
+    if (e == cudaSuccess)
+        e = launch_init_random_phase(pos_buf(ctx, 0), NN * ctx->nz_own, NN, NN * (size_t)ctx->z_first, seed, ctx->prm.eta1,
+                                     ctx->prm.eta2, ctx->stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "init_slab");
+    ctx->launches += 1;
+    ctx->cur = 0;
+    return U1U1_OK;
+}
+
+static int slab_relayout(u1u1_ctx *ctx, float *canon, int to_canonical)
+{
+    const size_t NN = (size_t)ctx->N * ctx->N;
+    cudaError_t e = launch_relayout(pos_buf(ctx, ctx->cur), mom_buf(ctx), canon, ctx->V, NN * ctx->nz_own, NN, 0, 20, to_canonical,
+                                    ctx->stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "slab relayout launch");
+    ctx->launches += 1;
+    return U1U1_OK;
+}
+
+extern "C" int u1u1_export_slab(u1u1_ctx *ctx, void *dst_dev)
+{
+    if (!ctx || !dst_dev) return ctx ? fail(ctx, U1U1_EINVAL, "dst is NULL") : U1U1_EINVAL;
+    if (!ctx->nz_own) return fail(ctx, U1U1_ESTATE, "export_slab needs u1u1_configure_slab first");
+    return slab_relayout(ctx, (float *)dst_dev, 1);
+}
+
+extern "C" int u1u1_import_slab(u1u1_ctx *ctx, const void *src_dev)
+{
+    if (!ctx || !src_dev) return ctx ? fail(ctx, U1U1_EINVAL, "src is NULL") : U1U1_EINVAL;
+    if (!ctx->nz_own) return fail(ctx, U1U1_ESTATE, "import_slab needs u1u1_configure_slab first");
+    return slab_relayout(ctx, (float *)src_dev, 0);
+}
+
+// my boundary planes of the CURRENT positions -> the neighbours' halo planes (needed once, after init / import: from
+// then on every step writes them itself).  Three contiguous chunks per plane (packs A, B, C).
+extern "C" int u1u1_push_halos(u1u1_ctx *ctx)
+{
+    if (!ctx) return U1U1_EINVAL;
+    if (!ctx->nz_own || !ctx->peer_up || !ctx->peer_dn) return fail(ctx, U1U1_ESTATE, "push_halos needs u1u1_configure_slab and u1u1_set_slab_peers first");
+    const size_t NN = (size_t)ctx->N * ctx->N, V = ctx->V, off = (size_t)ctx->cur * NPOS * V;
+    const float *mine = pos_buf(ctx, ctx->cur);
+    float *up = ctx->peer_up + off, *dn = ctx->peer_dn + off;
+    const size_t top = (size_t)ctx->nz_own, bot = 1, up_halo = 0, dn_halo = (size_t)ctx->nz_own + 1;
+    cudaError_t e = cudaSuccess;
+    for (int pack = 0; pack < 3 && e == cudaSuccess; pack++) {
+        const size_t base = pack == 0 ? 0 : pack == 1 ? 4 * V : 8 * V, w = pack == 2 ? 2 : 4;     // floats per site
+        e = cudaMemcpyAsync(up + base + w * NN * up_halo, mine + base + w * NN * top, w * NN * sizeof(float), cudaMemcpyDeviceToDevice, ctx->stream);
+        if (e == cudaSuccess)
+            e = cudaMemcpyAsync(dn + base + w * NN * dn_halo, mine + base + w * NN * bot, w * NN * sizeof(float), cudaMemcpyDeviceToDevice, ctx->stream);
+    }
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "push_halos");
     return U1U1_OK;
 }

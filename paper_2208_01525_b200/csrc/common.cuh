@@ -25,8 +25,18 @@ struct Lattice {
     const float *pos_in;  // positions at tau (read)
     float *pos_out;       // positions at tau + dtau (written)
     float *mom;           // momenta, updated in place
-    size_t V;             // N^3
+    size_t V;             // sites in one buffer: N^3, or N * N * (nz_own + 2) for a z slab
     int N;
+    // z slab of a lattice that is split over several GPUs (zero for the ordinary cubic lattice):
+    // the buffers hold planes 0 .. nz_own + 1, plane 0 and plane nz_own + 1 being copies of the neighbouring slabs'
+    // boundary planes.  The step kernel updates planes 1 .. nz_own and ALSO stores its top / bottom plane of pos_out
+    // into the halo plane of the neighbour above / below (plain stores through peer memory: NVLink when the neighbour
+    // lives on another GPU), so the exchange rides on the kernel's own output pass.
+    int nz_own;           // 0: cubic lattice, periodic in z inside the buffer
+    float *peer_up_out;   // pos_out buffer of the slab above (its plane 0 receives this slab's top plane)
+    float *peer_dn_out;   // pos_out buffer of the slab below (its plane nz_own_dn + 1 receives this slab's bottom plane)
+    size_t peer_dn_plane; // nz_own_dn + 1
+    size_t peer_up_V, peer_dn_V;   // sites in the neighbours' buffers (their pack offsets)
 };
 
 // float offset of logical component c (0..9) of site lin inside a 10 V-float buffer

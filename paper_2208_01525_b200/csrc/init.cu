@@ -26,10 +26,13 @@ __device__ inline void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint
 
 // init_kind 0: unit-modulus scalars with iid uniform phases 2 pi r / 2^32 (r[0] -> phi, r[1] -> psi).
 // Phases are evaluated in fp64 and rounded once, so the result is the fp32 rounding of the exact value.
-__global__ void init_random_phase_kernel(float *pos, size_t V, uint64_t seed, double eta1, double eta2)
+// `pos` holds `n_own` sites starting at buffer site `lin_off` (0 / all of them for the cubic lattice; one plane in / the
+// own planes for a z slab), whose GLOBAL site indices -- the Philox counters -- start at `gidx_off`.
+__global__ void init_random_phase_kernel(float *pos, size_t n_own, size_t lin_off, size_t gidx_off, uint64_t seed, double eta1,
+                                         double eta2)
 {
-    for (size_t lin = (size_t)blockIdx.x * blockDim.x + threadIdx.x; lin < V;
-         lin += (size_t)gridDim.x * blockDim.x) {
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_own; i += (size_t)gridDim.x * blockDim.x) {
+        const size_t lin = i + gidx_off;
         uint32_t r[4];
         philox4x32_10((uint32_t)lin, (uint32_t)(lin >> 32), 0u, 0u, (uint32_t)seed, (uint32_t)(seed >> 32), r);
         double sn, cs;
@@ -40,7 +43,7 @@ __global__ void init_random_phase_kernel(float *pos, size_t V, uint64_t seed, do
         sincospi(2.0 * ((double)r[1] * (1.0 / 4294967296.0)), &sn, &cs);
         a.z = (float)(eta2 * cs);
         a.w = (float)(eta2 * sn);
-        reinterpret_cast<float4 *>(pos)[lin] = a;           // pack A
+        reinterpret_cast<float4 *>(pos)[i + lin_off] = a;           // pack A
     }
 }
 
@@ -109,13 +112,14 @@ __global__ void normalise_kernel(const double *src, float *pos, size_t V, double
 
 // canonical [20][V] (component planes) <-> internal packed vectors.  ncomp canonical components
 // starting at c0 are moved; `canon` points at component c0's plane.
-__global__ void relayout_kernel(float *pos, float *mom, float *canon, size_t V, int c0, int ncomp,
+__global__ void relayout_kernel(float *pos, float *mom, float *canon, size_t V, size_t n_own, size_t lin_off, int c0, int ncomp,
                                 int to_canonical)
 {
-    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < (size_t)ncomp * V;
+    // n_own canonical sites per component, stored from buffer site lin_off on; V = sites in the buffer (pack offsets)
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < (size_t)ncomp * n_own;
          i += (size_t)gridDim.x * blockDim.x) {
-        const int c = c0 + (int)(i / V);
-        const size_t lin = i % V;
+        const int c = c0 + (int)(i / n_own);
+        const size_t lin = i % n_own + lin_off;
         int is_mom, comp;
         canonical_to_internal(c, is_mom, comp);
         float *internal = (is_mom ? mom : pos) + comp_off(comp, lin, V);
@@ -161,10 +165,10 @@ constexpr int GRID = RED_MAX_BLOCKS;      // grid-stride kernels: a few blocks p
 
 }  // namespace
 
-cudaError_t launch_init_random_phase(float *pos, size_t V, uint64_t seed, double eta1, double eta2,
-                                     cudaStream_t st)
+cudaError_t launch_init_random_phase(float *pos, size_t n_own, size_t lin_off, size_t gidx_off, uint64_t seed, double eta1,
+                                     double eta2, cudaStream_t st)
 {
-    init_random_phase_kernel<<<GRID, 256, 0, st>>>(pos, V, seed, eta1, eta2);
+    init_random_phase_kernel<<<GRID, 256, 0, st>>>(pos, n_own, lin_off, gidx_off, seed, eta1, eta2);
     return cudaGetLastError();
 }
 
@@ -197,10 +201,10 @@ cudaError_t launch_import_tiled(float *pos, float *mom, const float *canon, size
     return cudaGetLastError();
 }
 
-cudaError_t launch_relayout(float *pos, float *mom, float *canon, size_t V, int c0, int ncomp, int to_canonical,
-                            cudaStream_t st)
+cudaError_t launch_relayout(float *pos, float *mom, float *canon, size_t V, size_t n_own, size_t lin_off, int c0, int ncomp,
+                            int to_canonical, cudaStream_t st)
 {
-    relayout_kernel<<<GRID, 256, 0, st>>>(pos, mom, canon, V, c0, ncomp, to_canonical);
+    relayout_kernel<<<GRID, 256, 0, st>>>(pos, mom, canon, V, n_own, lin_off, c0, ncomp, to_canonical);
     return cudaGetLastError();
 }
 

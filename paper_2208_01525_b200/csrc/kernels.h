@@ -52,14 +52,14 @@ cudaError_t launch_segments(const uint8_t *cells, size_t V, int N, int tolerant,
                             double *partials, double *result, cudaStream_t st);
 
 // init.cu
-cudaError_t launch_init_random_phase(float *pos, size_t V, uint64_t seed, double eta1, double eta2,
-                                     cudaStream_t st);
+cudaError_t launch_init_random_phase(float *pos, size_t n_own, size_t lin_off, size_t gidx_off, uint64_t seed, double eta1,
+                                     double eta2, cudaStream_t st);
 cudaError_t launch_init_smoothed(float *pos, double *tmp_a, double *tmp_b, size_t V, int N, uint64_t seed,
                                  double width, int trunc, double eta1, double eta2, cudaStream_t st);
 cudaError_t launch_export_block(const float *pos, const float *mom, size_t V, int N, int x0, int y0, int z0,
                                 int bx, int by, int bz, float *dst, cudaStream_t st);
 cudaError_t launch_import_tiled(float *pos, float *mom, const float *canon, size_t V, int N, int n, cudaStream_t st);
-cudaError_t launch_relayout(float *pos, float *mom, float *canon, size_t V, int c0, int ncomp, int to_canonical,
-                            cudaStream_t st);
+cudaError_t launch_relayout(float *pos, float *mom, float *canon, size_t V, size_t n_own, size_t lin_off, int c0, int ncomp,
+                            int to_canonical, cudaStream_t st);
 
 }  // namespace u1u1

@@ -44,8 +44,8 @@ struct alignas(64) DiagMaps {
 };
 
 // host (tma_maps.cu): false if cuTensorMapEncodeTiled is unavailable or rejects the layout
-bool encode_halo_maps(PackMaps *m, const float *buf, size_t V, int N);
-bool encode_tile_maps(PackMaps *m, const float *buf, size_t V, int N);
+bool encode_halo_maps(PackMaps *m, const float *buf, size_t V, int N, int NZ);
+bool encode_tile_maps(PackMaps *m, const float *buf, size_t V, int N, int NZ);
 
 #ifdef __CUDACC__
 __device__ inline unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }

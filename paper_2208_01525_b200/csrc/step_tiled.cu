@@ -73,7 +73,9 @@ __device__ inline void set2(float2 &v, int i, float a) { if (i == 0) v.x = a; el
 // evaluated without cancellation; the Laplacian is their plain sum and the current is Im(f* d_i).  Rounding
 // errors then scale with |D f| dx instead of |f|, which brings the fp32 chain's Gauss residual close to the
 // storage floor wherever the fields are smooth.
-template <bool FAST, typename R, bool DIFF>
+// SLAB: the buffers hold a z slab with one halo plane on either side (common.cuh); no periodic wrap in z, and the
+// slab's top / bottom output planes are also stored into the neighbouring slabs' halo planes.
+template <bool FAST, typename R, bool DIFF, bool SLAB>
 __global__ void __launch_bounds__(NTHREADS, sizeof(R) == 8 ? 2 : 3)
 step_tiled_kernel(Lattice L, StepCoef k, int zchunk, int band, const __grid_constant__ StepMaps maps)
 {
@@ -85,11 +87,12 @@ step_tiled_kernel(Lattice L, StepCoef k, int zchunk, int band, const __grid_cons
     // 1-d grid, launch order = (tile x fastest, tile row within a band of `band` rows, z chunk, band): the CTAs that
     // are resident together cover one band of tile rows of one z chunk, and the next wave continues with the NEXT
     // chunk of the same band, whose two boundary planes the previous wave has just read
-    const int ntx = (N + TX - 1) / TX, nty = (N + TY - 1) / TY, nzc = (N + zchunk - 1) / zchunk;
+    const int NZO = SLAB ? L.nz_own : N, ZB = SLAB ? 1 : 0;     // own planes and the buffer index of the first of them
+    const int ntx = (N + TX - 1) / TX, nty = (N + TY - 1) / TY, nzc = (NZO + zchunk - 1) / zchunk;
     const int full = ntx * band * nzc, bnd = blockIdx.x / full, rem = blockIdx.x - bnd * full;
     const int rows = min(band, nty - bnd * band), bzc = rem / (ntx * rows), tl = rem - bzc * (ntx * rows);
-    const int x0 = (tl % ntx) * TX, y0 = (bnd * band + tl / ntx) * TY, z0 = bzc * zchunk;
-    const int wx = min(TX, N - x0), wy = min(TY, N - y0), nz = min(zchunk, N - z0);
+    const int x0 = (tl % ntx) * TX, y0 = (bnd * band + tl / ntx) * TY, z0 = ZB + bzc * zchunk;
+    const int wx = min(TX, N - x0), wy = min(TY, N - y0), nz = min(zchunk, ZB + NZO - z0);
     const bool active = tx < wx && ty < wy;
     // TMA boxes cannot wrap: only tiles whose halo lies inside the lattice take the TMA path (CTA-uniform)
     const bool tma = !(k.flags & 2) && tile_is_interior(x0, y0, N);
@@ -102,12 +105,12 @@ step_tiled_kernel(Lattice L, StepCoef k, int zchunk, int band, const __grid_cons
     CpPlan plan;                  // cp.async path: this thread's copies of one halo plane
     if (!tma) make_cp_plan(plan, tid, x0, y0, wx, wy, N);
     auto stage_cp = [&](int j) {          // every thread; caller commits the group
-        stage_plane_cp(plan, tid, pos, V, (size_t)wrapi(z0 + j, N) * NN, sbase + ((j + 1) & 3) * SLOT_BYTES);
+        stage_plane_cp(plan, tid, pos, V, (size_t)(SLAB ? z0 + j : wrapi(z0 + j, N)) * NN, sbase + ((j + 1) & 3) * SLOT_BYTES);
     };
     auto stage_tma = [&](int j) {         // one thread
         // evict-last: the neighbouring tiles re-read these lines as halo within a few planes (measured: -1 % DRAM reads)
-        stage_plane_tma(maps.pos, x0, y0, wrapi(z0 + j, N), sbase + ((j + 1) & 3) * SLOT_BYTES, bars + 8 * ((j + 1) & 3),
-                        pol_keep);
+        stage_plane_tma(maps.pos, x0, y0, SLAB ? z0 + j : wrapi(z0 + j, N), sbase + ((j + 1) & 3) * SLOT_BYTES,
+                        bars + 8 * ((j + 1) & 3), pol_keep);
     };
     auto stage_mom_tma = [&](int m) {     // one thread; momenta of relative plane m into ring slot m & 1
         const unsigned slot = sbase + OFF_MRING + (m & 1) * MSLOT_BYTES, bar = bars + 8 * (4 + (m & 1));
@@ -339,6 +342,20 @@ step_tiled_kernel(Lattice L, StepCoef k, int zchunk, int band, const __grid_cons
         __stcs(reinterpret_cast<float4 *>(L.pos_out) + lin, OA);
         __stcs(reinterpret_cast<float4 *>(L.pos_out + 4 * V) + lin, OB);
         __stcs(reinterpret_cast<float2 *>(L.pos_out + 8 * V) + lin, OC);
+        if (SLAB) {                     // the exchange: boundary planes go straight into the neighbours' halo planes
+            if (z0 + iz == L.nz_own) {
+                const size_t pl = gsite, PV = L.peer_up_V;          // plane 0 of the slab above
+                reinterpret_cast<float4 *>(L.peer_up_out)[pl] = OA;
+                reinterpret_cast<float4 *>(L.peer_up_out + 4 * PV)[pl] = OB;
+                reinterpret_cast<float2 *>(L.peer_up_out + 8 * PV)[pl] = OC;
+            }
+            if (z0 + iz == 1) {
+                const size_t pl = L.peer_dn_plane * NN + gsite, PV = L.peer_dn_V;
+                reinterpret_cast<float4 *>(L.peer_dn_out)[pl] = OA;
+                reinterpret_cast<float4 *>(L.peer_dn_out + 4 * PV)[pl] = OB;
+                reinterpret_cast<float2 *>(L.peer_dn_out + 8 * PV)[pl] = OC;
+            }
+        }
     }
     if (!tma) cp_async_wait<0>();
 }
@@ -356,11 +373,11 @@ int pick_zchunk(int N, int sms)
     return zc < N ? zc : N;
 }
 
-template <bool FAST, typename R, bool DIFF>
+template <bool FAST, typename R, bool DIFF, bool SLAB = false>
 cudaError_t launch_one(const Lattice &L, StepCoef k, cudaStream_t st, const StepMaps *m, int sms)
 {
     // per device and cheap: set on every launch rather than caching a per-process flag
-    cudaError_t ea = cudaFuncSetAttribute(step_tiled_kernel<FAST, R, DIFF>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+    cudaError_t ea = cudaFuncSetAttribute(step_tiled_kernel<FAST, R, DIFF, SLAB>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
     if (ea != cudaSuccess) return ea;
     StepMaps maps;
     if (!m) {
@@ -370,13 +387,14 @@ cudaError_t launch_one(const Lattice &L, StepCoef k, cudaStream_t st, const Step
         maps = *m;
     }
     const int zc = pick_zchunk(L.N, sms);
-    const int ntx = (L.N + TX - 1) / TX, nty = (L.N + TY - 1) / TY, nzc = (L.N + zc - 1) / zc;
+    const int nzo = SLAB ? L.nz_own : L.N;
+    const int ntx = (L.N + TX - 1) / TX, nty = (L.N + TY - 1) / TY, nzc = (nzo + zc - 1) / zc;
     // band height = the tile rows one wave of resident CTAs covers (SMs x CTAs per SM / tiles per row)
     const int per_sm = sizeof(R) == 8 ? 2 : 3;
     int band = (k.flags & 8) ? nty : (sms * per_sm + ntx - 1) / ntx;     // tuning flag 8: the order of a plain 3-d grid
     if (band > nty) band = nty;
     const unsigned grid = (unsigned)ntx * nty * nzc;
-    step_tiled_kernel<FAST, R, DIFF><<<grid, NTHREADS, SMEM_BYTES, st>>>(L, k, zc, band, maps);
+    step_tiled_kernel<FAST, R, DIFF, SLAB><<<grid, NTHREADS, SMEM_BYTES, st>>>(L, k, zc, band, maps);
     return cudaGetLastError();
 }
 
@@ -388,6 +406,7 @@ bool step_tiled_supports(int N) { return N >= 8 && (N % 4) == 0; }
 // maps: tensor maps of (L.pos_in, L.mom), or NULL for lattices too small for any interior tile; sms = SM count
 cudaError_t launch_step_tiled(const Lattice &L, const StepCoef &k, cudaStream_t st, int mode, const StepMaps *maps, int sms)
 {
+    if (L.nz_own) return mode == 5 ? launch_one<true, float, true, true>(L, k, st, maps, sms) : cudaErrorNotSupported;
     switch (mode) {
         case 0: return launch_one<false, double, false>(L, k, st, maps, sms);
         case 1: return launch_one<true, double, false>(L, k, st, maps, sms);

@@ -31,12 +31,12 @@ EncodeTiledFn encode_fn()
 // must be 16-byte aligned, i.e. (W x) a multiple of 4 floats: any x for W = 4, even x for W = 2.
 // (Measured dead ends: a 4-d (component, x, y, z) map makes TMA issue 16-byte requests, 25 % slower; 8-byte element
 // types and unaligned origins raise `illegal instruction` on sm_100a.)
-bool encode_pack(CUtensorMap *m, const float *base, int W, int N, int bx, int by)
+bool encode_pack(CUtensorMap *m, const float *base, int W, int N, int NZ, int bx, int by)
 {
     EncodeTiledFn fn = encode_fn();
     if (!fn) return false;
     const cuuint64_t n = (cuuint64_t)N, w = (cuuint64_t)W;
-    const cuuint64_t dims[3] = {w * n, n, n}, strides[2] = {4 * w * n, 4 * w * n * n};
+    const cuuint64_t dims[3] = {w * n, n, (cuuint64_t)NZ}, strides[2] = {4 * w * n, 4 * w * n * n};
     const cuuint32_t box[3] = {(cuuint32_t)(W * bx), (cuuint32_t)by, 1}, es[3] = {1, 1, 1};
     return fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, (void *)base, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
@@ -44,16 +44,17 @@ bool encode_pack(CUtensorMap *m, const float *base, int W, int N, int bx, int by
 
 }  // namespace
 
-bool encode_halo_maps(PackMaps *m, const float *buf, size_t V, int N)
+// NZ = planes in the buffer (N for the cubic lattice, nz_own + 2 for a z slab); V = N * N * NZ
+bool encode_halo_maps(PackMaps *m, const float *buf, size_t V, int N, int NZ)
 {
-    return encode_pack(&m->A, buf, 4, N, COLS, ROWS) && encode_pack(&m->B, buf + 4 * V, 4, N, COLS, ROWS) &&
-           encode_pack(&m->C, buf + 8 * V, 2, N, CCOLS, ROWS);
+    return encode_pack(&m->A, buf, 4, N, NZ, COLS, ROWS) && encode_pack(&m->B, buf + 4 * V, 4, N, NZ, COLS, ROWS) &&
+           encode_pack(&m->C, buf + 8 * V, 2, N, NZ, CCOLS, ROWS);
 }
 
-bool encode_tile_maps(PackMaps *m, const float *buf, size_t V, int N)
+bool encode_tile_maps(PackMaps *m, const float *buf, size_t V, int N, int NZ)
 {
-    return encode_pack(&m->A, buf, 4, N, TX, TY) && encode_pack(&m->B, buf + 4 * V, 4, N, TX, TY) &&
-           encode_pack(&m->C, buf + 8 * V, 2, N, TX, TY);
+    return encode_pack(&m->A, buf, 4, N, NZ, TX, TY) && encode_pack(&m->B, buf + 4 * V, 4, N, NZ, TX, TY) &&
+           encode_pack(&m->C, buf + 8 * V, 2, N, NZ, TX, TY);
 }
 
 }  // namespace u1u1

@@ -135,3 +135,61 @@ class Lattice:
 
     def launch_count(self) -> int:
         return int(self.lib.u1u1_launch_count(self._ctx))
+
+
+class Slab:
+    """One z slab of a lattice split over several GPUs (include/u1u1.h, "z slabs"): owns the slab's state buffer and a
+    context; the methods are the slab calls of the C ABI.  Argument marshalling only."""
+
+    def __init__(self, N: int, nz_own: int, z_first: int, device: str = "cuda:0", stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise B.U1U1Error("CUDA device required: libu1u1 has no CPU fallback")
+        self._torch = torch
+        self.lib = B.load()
+        self.N, self.nz_own, self.z_first = int(N), int(nz_own), int(z_first)
+        self.device = torch.device(device)
+        sb = self.lib.u1u1_slab_state_bytes(self.N, self.nz_own)
+        if sb == 0:
+            raise B.U1U1Error(f"unsupported slab N={N}, nz_own={nz_own}")
+        with torch.cuda.device(self.device):
+            self.state = torch.zeros(sb, dtype=torch.uint8, device=self.device)
+            self.scratch = torch.empty(1 << 20, dtype=torch.uint8, device=self.device)
+            self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        self._ctx = ctypes.c_void_p()
+        rc = self.lib.u1u1_create(ctypes.byref(self._ctx), self.state.data_ptr(), sb, self.scratch.data_ptr(),
+                                  self.scratch.numel(), self.stream.cuda_stream)
+        if rc:
+            raise B.U1U1Error(f"u1u1_create: {self.lib.u1u1_last_error(None).decode()}")
+
+    _check = Lattice._check
+    close = Lattice.close
+    __del__ = Lattice.__del__
+    set_params = Lattice.set_params
+    step = Lattice.step
+    launch_count = Lattice.launch_count
+
+    def configure_slab(self, dx: float, params: B.Params):
+        self._check(self.lib.u1u1_configure_slab(self._ctx, self.N, self.nz_own, self.z_first, dx, ctypes.byref(params)),
+                    "configure_slab")
+
+    def set_slab_peers(self, up_state_ptr: int, dn_state_ptr: int):
+        self._check(self.lib.u1u1_set_slab_peers(self._ctx, up_state_ptr, dn_state_ptr), "set_slab_peers")
+
+    def init_slab(self, seed: int):
+        self._check(self.lib.u1u1_init_slab(self._ctx, seed), "init_slab")
+
+    def push_halos(self):
+        self._check(self.lib.u1u1_push_halos(self._ctx), "push_halos")
+
+    def export_slab(self):
+        t = self._torch.empty((20, self.nz_own, self.N, self.N), dtype=self._torch.float32, device=self.device)
+        self._check(self.lib.u1u1_export_slab(self._ctx, t.data_ptr()), "export_slab")
+        return t
+
+    def import_slab(self, t):
+        torch = self._torch
+        t = t.to(device=self.device, dtype=torch.float32).contiguous()
+        assert tuple(t.shape) == (20, self.nz_own, self.N, self.N), t.shape
+        self._check(self.lib.u1u1_import_slab(self._ctx, t.data_ptr()), "import_slab")
+        self.stream.synchronize()
