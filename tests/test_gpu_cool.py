@@ -66,3 +66,21 @@ def test_paper_ic_pipeline_matches_oracle():
     assert np.allclose(g, O.gauss_violation(gpu, DX, K, cG), rtol=1e-4)
     with pytest.raises(U1U1Error, match="EUNSTABLE"):
         lat.cool(1, 0.05)                                          # 0.05 * (48 + 2) >= 2
+
+
+def test_cooling_guard_and_weights():
+    """The explicit-diffusion guard covers the links (12/dx^2 + 2 e^2 sigma^2) as well as the scalars, and a cooling call
+    resets the diagnostic weights to a = 1 (the cooling equations carry no scale factor)."""
+    from paper_2208_01525_b200 import Lattice, Params, U1U1Error
+    lat = Lattice(16)
+    lat.init_fields(2, DX, Params(tau_norm=1.0))
+    lat.step(2, 3.0, 0.5, 1.0)
+    assert lat.diagnostics()["c"] > 9.0                            # c = a^2 of the last step
+    lat.cool(2, DCOOL)
+    d = lat.diagnostics()
+    assert d["c"] == 1.0 and d["a"] == 1.0 and d["sum_kin"] == 0.0
+    strong = Lattice(16)
+    strong.init_fields(2, DX, Params(lambda1=0.5, lambda2=0.5, e1=2.0, e2=2.0, kappa=0.1))   # 2 e^2 = 8 > lambda
+    with pytest.raises(U1U1Error, match="EUNSTABLE"):
+        strong.cool(1, 0.036)                                      # 0.036 * (48 + 0.5) < 2 <= 0.036 * (48 + 8)
+    strong.cool(1, 0.035)

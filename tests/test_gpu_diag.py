@@ -136,6 +136,29 @@ def test_fused_sweep_staging_paths_bit_identical():
     assert outs[0][0]["sumW_p"] > 0 and outs[0][0]["cells_pq"] > 0
 
 
+def test_diagnostics_fail_loudly_beyond_the_range_of_the_winding_sweep():
+    """The wrap counts of the winding sweep live in byte lanes (|n| <= 31): a link phase beyond |theta| = 180 must be
+    reported as an error, not as a wrong winding (reading R-9: the links are non-compact and may drift)."""
+    from paper_2208_01525_b200 import Lattice, Params, U1U1Error
+    import torch
+    N = 16
+    s0 = np.zeros((20, N, N, N), dtype=np.float32)
+    s0[0], s0[4] = 1.0, 1.0
+    s0[9, 3, 4, 5] = 150.0
+    lat = Lattice(N)
+    lat.configure(DX, Params())
+    lat.import_state(torch.from_numpy(s0))
+    d = lat.diagnostics()
+    # one link of 150 rad on the vacuum puts a flux of 150 = 23.87 x 2 pi through its four plaquettes: |W| = 24 on each
+    assert d["max_theta"] == 150.0 and d["sumW_p"] == 4 * 24 and d["maxW"] == 24 and d["sumW_q"] == 0
+    ref = O.diagnostics(s0.astype(np.float64), DX, O.Couplings(), 1.0)
+    assert ref["sumW_p"] == 96 and ref["maxW_p"] == 24
+    s0[15, 7, 7, 7] = -200.0
+    lat.import_state(torch.from_numpy(s0))
+    with pytest.raises(U1U1Error, match="ESTATE"):
+        lat.diagnostics()
+
+
 def test_windings_with_exactly_zero_sites():
     """Reading R-15: atan2(0, 0) = 0, i.e. a link with an end point where the field is exactly zero has chi = 0 in the
     printed formula.  Zero sites sprinkled over a state with strings (vortex cores put exactly ON lattice sites do
