@@ -44,7 +44,7 @@ struct alignas(64) DiagMaps {
 };
 
 // host (tma_maps.cu): false if cuTensorMapEncodeTiled is unavailable or rejects the layout
-bool encode_halo_maps(PackMaps *m, const float *buf, size_t V, int N, int NZ);
+bool encode_halo_maps(PackMaps *m, const float *buf, size_t V, int N, int NZ, int rows = ROWS);
 bool encode_tile_maps(PackMaps *m, const float *buf, size_t V, int N, int NZ);
 
 #ifdef __CUDACC__

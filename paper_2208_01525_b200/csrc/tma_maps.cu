@@ -45,10 +45,11 @@ bool encode_pack(CUtensorMap *m, const float *base, int W, int N, int NZ, int bx
 }  // namespace
 
 // NZ = planes in the buffer (N for the cubic lattice, nz_own + 2 for a z slab); V = N * N * NZ
-bool encode_halo_maps(PackMaps *m, const float *buf, size_t V, int N, int NZ)
+// rows = box height (ROWS = the 8-row tiles + halo)
+bool encode_halo_maps(PackMaps *m, const float *buf, size_t V, int N, int NZ, int rows)
 {
-    return encode_pack(&m->A, buf, 4, N, NZ, COLS, ROWS) && encode_pack(&m->B, buf + 4 * V, 4, N, NZ, COLS, ROWS) &&
-           encode_pack(&m->C, buf + 8 * V, 2, N, NZ, CCOLS, ROWS);
+    return encode_pack(&m->A, buf, 4, N, NZ, COLS, rows) && encode_pack(&m->B, buf + 4 * V, 4, N, NZ, COLS, rows) &&
+           encode_pack(&m->C, buf + 8 * V, 2, N, NZ, CCOLS, rows);
 }
 
 bool encode_tile_maps(PackMaps *m, const float *buf, size_t V, int N, int NZ)
