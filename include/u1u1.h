@@ -190,7 +190,7 @@ int u1u1_export_labels(u1u1_ctx *ctx, void *labels_dev);
  * lives on another GPU), so there is no separate exchange pass.  Between two steps the caller must make sure that every
  * rank has finished the previous one (stream-ordered barrier / torch.distributed).  All slabs must have the same nz_own.
  * Available on a slab: set_params, step (n = 1, kernel_variant 0), init_slab, import_slab / export_slab, push_halos,
- * launch_count; the diagnostics calls need a cubic lattice (U1U1_ESTATE). */
+ * launch_count and the slab diagnostics below; the other diagnostics calls need a cubic lattice (U1U1_ESTATE). */
 size_t u1u1_slab_state_bytes(int32_t N, int32_t nz_own);
 int u1u1_configure_slab(u1u1_ctx *ctx, int32_t N, int32_t nz_own, int64_t z_first, double dx, const u1u1_params *params);
 /* DEVICE pointers to the STATE buffers (as given to u1u1_create) of the slabs above and below (periodic: the top
@@ -205,6 +205,19 @@ int u1u1_import_slab(u1u1_ctx *ctx, const void *src_dev);
 /* Copy this slab's boundary planes of the current positions into the neighbours' halo planes (once, after init_slab /
  * import_slab on every rank; afterwards every step does it itself). */
 int u1u1_push_halos(u1u1_ctx *ctx);
+
+/* Diagnostics of a lattice in z slabs.  (1) every rank: u1u1_push_diag_halos (its top plane of E_z, H_z goes into the
+ * momentum halo plane of the slab above: div E of the first own plane needs it), then a barrier; (2) every rank:
+ * u1u1_slab_diagnostics_partial fills raw_host[U1U1_SLAB_NRAW] with the fused sweep's raw results over its own planes
+ * (scratch must hold u1u1_slab_scratch_bytes); (3) the ranks reduce: SUM over the first U1U1_SLAB_NSUM values, MAX over
+ * the rest; (4) u1u1_slab_diagnostics_finish turns the reduced array into the u1u1_diagnostics output for the lattice of
+ * nz_global planes (the one-cell-tolerance counts, which would need cell-array halos, are NaN). */
+#define U1U1_SLAB_NRAW 28
+#define U1U1_SLAB_NSUM 24
+size_t u1u1_slab_scratch_bytes(int32_t N, int32_t nz_own);
+int u1u1_push_diag_halos(u1u1_ctx *ctx);
+int u1u1_slab_diagnostics_partial(u1u1_ctx *ctx, double *raw_host);
+int u1u1_slab_diagnostics_finish(u1u1_ctx *ctx, const double *raw_reduced_host, int64_t nz_global, double *out_host);
 
 /* Number of kernel launches issued by this context so far (for bench.py's gpu_launches). */
 uint64_t u1u1_launch_count(const u1u1_ctx *ctx);

@@ -53,7 +53,9 @@ SYMBOLS = ["u1u1_state_bytes", "u1u1_scratch_bytes", "u1u1_create", "u1u1_destro
            "u1u1_diagnostics", "u1u1_gauss_violation", "u1u1_export_state", "u1u1_import_state",
            "u1u1_export_state_host", "u1u1_import_state_host", "u1u1_export_windings", "u1u1_export_block", "u1u1_launch_count", "u1u1_pq_segments", "u1u1_export_labels", "u1u1_import_state_tiled",
            "u1u1_slab_state_bytes", "u1u1_configure_slab", "u1u1_set_slab_peers", "u1u1_init_slab", "u1u1_export_slab",
-           "u1u1_import_slab", "u1u1_push_halos"]
+           "u1u1_import_slab", "u1u1_push_halos", "u1u1_slab_scratch_bytes", "u1u1_push_diag_halos",
+           "u1u1_slab_diagnostics_partial", "u1u1_slab_diagnostics_finish"]
+SLAB_NRAW, SLAB_NSUM = 28, 24
 
 
 def load():
@@ -97,6 +99,10 @@ def load():
     L.u1u1_export_slab.argtypes = [vp, vp]
     L.u1u1_import_slab.argtypes = [vp, vp]
     L.u1u1_push_halos.argtypes = [vp]
+    L.u1u1_slab_scratch_bytes.argtypes = [i32, i32]; L.u1u1_slab_scratch_bytes.restype = ctypes.c_size_t
+    L.u1u1_push_diag_halos.argtypes = [vp]
+    L.u1u1_slab_diagnostics_partial.argtypes = [vp, dp]
+    L.u1u1_slab_diagnostics_finish.argtypes = [vp, dp, ctypes.c_int64, dp]
     _lib = L
     return L
 

@@ -421,6 +421,7 @@ static FusedCoef fused_coef(const u1u1_ctx *ctx)
     k.c = (float)ctx->c;
     k.inv_c = (float)(1.0 / ctx->c);
     k.flags = P.kernel_variant >> 4;
+    k.nz_own = ctx->nz_own;
     return k;
 }
 
@@ -483,22 +484,11 @@ static int run_sweep(u1u1_ctx *ctx, bool with_codes)
     return U1U1_OK;
 }
 
-extern "C" int u1u1_diagnostics(u1u1_ctx *ctx, double *out)
+// out slots from the raw sums r[0 .. FUSED_NRES) of the sweep and the tolerant counts r[32], r[33] over `sites` sites
+static void derive_diagnostics(const u1u1_ctx *ctx, const double *r, double sites, double *out)
 {
-    if (!ctx || !out) return ctx ? fail(ctx, U1U1_EINVAL, "out is NULL") : U1U1_EINVAL;
-    if (!ctx->configured) return fail(ctx, U1U1_ESTATE, "diagnostics before configure/init_fields");
-    if (int rc = cubic_only(ctx, "diagnostics")) return rc;
-    const size_t V = ctx->V;
-    if (int rc = run_sweep(ctx, false)) return rc;
-    double r[34];
-    if (int rc = fetch(ctx, r, 34)) return rc;
-    // the byte lanes of the winding sweep hold wrap counts |n| <= 31: fail loudly beyond (non-compact links, reading R-9)
-    if (r[FR_MAXTH] > 180.0) {
-        ctx->diag_valid = false;
-        return fail(ctx, U1U1_ESTATE, "diagnostics: a link phase exceeds |theta| = 180, beyond the range of the winding sweep");
-    }
     memset(out, 0, U1U1_DIAG_LEN * sizeof(double));
-    const double dx = ctx->dx, vol = (double)V * dx * dx * dx;
+    const double dx = ctx->dx, vol = sites * dx * dx * dx;
     out[U1U1_D_TAU] = ctx->tau_pos;
     out[U1U1_D_A] = ctx->a;
     out[U1U1_D_C] = ctx->c;
@@ -536,6 +526,22 @@ extern "C" int u1u1_diagnostics(u1u1_ctx *ctx, double *out)
     out[U1U1_D_L_PQ_TOL] = 0.5 * dx * (r[32] + r[33]);
     out[U1U1_D_MAX_THETA] = r[FR_MAXTH];
     gauss_norms(r + FR_GAUSS, r + FR_GMAX, out + U1U1_D_GAUSS);
+}
+
+extern "C" int u1u1_diagnostics(u1u1_ctx *ctx, double *out)
+{
+    if (!ctx || !out) return ctx ? fail(ctx, U1U1_EINVAL, "out is NULL") : U1U1_EINVAL;
+    if (!ctx->configured) return fail(ctx, U1U1_ESTATE, "diagnostics before configure/init_fields");
+    if (int rc = cubic_only(ctx, "diagnostics")) return rc;
+    if (int rc = run_sweep(ctx, false)) return rc;
+    double r[34];
+    if (int rc = fetch(ctx, r, 34)) return rc;
+    // the byte lanes of the winding sweep hold wrap counts |n| <= 31: fail loudly beyond (non-compact links, reading R-9)
+    if (r[FR_MAXTH] > 180.0) {
+        ctx->diag_valid = false;
+        return fail(ctx, U1U1_ESTATE, "diagnostics: a link phase exceeds |theta| = 180, beyond the range of the winding sweep");
+    }
+    derive_diagnostics(ctx, r, (double)ctx->V, out);
     return U1U1_OK;
 }
 
@@ -816,5 +822,66 @@ extern "C" int u1u1_push_halos(u1u1_ctx *ctx)
             e = cudaMemcpyAsync(dn + base + w * NN * dn_halo, mine + base + w * NN * bot, w * NN * sizeof(float), cudaMemcpyDeviceToDevice, ctx->stream);
     }
     if (e != cudaSuccess) return cuda_fail(ctx, e, "push_halos");
+    return U1U1_OK;
+}
+
+// Diagnostics of a lattice in z slabs: every rank sweeps its own planes (u1u1_slab_diagnostics_partial), the ranks add the
+// first U1U1_SLAB_NSUM raw values and take the maximum of the rest, and any rank turns the reduced array into the
+// u1u1_diagnostics output (u1u1_slab_diagnostics_finish).  Before the sweep the momentum pack C of the plane below must
+// be in place (u1u1_push_diag_halos on every rank, then a barrier); the positions' upper halo is there from the step.
+extern "C" int u1u1_push_diag_halos(u1u1_ctx *ctx)
+{
+    if (!ctx) return U1U1_EINVAL;
+    if (!ctx->nz_own || !ctx->peer_up || !ctx->peer_dn) return fail(ctx, U1U1_ESTATE, "push_diag_halos needs u1u1_configure_slab and u1u1_set_slab_peers first");
+    const size_t NN = (size_t)ctx->N * ctx->N, V = ctx->V, moff = (size_t)2 * NPOS * V + 8 * V;       // pack C of the momenta
+    // my top own plane of (E_z, H_z) -> plane 0 of the slab above
+    cudaError_t e = cudaMemcpyAsync(ctx->peer_up + moff, ctx->state + moff + 2 * NN * (size_t)ctx->nz_own, 2 * NN * sizeof(float),
+                                    cudaMemcpyDeviceToDevice, ctx->stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "push_diag_halos");
+    return U1U1_OK;
+}
+
+extern "C" size_t u1u1_slab_scratch_bytes(int32_t N, int32_t nz_own)
+{
+    if (!slab_ok(N, nz_own)) return 0;
+    const size_t Vb = (size_t)N * N * (size_t)(nz_own + 2);
+    return ((2 * Vb + 255) / 256) * 256 + ((size_t)RED_MAX_BLOCKS * RED_SLOTS + 64) * sizeof(double);
+}
+
+extern "C" int u1u1_slab_diagnostics_partial(u1u1_ctx *ctx, double *raw)
+{
+    if (!ctx || !raw) return ctx ? fail(ctx, U1U1_EINVAL, "raw is NULL") : U1U1_EINVAL;
+    if (!ctx->nz_own) return fail(ctx, U1U1_ESTATE, "slab_diagnostics_partial needs u1u1_configure_slab first");
+    if (ctx->scratch_bytes < u1u1_slab_scratch_bytes(ctx->N, ctx->nz_own)) return fail(ctx, U1U1_ESIZE, "scratch buffer smaller than u1u1_slab_scratch_bytes(N, nz_own)");
+    if (int rc = prepare_device(ctx)) return rc;
+    // slab scratch: [cells 2 V_buf] pad-> [partials][result]
+    double *part = (double *)(ctx->scratch + ((2 * ctx->V + 255) / 256) * 256), *res = part + (size_t)RED_MAX_BLOCKS * RED_SLOTS;
+    DiagMaps maps;
+    if (ctx->maps_ready) {
+        maps.pos = ctx->pos_halo[ctx->cur];
+        maps.mom = ctx->mom_halo;
+    }
+    int nb = 0;
+    cudaError_t e = launch_diag_fused(pos_buf(ctx, ctx->cur), mom_buf(ctx), ctx->V, ctx->N, fused_coef(ctx), ctx->scratch, nullptr, part,
+                                      &nb, ctx->maps_ready ? &maps : nullptr, ctx->sms, ctx->stream);
+    if (e == cudaSuccess) e = launch_fold(part, nb, FUSED_NRES, FUSED_NSUM, res, ctx->stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "slab diagnostics kernel launch");
+    ctx->launches += 2;
+    e = cudaMemcpyAsync(raw, res, FUSED_NRES * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "slab diagnostics readback");
+    return U1U1_OK;
+}
+
+extern "C" int u1u1_slab_diagnostics_finish(u1u1_ctx *ctx, const double *raw_reduced, int64_t nz_global, double *out)
+{
+    if (!ctx || !raw_reduced || !out) return ctx ? fail(ctx, U1U1_EINVAL, "NULL argument") : U1U1_EINVAL;
+    if (!ctx->nz_own || nz_global < ctx->nz_own) return fail(ctx, U1U1_ESTATE, "slab_diagnostics_finish needs a slab context and the global number of planes");
+    if (raw_reduced[FR_MAXTH] > 180.0)
+        return fail(ctx, U1U1_ESTATE, "diagnostics: a link phase exceeds |theta| = 180, beyond the range of the winding sweep");
+    double r[34];
+    for (int k = 0; k < FUSED_NRES; k++) r[k] = raw_reduced[k];
+    for (int k = FUSED_NRES; k < 34; k++) r[k] = NAN;        // the tolerant overlap needs cell-array halos: not on slabs
+    derive_diagnostics(ctx, r, (double)ctx->N * ctx->N * (double)nz_global, out);
     return U1U1_OK;
 }

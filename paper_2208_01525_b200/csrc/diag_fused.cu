@@ -59,7 +59,11 @@ diag_fused_kernel(const float *__restrict__ posp, const float *__restrict__ momp
     const char *pos = reinterpret_cast<const char *>(posp);
     const unsigned long long pol_stream = (k.flags & 32) ? policy_evict_last() : policy_evict_first();
     const unsigned long long pol_keep = (k.flags & 16) ? policy_evict_first() : policy_evict_last();
-    const int ntx = (N + TX - 1) / TX, nty = (N + TY - 1) / TY, nzc = (N + zchunk - 1) / zchunk;
+    // z extent: the whole periodic lattice, or the own planes 1 .. nz_own of a z slab (halo planes 0 and nz_own + 1 are
+    // only read: positions above for the forward z neighbours, momentum pack C below for div E)
+    const int NZO = k.nz_own ? k.nz_own : N, ZB = k.nz_own ? 1 : 0;
+    const bool zwrap = k.nz_own == 0;
+    const int ntx = (N + TX - 1) / TX, nty = (N + TY - 1) / TY, nzc = (NZO + zchunk - 1) / zchunk;
     const int items = ntx * nty * nzc;
     const float4 *gMA = reinterpret_cast<const float4 *>(momp);
     const float2 *gMC = reinterpret_cast<const float2 *>(momp + 8 * V);
@@ -77,8 +81,8 @@ diag_fused_kernel(const float *__restrict__ posp, const float *__restrict__ momp
         // item -> (tile, chunk) in band order (see step_tiled.cu)
         const int full = ntx * band * nzc, bnd = item / full, rem = item - bnd * full;
         const int rows = min(band, nty - bnd * band), bzc = rem / (ntx * rows), tl = rem - bzc * (ntx * rows);
-        const int x0 = (tl % ntx) * TX, y0 = (bnd * band + tl / ntx) * TY, z0 = bzc * zchunk;
-        const int wx = min(TX, N - x0), wy = min(TY, N - y0), nz = min(zchunk, N - z0);
+        const int x0 = (tl % ntx) * TX, y0 = (bnd * band + tl / ntx) * TY, z0 = ZB + bzc * zchunk;
+        const int wx = min(TX, N - x0), wy = min(TY, N - y0), nz = min(zchunk, ZB + NZO - z0);
         const bool active = tx < wx && ty < wy;
         const bool tma = !(k.flags & 2) && tile_is_interior(x0, y0, N);
 
@@ -96,7 +100,7 @@ diag_fused_kernel(const float *__restrict__ posp, const float *__restrict__ momp
         if (!tma) make_cp_plan(plan, tid, x0, y0, wx, wy, N);
         const unsigned pb = tma ? gpos : 0u, mb = tma ? gmom : 0u;
         auto stage_pos = [&](int j, unsigned slot) {
-            const int z = wrapi(z0 + j, N);
+            const int z = zwrap ? wrapi(z0 + j, N) : z0 + j;
             if (tma) stage_plane_tma(maps.pos, x0, y0, z, sbase + slot * SLOT_BYTES, bars + 8 * slot, pol_keep);
             else stage_plane_cp(plan, tid, pos, V, (size_t)z * NN, sbase + slot * SLOT_BYTES);
         };
@@ -132,7 +136,7 @@ diag_fused_kernel(const float *__restrict__ posp, const float *__restrict__ momp
         size_t lin = (size_t)z0 * NN + gsite;
         // E_z, H_z of plane z0 - 1 (for div E of the first plane)
         float2 ez_prev = make_float2(0.f, 0.f);
-        if (active) ez_prev = __ldg(gMC + (size_t)wrapi(z0 - 1, N) * NN + gsite);
+        if (active) ez_prev = __ldg(gMC + (size_t)(zwrap ? wrapi(z0 - 1, N) : z0 - 1) * NN + gsite);
 
         // extended sites: the tile plus its +x column and +y row (the cells of the last column / row need their
         // plaquettes).  Pass 1 = own element of every thread; pass 2 = the extra row (32 lanes of one warp) and the
@@ -471,8 +475,10 @@ cudaError_t launch_diag_fused(const float *pos, const float *mom, size_t V, int 
         memset(&m, 0, sizeof m);
         k.flags |= 2;
     }
-    const int zc = (k.flags & 64) ? (N >= 16 ? 16 : N) : (k.flags & 128) ? (N >= 32 ? 32 : N) : fused_zchunk(N);   // tuning flags
-    const int ntx = (N + TX - 1) / TX, nty = (N + TY - 1) / TY, nzc = (N + zc - 1) / zc;
+    const int nzo = k.nz_own ? k.nz_own : N;              // planes to sweep: the lattice, or the own planes of a z slab
+    int zc = (k.flags & 64) ? 16 : (k.flags & 128) ? 32 : fused_zchunk(N);   // tuning flags
+    if (zc > nzo) zc = nzo;
+    const int ntx = (N + TX - 1) / TX, nty = (N + TY - 1) / TY, nzc = (nzo + zc - 1) / zc;
     const long items = (long)ntx * nty * nzc;
     long grid = (long)sms * FUSED_CTAS;
     if (grid > RED_MAX_BLOCKS) grid = RED_MAX_BLOCKS;

@@ -33,6 +33,7 @@ struct FusedCoef {
     float sig1sq, sig2sq;
     float c, inv_c;              // a^{2 beta} and its inverse
     int flags;                   // 2 = no TMA (cp.async staging everywhere)
+    int nz_own;                  // 0: cubic lattice, periodic in z; else a z slab: own planes 1 .. nz_own of nz_own + 2, no z wrap
 };
 struct DiagMaps;
 cudaError_t launch_diag_fused(const float *pos, const float *mom, size_t V, int N, FusedCoef k, uint8_t *cells, uint8_t *codes,

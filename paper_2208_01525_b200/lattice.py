@@ -154,7 +154,7 @@ class Slab:
             raise B.U1U1Error(f"unsupported slab N={N}, nz_own={nz_own}")
         with torch.cuda.device(self.device):
             self.state = torch.zeros(sb, dtype=torch.uint8, device=self.device)
-            self.scratch = torch.empty(1 << 20, dtype=torch.uint8, device=self.device)
+            self.scratch = torch.empty(self.lib.u1u1_slab_scratch_bytes(self.N, self.nz_own), dtype=torch.uint8, device=self.device)
             self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
         self._ctx = ctypes.c_void_p()
         rc = self.lib.u1u1_create(ctypes.byref(self._ctx), self.state.data_ptr(), sb, self.scratch.data_ptr(),
@@ -181,6 +181,20 @@ class Slab:
 
     def push_halos(self):
         self._check(self.lib.u1u1_push_halos(self._ctx), "push_halos")
+
+    def push_diag_halos(self):
+        self._check(self.lib.u1u1_push_diag_halos(self._ctx), "push_diag_halos")
+
+    def slab_diagnostics_partial(self) -> np.ndarray:
+        raw = (ctypes.c_double * B.SLAB_NRAW)()
+        self._check(self.lib.u1u1_slab_diagnostics_partial(self._ctx, raw), "slab_diagnostics_partial")
+        return np.array(raw[:])
+
+    def slab_diagnostics_finish(self, raw_reduced, nz_global: int) -> dict:
+        raw = (ctypes.c_double * B.SLAB_NRAW)(*[float(v) for v in raw_reduced])
+        out = (ctypes.c_double * B.DIAG_LEN)()
+        self._check(self.lib.u1u1_slab_diagnostics_finish(self._ctx, raw, nz_global, out), "slab_diagnostics_finish")
+        return {k: out[i] for i, k in enumerate(B.DIAG_SLOTS)}
 
     def export_slab(self):
         t = self._torch.empty((20, self.nz_own, self.N, self.N), dtype=self._torch.float32, device=self.device)

@@ -80,6 +80,31 @@ class SlabRing:
         import torch
         return torch.cat([s.export_slab() for s in self.slabs], dim=1)
 
+    def diagnostics(self):
+        """The u1u1_diagnostics output of the whole lattice: per-slab sweeps, then the reduction the ranks would do."""
+        for s in self.slabs:
+            s.push_diag_halos()
+        raws = [s.slab_diagnostics_partial() for s in self.slabs]
+        return self.slabs[0].slab_diagnostics_finish(reduce_raw(raws), self.nz_global)
+
+
+def reduce_raw(raws):
+    """SUM over the first SLAB_NSUM raw values, MAX over the rest (what the all-reduce pair of the ranks computes)."""
+    import numpy as np
+    a = np.stack(raws)
+    return np.concatenate([a[:, :B.SLAB_NSUM].sum(axis=0), a[:, B.SLAB_NSUM:].max(axis=0)])
+
+
+def all_reduce_raw(raw, dist, device):
+    """The same across ranks: one SUM and one MAX all-reduce of a handful of doubles."""
+    import numpy as np
+    import torch
+    t = torch.tensor(raw, dtype=torch.float64, device=device)
+    head, tail = t[:B.SLAB_NSUM].clone(), t[B.SLAB_NSUM:].clone()
+    dist.all_reduce(head, op=dist.ReduceOp.SUM)
+    dist.all_reduce(tail, op=dist.ReduceOp.MAX)
+    return np.concatenate([head.cpu().numpy(), tail.cpu().numpy()])
+
 
 def open_peer_states(state, dist, rank: int, world: int, up: int, dn: int):
     """Every rank publishes the CUDA IPC handle of its state tensor; returns tensors aliasing the state buffers of the
@@ -140,8 +165,15 @@ def run(size: int, steps: int, seed: int = 5, nz_global: int | None = None, chec
         barrier()
     torch.cuda.synchronize()
     wall = time.perf_counter() - t0
+    # diagnostics of the whole lattice: halo of E_z below, per-rank sweep, reduction of 28 doubles
+    slab.push_diag_halos()
+    barrier()
+    raw = all_reduce_raw(slab.slab_diagnostics_partial(), dist, "cpu" if dist.get_backend() == "gloo" else f"cuda:{dev}")
+    d = slab.slab_diagnostics_finish(raw, nzg)
     out = {"rank": rank, "world": world, "N": size, "nz_global": nzg, "nz_own": nz, "steps": steps, "wall_s": wall,
-           "site_updates_per_s": size * size * nzg * steps / wall, "backend": dist.get_backend(), "shared_gpu": shared_gpu}
+           "site_updates_per_s": size * size * nzg * steps / wall, "backend": dist.get_backend(), "shared_gpu": shared_gpu,
+           "diagnostics": {k: d[k] for k in ("tau", "sumW_p", "sumW_q", "cells_pq", "maxW", "xi_W", "sum_L", "energy",
+                                             "gauss_rel_p", "gauss_rel_q", "max_theta")}}
     if rank == 0:
         emit(json.dumps(out))
     dist.barrier()

@@ -64,6 +64,44 @@ def test_slab_ring_on_a_generic_state_against_the_oracle():
     assert max(err.values()) < 3e-5, err
 
 
+@pytest.mark.parametrize("N,world,nzg", [(128, 2, None), (64, 4, None), (48, 3, 96)])
+def test_slab_diagnostics_reduce_to_the_single_lattice(N, world, nzg):
+    """Every slab sweeps its own planes (positions' upper halo from the step, E_z of the plane below pushed first), the
+    28 raw values are reduced like the ranks' all-reduce pair does, and the result is the u1u1_diagnostics output of the
+    whole lattice: integer counts identical, sums equal up to the grouping of the fp32 partial sums."""
+    import torch
+    from paper_2208_01525_b200 import Lattice, Params
+    from paper_2208_01525_b200.zslab import SlabRing
+    prm = Params(tau_norm=40.0, friction=0.5)
+    ring = SlabRing(N, world, DX, prm, nz_global=nzg)
+    ring.init(7)
+    ring.step(25, 1.0, 0.5, 1.0, DTAU)
+    d = ring.diagnostics()
+    if nzg is None:
+        ref = Lattice(N)
+        ref.init_fields(7, DX, prm)
+        ref.step(25, 1.0, 0.5, 1.0)
+        want = ref.diagnostics()
+        ints = ("tau", "a", "c", "sumW_p", "sumW_q", "cells_p", "cells_q", "cells_pq", "near_p", "near_q", "maxW", "max_theta",
+                "gauss_max_p", "gauss_max_q", "L_p", "L_q", "L_pq", "xi_p", "xi_q", "xi_pq", "xi_W", "f_total", "f_p")
+        assert all(d[k] == want[k] for k in ints), {k: (d[k], want[k]) for k in ints if d[k] != want[k]}
+        for k in ("sum_L", "sum_kin_L", "sum_grad_L", "sum_kin_V", "sum_grad_V", "sum_vint", "sum_kin", "sum_grad", "sum_elec",
+                  "sum_mag", "sum_pot", "energy", "xi_L", "v2_L", "v2_pq", "gauss_l2_p", "gauss_rho_p", "gauss_rel_p", "gauss_rel_q"):
+            assert np.isclose(d[k], want[k], rtol=2e-6, atol=1e-6 * abs(want["sum_grad"]) if k.startswith("sum_") else 0), (k, d[k], want[k])
+        assert want["sumW_p"] > 0 and want["gauss_rel_p"] < 1e-5
+    else:                                               # non-cubic global lattice: against the oracle on the gathered state
+        snap = ring.export_global().cpu().numpy().astype(np.float64)
+        _, c, _, _ = O.scalars(1.0 + 25 * DTAU, 0.5, 1.0, DTAU, 40.0)
+        ref = O.diagnostics(snap, DX, O.Couplings(), c)
+        assert abs(d["sumW_p"] - ref["sumW_p"]) <= d["near_p"] + ref["near_p"] and d["sumW_p"] > 0
+        assert abs(d["cells_pq"] - ref["cells_pq"]) <= d["near_p"] + d["near_q"] + ref["near_p"] + ref["near_q"]
+        scale = ref["sum_kin"] + ref["sum_grad"] + ref["sum_elec"] + ref["sum_mag"] + abs(ref["sum_pot"])
+        for k in ("sum_kin", "sum_grad", "sum_elec", "sum_mag", "sum_pot", "sum_L"):
+            assert abs(d[k] - ref[k]) < 2e-6 * scale, (k, d[k], ref[k])
+        assert np.isclose(d["xi_W"], ref["xi_W"], rtol=1e-3)
+    assert np.isnan(d["L_pq_tol"])                      # the tolerant overlap needs cell-array halos: not on slabs
+
+
 def test_slab_calls_out_of_order():
     from paper_2208_01525_b200 import Slab, Params, U1U1Error
     s = Slab(32, 8, 0)
@@ -102,3 +140,7 @@ def test_two_ranks_sharing_the_gpu_over_cuda_ipc(tmp_path):
     ref.init_fields(5, DX, Params(tau_norm=256.0, friction=0.5))
     ref.step(steps, 1.0, 0.5, 1.0)
     assert torch.equal(got, ref.export_state().cpu())
+    want = ref.diagnostics()                            # the ranks' all-reduced diagnostics
+    for k, v in line["diagnostics"].items():
+        assert np.isclose(v, want[k], rtol=2e-6), (k, v, want[k])
+    assert line["diagnostics"]["sumW_p"] == want["sumW_p"] and line["diagnostics"]["cells_pq"] == want["cells_pq"]
