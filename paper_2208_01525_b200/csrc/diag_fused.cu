@@ -17,6 +17,7 @@
 // (atan2(0,0) = 0, R-15: chi = 0) or within 1e-5 of the cut are flagged and take a slow path that evaluates the
 // printed formula.
 #include <cstring>
+#include <type_traits>
 
 #include "common.cuh"
 #include "kernels.h"
@@ -82,9 +83,13 @@ diag_fused_kernel(const float *__restrict__ posp, const float *__restrict__ momp
         const int full = ntx * band * nzc, bnd = item / full, rem = item - bnd * full;
         const int rows = min(band, nty - bnd * band), bzc = rem / (ntx * rows), tl = rem - bzc * (ntx * rows);
         const int x0 = (tl % ntx) * TX, y0 = (bnd * band + tl / ntx) * TY, z0 = ZB + bzc * zchunk;
-        const int wx = min(TX, N - x0), wy = min(TY, N - y0), nz = min(zchunk, ZB + NZO - z0);
-        const bool active = tx < wx && ty < wy;
-        const bool tma = !(k.flags & 2) && tile_is_interior(x0, y0, N);
+        const int nz = min(zchunk, ZB + NZO - z0);
+        // Two instances of the item body: interior tiles (full 32 x 8 tile, TMA staging: every tile predicate and the
+        // cp.async path fold away at compile time -- 92 % of the tiles at 1024^3) and boundary / ragged tiles.
+        auto run_item = [&](auto interior) {
+        constexpr bool tma = decltype(interior)::value;
+        const int wx = tma ? TX : min(TX, N - x0), wy = tma ? TY : min(TY, N - y0);
+        const bool active = tma || (tx < wx && ty < wy);
 
         // this item's partial sums in fp32 (at most zchunk terms each), folded into the per-warp fp64 accumulators at its end
         float gf[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f}, df[11] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
@@ -141,7 +146,7 @@ diag_fused_kernel(const float *__restrict__ posp, const float *__restrict__ momp
         // extended sites: the tile plus its +x column and +y row (the cells of the last column / row need their
         // plaquettes).  Pass 1 = own element of every thread; pass 2 = the extra row (32 lanes of one warp) and the
         // extra column (9 lanes of the next warp), rotated over the warps from plane to plane to spread the load.
-        const bool own_ext = tx <= wx && ty <= wy;
+        const bool own_ext = tma || (tx <= wx && ty <= wy);
         const int e_row = (TY + 1) * COLS + lane + 1, e_col = (lane + 1) * COLS + TX + 1;
         auto do_alpha = [&](int e, const char *sn, int nxt) {          // phases of one site of plane `sn` into alpha[nxt]
             const float4 a = *reinterpret_cast<const float4 *>(sn + e * 16);
@@ -447,6 +452,9 @@ diag_fused_kernel(const float *__restrict__ posp, const float *__restrict__ momp
         amax(FR_GMAX + 1, (double)__uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(gmax[1]))));
         amax(FR_MAXW, (double)__reduce_max_sync(0xffffffffu, (unsigned)max(maxw, wany ? 1 : 0)));
         amax(FR_MAXTH, (double)__uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(maxth))));
+        };
+        if (!(k.flags & 2) && tile_is_interior(x0, y0, N)) run_item(std::true_type{});
+        else run_item(std::false_type{});
     }
 
     // ---- per-CTA partials: the 8 warps' accumulators in fixed order ----
