@@ -9,11 +9,14 @@ namespace u1u1 {
 // ------------------------------------------------------------------------------------------------
 // Internal HBM layout: packed vectors per site, site index lin = x + N (y + N z).
 // A position buffer (10 V floats) and the momentum buffer (10 V floats) have the same shape:
-//   pack A: float4[V]  (phi_re, phi_im, psi_re, psi_im)        | momenta: (Pi_re, Pi_im, Psi_re, Psi_im)
-//   pack B: float4[V]  (thetaA_x, thetaA_y, thetaB_x, thetaB_y) | (E_x, E_y, H_x, H_y)
+//   pack A: float4[V]  (phi_re, psi_re, phi_im, psi_im)        | momenta: (Pi_re, Psi_re, Pi_im, Psi_im)
+//   pack B: float4[V]  (thetaA_x, thetaB_x, thetaA_y, thetaB_y) | (E_x, H_x, E_y, H_y)
 //   pack C: float2[V]  (thetaA_z, thetaB_z)                     | (E_z, H_z)
 // so one site moves as 3 vector loads + 6 vector stores, and a stencil neighbour's scalars (both
 // sectors) or in-plane links (both sectors) arrive in one 128-bit shared-memory read.
+// The SAME quantity of the two sectors always sits in an aligned pair of adjacent words: the two sectors obey the
+// same equations, so the step kernel runs them through the packed fp32x2 instructions of sm_100 (FFMA2 / FADD2 /
+// FMUL2: one issue slot for both sectors) straight from the 64-bit halves of its vector loads.
 // state buffer = [pos0 | pos1 | mom], 30 V floats.
 // "Logical" component order used by the scalar accessors: 0 phi_re 1 phi_im 2 psi_re 3 psi_im
 // 4..6 thetaA_xyz 7..9 thetaB_xyz (momenta: Pi, Psi, E_xyz, H_xyz).
@@ -42,10 +45,15 @@ struct Lattice {
 // float offset of logical component c (0..9) of site lin inside a 10 V-float buffer
 __host__ __device__ inline size_t comp_off(int c, size_t lin, size_t V)
 {
-    if (c < 4) return 4 * lin + (size_t)c;
+    if (c < 4) return 4 * lin + (size_t)(2 * (c & 1) + (c >> 1));
     const int s = (c - 4) / 3, i = (c - 4) % 3;
-    return i < 2 ? 4 * V + 4 * lin + (size_t)(2 * s + i) : 8 * V + 2 * lin + (size_t)s;
+    return i < 2 ? 4 * V + 4 * lin + (size_t)(2 * i + s) : 8 * V + 2 * lin + (size_t)s;
 }
+
+// first (re / x link) and second (im / y link) word of sector s in a float4 of pack A or B; word of sector s in pack C
+__host__ __device__ inline float pk0(const float4 &v, int s) { return s ? v.y : v.x; }
+__host__ __device__ inline float pk1(const float4 &v, int s) { return s ? v.w : v.z; }
+__host__ __device__ inline float pkc(const float2 &v, int s) { return s ? v.y : v.x; }
 
 // canonical component -> (is_momentum, logical component)
 __host__ __device__ inline void canonical_to_internal(int c, int &is_mom, int &plane)

@@ -47,13 +47,13 @@ __global__ void __launch_bounds__(RED_BLOCK) gauss_kernel(const float *pos, cons
         const float2 ec = MC[lin], ecz = MC[w.at(x, y, w.m(z))];
 #pragma unroll
         for (int s = 0; s < 2; s++) {
-            const float E[3] = {s ? eb.z : eb.x, s ? eb.w : eb.y, s ? ec.y : ec.x};
-            const float Em[3] = {s ? ebx.z : ebx.x, s ? eby.w : eby.y, s ? ecz.y : ecz.x};
+            const float E[3] = {pk0(eb, s), pk1(eb, s), pkc(ec, s)};
+            const float Em[3] = {pk0(ebx, s), pk1(eby, s), pkc(ecz, s)};
             double div = 0.0;
 #pragma unroll
             for (int i = 0; i < 3; i++) div += ((double)E[i] - (double)Em[i]) * k.inv_dx;
-            const double fr = s ? a.z : a.x, fi = s ? a.w : a.y;
-            const double pr = s ? ma.z : ma.x, pi = s ? ma.w : ma.y;
+            const double fr = pk0(a, s), fi = pk1(a, s);
+            const double pr = pk0(ma, s), pi = pk1(ma, s);
             const double e0 = s ? k.e2 : k.e1;
             const double rho = 2.0 * e0 * e0 * k.cG * (fr * pi - fi * pr);
             const double g = div - rho;

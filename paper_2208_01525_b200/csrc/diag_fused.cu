@@ -150,8 +150,8 @@ diag_fused_kernel(const float *__restrict__ posp, const float *__restrict__ momp
         const int e_row = (TY + 1) * COLS + lane + 1, e_col = (lane + 1) * COLS + TX + 1;
         auto do_alpha = [&](int e, const char *sn, int nxt) {          // phases of one site of plane `sn` into alpha[nxt]
             const float4 a = *reinterpret_cast<const float4 *>(sn + e * 16);
-            alpha[(nxt * 2 + 0) * NELEM + e] = site_phase(a.x, a.y);
-            alpha[(nxt * 2 + 1) * NELEM + e] = site_phase(a.z, a.w);
+            alpha[(nxt * 2 + 0) * NELEM + e] = site_phase(a.x, a.z);
+            alpha[(nxt * 2 + 1) * NELEM + e] = site_phase(a.y, a.w);
         };
         // wrap counts of the x and y links of one site of plane `sn` (links that leave the extended tile -- x links of
         // the extra column, y links of the extra row -- are evaluated on whatever the neighbouring shared-memory words
@@ -161,8 +161,8 @@ diag_fused_kernel(const float *__restrict__ posp, const float *__restrict__ momp
             const float *ap = alpha + (nxt * 2 + 0) * NELEM + e, *aq = alpha + (nxt * 2 + 1) * NELEM + e;
             a0p = ap[0];
             a0q = aq[0];
-            const unsigned X = __byte_perm(link_lane(a0p, ap[1], Bn.x), link_lane(a0q, aq[1], Bn.z), 0x5410);
-            const unsigned Y = __byte_perm(link_lane(a0p, ap[COLS], Bn.y), link_lane(a0q, aq[COLS], Bn.w), 0x5410);
+            const unsigned X = __byte_perm(link_lane(a0p, ap[1], Bn.x), link_lane(a0q, aq[1], Bn.y), 0x5410);
+            const unsigned Y = __byte_perm(link_lane(a0p, ap[COLS], Bn.z), link_lane(a0q, aq[COLS], Bn.w), 0x5410);
             XY[nxt * NELEM + e] = make_uint2(X, Y);
         };
         auto do_links = [&](int e, const char *sc, const char *sn, int cur) {      // + the z links of plane `sc`
@@ -241,11 +241,11 @@ diag_fused_kernel(const float *__restrict__ posp, const float *__restrict__ momp
                 float kin = 0.f, grad = 0.f, elec = 0.f, mag = 0.f, m2[2];
 #pragma unroll
                 for (int s = 0; s < 2; s++) {
-                    const float fr = s ? Ac.z : Ac.x, fi = s ? Ac.w : Ac.y;
-                    const float pr = s ? MA.z : MA.x, pi = s ? MA.w : MA.y;
+                    const float fr = pk0(Ac, s), fi = pk1(Ac, s);
+                    const float pr = pk0(MA, s), pi = pk1(MA, s);
                     // Gauss (Eq. 9-10): differences and the charge density in fp64 (g is a 1e-6 cancellation)
-                    const float E[3] = {s ? MB.z : MB.x, s ? MB.w : MB.y, s ? MC.y : MC.x};
-                    const float Em[3] = {s ? MBxm.z : MBxm.x, s ? MBym.w : MBym.y, s ? ez_prev.y : ez_prev.x};
+                    const float E[3] = {pk0(MB, s), pk1(MB, s), pkc(MC, s)};
+                    const float Em[3] = {pk0(MBxm, s), pk1(MBym, s), pkc(ez_prev, s)};
                     const double div = (((double)E[0] - (double)Em[0]) + ((double)E[1] - (double)Em[1]) + ((double)E[2] - (double)Em[2])) * k.inv_dx;
                     const double rho = (s ? k.rho2 : k.rho1) * ((double)fr * (double)pi - (double)fi * (double)pr);
                     const float gl = (float)(div - rho), rl = (float)rho, dl = (float)div;
@@ -256,9 +256,9 @@ diag_fused_kernel(const float *__restrict__ posp, const float *__restrict__ momp
                     // densities (fp32 per-site terms)
                     kin = fmaf(pr, pr, fmaf(pi, pi, kin));
                     m2[s] = fmaf(fr, fr, fi * fi);
-                    const float th[3] = {s ? Bc.z : Bc.x, s ? Bc.w : Bc.y, s ? Cc.y : Cc.x};
-                    const float nr[3] = {s ? Axp.z : Axp.x, s ? Ayp.z : Ayp.x, s ? Azp.z : Azp.x};
-                    const float ni[3] = {s ? Axp.w : Axp.y, s ? Ayp.w : Ayp.y, s ? Azp.w : Azp.y};
+                    const float th[3] = {pk0(Bc, s), pk1(Bc, s), pkc(Cc, s)};
+                    const float nr[3] = {pk0(Axp, s), pk0(Ayp, s), pk0(Azp, s)};
+                    const float ni[3] = {pk1(Axp, s), pk1(Ayp, s), pk1(Azp, s)};
                     float g2 = 0.f, e2 = 0.f;
 #pragma unroll
                     for (int i = 0; i < 3; i++) {
@@ -270,9 +270,9 @@ diag_fused_kernel(const float *__restrict__ posp, const float *__restrict__ momp
                         maxth = fmaxf(maxth, fabsf(th[i]));
                     }
                     // plaquettes (i, j) = (x,y), (x,z), (y,z)
-                    const float ty_x = s ? Bxp.w : Bxp.y, tx_y = s ? Byp.z : Byp.x;
-                    const float tz_x = s ? Cxp.y : Cxp.x, tx_z = s ? Bzp.z : Bzp.x;
-                    const float tz_y = s ? Cyp.y : Cyp.x, ty_z = s ? Bzp.w : Bzp.y;
+                    const float ty_x = pk1(Bxp, s), tx_y = pk0(Byp, s);
+                    const float tz_x = pkc(Cxp, s), tx_z = pk0(Bzp, s);
+                    const float tz_y = pkc(Cyp, s), ty_z = pk1(Bzp, s);
                     const float P0 = th[0] + ty_x - tx_y - th[1], P1 = th[0] + tz_x - tx_z - th[2], P2 = th[1] + tz_y - ty_z - th[2];
                     grad = fmaf(g2, k.inv_dx2, grad);
                     elec = fmaf(e2, s ? k.el2 : k.el1, elec);
@@ -343,11 +343,11 @@ diag_fused_kernel(const float *__restrict__ posp, const float *__restrict__ momp
                     // own plaquettes; with a degenerate link (chi = 0 there, reading R-15) the printed formula
                     auto ph = [&](const char *s, int e, int sec) {
                         const float4 a = *reinterpret_cast<const float4 *>(s + e * 16);
-                        return sec ? site_phase(a.z, a.w) : site_phase(a.x, a.y);
+                        return site_phase(pk0(a, sec), pk1(a, sec));
                     };
                     auto th_xy = [&](const char *s, int e, int sec, int dir) {
                         const float4 b = *reinterpret_cast<const float4 *>(s + OFF_B + e * 16);
-                        return dir == 0 ? (sec ? b.z : b.x) : (sec ? b.w : b.y);
+                        return dir == 0 ? pk0(b, sec) : pk1(b, sec);
                     };
                     auto th_z = [&](const char *s, int e, int sec) {
                         const int r = e / COLS;

@@ -39,9 +39,9 @@ __global__ void init_random_phase_kernel(float *pos, size_t n_own, size_t lin_of
         sincospi(2.0 * ((double)r[0] * (1.0 / 4294967296.0)), &sn, &cs);
         float4 a;
         a.x = (float)(eta1 * cs);
-        a.y = (float)(eta1 * sn);
+        a.z = (float)(eta1 * sn);
         sincospi(2.0 * ((double)r[1] * (1.0 / 4294967296.0)), &sn, &cs);
-        a.z = (float)(eta2 * cs);
+        a.y = (float)(eta2 * cs);
         a.w = (float)(eta2 * sn);
         reinterpret_cast<float4 *>(pos)[i + lin_off] = a;           // pack A
     }

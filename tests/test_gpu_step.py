@@ -226,6 +226,22 @@ def test_staging_paths_bit_identical(base):
     assert np.array_equal(outs[0], outs[1]) and np.array_equal(outs[0], outs[2])
 
 
+def test_packed_chain_bit_identical_to_scalar_chain():
+    """The default kernel runs both sectors through packed fp32x2 instructions (FFMA2 / FADD2 / FMUL2): the same IEEE
+    operations in the same order as the scalar difference-form chain (tuning flag 1), so the states must be bit-identical
+    -- with unequal couplings in the two sectors, friction, and on interior, boundary and ragged tiles."""
+    from paper_2208_01525_b200 import Params
+    N = 132
+    s0 = inputs.to_f32_exact(inputs.random_state((N, N, N), seed=37))
+    outs = []
+    for flags in (0, 1, 1 + 2):
+        prm = Params(lambda1=2.0, lambda2=1.7, e1=1.0, e2=0.8, eta1=1.0, eta2=1.1, kappa=0.6, friction=0.9,
+                     kernel_variant=16 * flags, tau_norm=1.5)
+        out, _ = run_gpu(s0, N, prm, [(3, 2.0, 0.5, 1.0), (2, 2.3, 0.5, -1.0)])
+        outs.append(out)
+    assert np.array_equal(outs[0], outs[1]) and np.array_equal(outs[0], outs[2])
+
+
 @pytest.mark.parametrize("variant,tol", [(0, 2e-5), (7, 1e-5), (4, 2e-5)])
 def test_large_link_phases(variant, tol):
     """Non-compact links far outside (-pi, pi] (|theta| up to ~40, reading R-9): the SFU phasor's error grows like
