@@ -209,7 +209,7 @@ def run_ours(args):
     build.build()
     N = args.size
     V = N ** 3
-    lat = Lattice(N, device=f"cuda:{local}")
+    lat = Lattice(N, device=f"cuda:{local}", aux=bool(args.tb))
     prm = Params(tau_norm=256.0, friction=0.5, kernel_variant=args.variant)
     lat.init_fields(replica_seed(rank), DX, prm)
     lat.step(args.prephase, TAU0, ERA, S)                    # damped prephase (config 5: 200 steps)
@@ -342,6 +342,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--prephase", type=int, default=PREPHASE_STEPS)
     ap.add_argument("--variant", type=int, default=0)
+    ap.add_argument("--tb", type=int, default=1, help="1: second momentum buffer -> two steps per pass (step_tb.cu); 0: one-step kernel")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

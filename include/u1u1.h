@@ -69,7 +69,10 @@ typedef struct {
                                 1 / 3 = reference one-thread-per-site kernel in fp32 / fp64.
                                 Bits 4.. are tuning switches (0 in production): 16*2 = cp.async staging everywhere
                                 (no TMA), 16*4 = momenta by ld.global.cs, 16*8 = plain grid order (step kernel);
-                                16*16 / 16*32 = L2 policies, 16*64 / 16*128 = 16 / 32-plane chunks (diagnostics).  */
+                                16*1 = variant 0 in scalar instead of packed fp32x2 instructions (same bits);
+                                16*16 / 16*32 = L2 policies, 16*64 / 16*128 = 16 / 32-plane chunks (diagnostics);
+                                16*256 = one-step kernel even with an aux buffer, 16*512 / 16*1024 = 16 / 64-plane
+                                chunks of the two-steps-per-pass kernel.  */
 } u1u1_params;
 
 /* Bytes of device memory the caller must provide for an N^3 lattice.
@@ -79,6 +82,17 @@ typedef struct {
  *          partials. */
 size_t u1u1_state_bytes(int32_t N);
 size_t u1u1_scratch_bytes(int32_t N);
+
+/* Optional second momentum buffer (10 fp32 words/site, DEVICE, 256-byte aligned; NULL detaches it).  With it,
+ * u1u1_step advances TWO leapfrog steps per pass over the lattice (temporal blocking): a thread
+ * block evaluates step 1 on its tile plus a one-site halo into shared memory and step 2 from there, so each site's 20
+ * words make one HBM round trip per two steps (80 B per site-update instead of 160).  That kernel reads the halo
+ * sites' momenta while neighbouring blocks update theirs, hence momenta go from one buffer to the other; the library
+ * tracks which one is current.  Results are bit-identical to the one-step kernel's.  Cubic lattices, kernel_variant 0;
+ * an odd last step of a call takes the one-step kernel.  May be called before or after u1u1_configure; must hold
+ * u1u1_aux_bytes(N).  1024^3: 43 GB on top of the 129 GB state (fits the 180 GB of a B200). */
+size_t u1u1_aux_bytes(int32_t N);
+int u1u1_set_aux(u1u1_ctx *ctx, void *aux_dev, size_t aux_bytes);
 
 /* Create a context over caller-owned DEVICE buffers (256-byte aligned) and a CUDA stream.
  * Nothing is launched.  *ctx is a small HOST object, released by u1u1_destroy. */

@@ -48,7 +48,7 @@ class U1U1Error(RuntimeError):
 
 
 _lib = None
-SYMBOLS = ["u1u1_state_bytes", "u1u1_scratch_bytes", "u1u1_create", "u1u1_destroy", "u1u1_last_error",
+SYMBOLS = ["u1u1_state_bytes", "u1u1_scratch_bytes", "u1u1_aux_bytes", "u1u1_set_aux", "u1u1_create", "u1u1_destroy", "u1u1_last_error",
            "u1u1_configure", "u1u1_init_fields", "u1u1_set_params", "u1u1_set_time", "u1u1_step", "u1u1_cool",
            "u1u1_diagnostics", "u1u1_gauss_violation", "u1u1_export_state", "u1u1_import_state",
            "u1u1_export_state_host", "u1u1_import_state_host", "u1u1_export_windings", "u1u1_export_block", "u1u1_launch_count", "u1u1_pq_segments", "u1u1_export_labels", "u1u1_import_state_tiled",
@@ -71,6 +71,8 @@ def load():
     dp, pp = ctypes.POINTER(ctypes.c_double), ctypes.POINTER(Params)
     L.u1u1_state_bytes.argtypes = [i32]; L.u1u1_state_bytes.restype = ctypes.c_size_t
     L.u1u1_scratch_bytes.argtypes = [i32]; L.u1u1_scratch_bytes.restype = ctypes.c_size_t
+    L.u1u1_aux_bytes.argtypes = [i32]; L.u1u1_aux_bytes.restype = ctypes.c_size_t
+    L.u1u1_set_aux.argtypes = [vp, vp, ctypes.c_size_t]
     L.u1u1_create.argtypes = [ctypes.POINTER(vp), vp, ctypes.c_size_t, vp, ctypes.c_size_t, vp]
     L.u1u1_destroy.argtypes = [vp]; L.u1u1_destroy.restype = None
     L.u1u1_last_error.argtypes = [vp]; L.u1u1_last_error.restype = ctypes.c_char_p

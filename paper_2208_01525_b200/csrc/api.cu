@@ -40,7 +40,13 @@ struct u1u1_ctx {
     // device properties and TMA tensor maps, set up on the first launch (nothing here needs a GPU before that)
     int sms = 0;
     bool maps_ready = false;
-    PackMaps pos_halo[2], mom_halo, mom_tile;
+    PackMaps pos_halo[2], mom_halo[2], mom_tile[2];     // momenta: [0] the buffer inside `state`, [1] the aux buffer
+    PackMaps pos_halo2[2];                               // two-site-halo boxes of the positions (two-steps-per-pass kernel)
+    // optional second momentum buffer (u1u1_set_aux): enables the two-steps-per-pass kernel, which reads the momenta
+    // from one buffer and writes them to the other
+    float *aux = nullptr;
+    size_t aux_bytes = 0;
+    int mcur = 0;                // which momentum buffer is current: 0 = inside `state`, 1 = aux
     // second stream and events of the pipelined host copies, created on first use
     cudaStream_t copy_stream = nullptr;
     cudaEvent_t ev_kernel[2] = {nullptr, nullptr}, ev_copy[2] = {nullptr, nullptr};
@@ -78,6 +84,31 @@ extern "C" size_t u1u1_scratch_bytes(int32_t N)
     if (!size_ok(N)) return 0;
     const size_t V = (size_t)N * N * N;
     return scratch_partials_offset(V) + ((size_t)RED_MAX_BLOCKS * RED_SLOTS + 64) * sizeof(double);
+}
+
+extern "C" size_t u1u1_aux_bytes(int32_t N)
+{
+    if (!size_ok(N)) return 0;
+    return (size_t)NMOM * (size_t)N * N * N * sizeof(float);
+}
+
+extern "C" int u1u1_set_aux(u1u1_ctx *ctx, void *aux_dev, size_t aux_bytes)
+{
+    if (!ctx) return U1U1_EINVAL;
+    if (ctx->nz_own) return fail(ctx, U1U1_ESTATE, "set_aux is not available on a z slab");
+    if (aux_dev && (((uintptr_t)aux_dev & 255) || (ctx->configured && aux_bytes < u1u1_aux_bytes(ctx->N))))
+        return fail(ctx, U1U1_ESIZE, "aux buffer must be 256-byte aligned and hold u1u1_aux_bytes(N)");
+    if (ctx->mcur == 1) {                     // the momenta live in the old aux buffer: bring them home first
+        cudaError_t e = cudaMemcpyAsync(ctx->state + (size_t)2 * NPOS * ctx->V, ctx->aux, (size_t)NMOM * ctx->V * sizeof(float),
+                                        cudaMemcpyDeviceToDevice, ctx->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "set_aux: moving the momenta back");
+        ctx->mcur = 0;
+    }
+    ctx->aux = (float *)aux_dev;
+    ctx->aux_bytes = aux_dev ? aux_bytes : 0;
+    ctx->maps_ready = false;
+    return U1U1_OK;
 }
 
 extern "C" int u1u1_create(u1u1_ctx **out, void *state_dev, size_t state_bytes, void *scratch_dev,
@@ -129,13 +160,14 @@ static int check_params(u1u1_ctx *ctx, const u1u1_params *p)
     if (p->init_kind != 0 && p->init_kind != 1) return fail(ctx, U1U1_EINVAL, "init_kind must be 0 or 1");
     if (p->init_kind == 1 && (!(p->smooth_width > 0) || p->smooth_trunc < 1 || p->smooth_trunc > 32))
         return fail(ctx, U1U1_EINVAL, "init_kind 1 needs smooth_width > 0 and 1 <= smooth_trunc <= 32");
-    if (p->kernel_variant < 0 || (p->kernel_variant & 15) > 7 || p->kernel_variant > 4095)
+    if (p->kernel_variant < 0 || (p->kernel_variant & 15) > 7 || p->kernel_variant > 65535)
         return fail(ctx, U1U1_EINVAL, "kernel_variant must be 0..7 (+16*tuning flags)");
     return U1U1_OK;
 }
 
 static float *pos_buf(u1u1_ctx *ctx, int which) { return ctx->state + (size_t)which * NPOS * ctx->V; }
-static float *mom_buf(u1u1_ctx *ctx) { return ctx->state + (size_t)2 * NPOS * ctx->V; }
+static float *mom_buf_at(u1u1_ctx *ctx, int which) { return which ? ctx->aux : ctx->state + (size_t)2 * NPOS * ctx->V; }
+static float *mom_buf(u1u1_ctx *ctx) { return mom_buf_at(ctx, ctx->mcur); }
 static uint8_t *cells_buf(u1u1_ctx *ctx) { return ctx->scratch; }
 static uint8_t *work_buf(u1u1_ctx *ctx) { return ctx->scratch + 2 * ctx->V; }
 static double *partials(u1u1_ctx *ctx) { return (double *)(ctx->scratch + scratch_partials_offset(ctx->V)); }
@@ -153,10 +185,15 @@ static int prepare_device(u1u1_ctx *ctx)
     }
     if (!ctx->maps_ready && step_tiled_uses_tma(ctx->N)) {
         const int NZ = ctx->nz_own ? ctx->nz_own + 2 : ctx->N;
-        const bool ok = encode_halo_maps(&ctx->pos_halo[0], pos_buf(ctx, 0), ctx->V, ctx->N, NZ) &&
+        bool ok = encode_halo_maps(&ctx->pos_halo[0], pos_buf(ctx, 0), ctx->V, ctx->N, NZ) &&
                         encode_halo_maps(&ctx->pos_halo[1], pos_buf(ctx, 1), ctx->V, ctx->N, NZ) &&
-                        encode_halo_maps(&ctx->mom_halo, mom_buf(ctx), ctx->V, ctx->N, NZ) &&
-                        encode_tile_maps(&ctx->mom_tile, mom_buf(ctx), ctx->V, ctx->N, NZ);
+                        encode_halo_maps(&ctx->mom_halo[0], mom_buf_at(ctx, 0), ctx->V, ctx->N, NZ) &&
+                        encode_tile_maps(&ctx->mom_tile[0], mom_buf_at(ctx, 0), ctx->V, ctx->N, NZ);
+        if (ok && ctx->aux)
+            ok = encode_halo_maps(&ctx->mom_halo[1], ctx->aux, ctx->V, ctx->N, NZ) &&
+                 encode_tile_maps(&ctx->mom_tile[1], ctx->aux, ctx->V, ctx->N, NZ) &&
+                 encode_halo2_maps(&ctx->pos_halo2[0], pos_buf(ctx, 0), ctx->V, ctx->N, NZ) &&
+                 encode_halo2_maps(&ctx->pos_halo2[1], pos_buf(ctx, 1), ctx->V, ctx->N, NZ);
         if (!ok) return fail(ctx, U1U1_ECUDA, "cuTensorMapEncodeTiled unavailable or rejected the layout (TMA is required)");
         ctx->maps_ready = true;
     }
@@ -171,6 +208,7 @@ extern "C" int u1u1_configure(u1u1_ctx *ctx, int32_t N, double dx, const u1u1_pa
     if (int rc = check_params(ctx, params)) return rc;
     if (ctx->state_bytes < u1u1_state_bytes(N)) return fail(ctx, U1U1_ESIZE, "state buffer smaller than u1u1_state_bytes(N)");
     if (ctx->scratch_bytes < u1u1_scratch_bytes(N)) return fail(ctx, U1U1_ESIZE, "scratch buffer smaller than u1u1_scratch_bytes(N)");
+    if (ctx->aux && ctx->aux_bytes < u1u1_aux_bytes(N)) return fail(ctx, U1U1_ESIZE, "aux buffer smaller than u1u1_aux_bytes(N)");
     ctx->N = N;
     ctx->V = (size_t)N * N * N;
     ctx->nz_own = 0;
@@ -180,6 +218,7 @@ extern "C" int u1u1_configure(u1u1_ctx *ctx, int32_t N, double dx, const u1u1_pa
     ctx->prm = *params;
     ctx->configured = true;
     ctx->cur = 0;
+    ctx->mcur = 0;
     ctx->tau_pos = params->tau_norm;
     ctx->a = ctx->c = ctx->cG = 1.0;
     ctx->diag_valid = ctx->codes_valid = ctx->labels_valid = false;
@@ -269,7 +308,7 @@ static cudaError_t launch_step(u1u1_ctx *ctx, const StepCoef &q)
     StepMaps maps;
     if (ctx->maps_ready) {
         maps.pos = ctx->pos_halo[ctx->cur];
-        maps.mom = ctx->mom_tile;
+        maps.mom = ctx->mom_tile[ctx->mcur];
     }
     return launch_step_tiled(L, q, ctx->stream, tiled_mode(kv), ctx->maps_ready ? &maps : nullptr, ctx->sms);
 }
@@ -295,9 +334,9 @@ extern "C" int u1u1_step(u1u1_ctx *ctx, int32_t n, double tau, double era_m, dou
         return fail(ctx, U1U1_EINVAL, "a z slab steps one step per call (the ranks synchronise in between) with kernel_variant 0");
     const u1u1_params &P = ctx->prm;
     const double dx = ctx->dx, dt = P.dtau, f = P.friction;
-    for (int k = 0; k < n; k++) {
-        const double tk = tau + k * dt;
-        double a, c, delta, omega;
+    // coefficients of the step that starts at conformal time tk (fp64 on the host, rounded once)
+    auto coef_at = [&](double tk, StepCoef &q, double &c, double &delta, double &omega) -> int {
+        double a;
         scalars_at(ctx, tk, era_m, s, a, c, delta, omega);
         const double lam = std::fmax(P.lambda1 * P.eta1 * P.eta1, P.lambda2 * P.eta2 * P.eta2) +
                            2.0 * P.kappa * std::fmax(P.eta1 * P.eta1, P.eta2 * P.eta2);
@@ -306,7 +345,6 @@ extern "C" int u1u1_step(u1u1_ctx *ctx, int32_t n, double tau, double era_m, dou
             snprintf(buf, sizeof buf, "leapfrog unstable at tau=%g: dtau^2 (12/dx^2 + (lambda+2kappa) sigma^2 a^{2s}) >= 4 (a^{2s}=%g)", tk, c);
             return fail(ctx, U1U1_EUNSTABLE, buf);
         }
-        StepCoef q;
         q.aS = (float)(f * (1.0 - delta) / (1.0 + delta));
         q.bS = (float)(f * dt / (1.0 + delta));
         q.aG = (float)(f * (1.0 - omega) / (1.0 + omega));
@@ -325,18 +363,46 @@ extern "C" int u1u1_step(u1u1_ctx *ctx, int32_t n, double tau, double era_m, dou
         q.aSm1 = (float)(f * (1.0 - delta) / (1.0 + delta) - 1.0);
         q.aGm1 = (float)(f * (1.0 - omega) / (1.0 + omega) - 1.0);
         q.flags = P.kernel_variant >> 4;
+        return U1U1_OK;
+    };
+    // Two steps per pass (step_tb.cu) whenever the caller has provided the second momentum buffer (u1u1_set_aux): default
+    // kernel variant, cubic lattice; tuning flag 256 keeps the one-step kernel.  An odd last step takes the one-step kernel.
+    const bool pairs = ctx->aux && !ctx->nz_own && (P.kernel_variant & 15) == 0 && !((P.kernel_variant >> 4) & (1 | 256)) &&
+                       step_tb_supports(ctx->N);
+    for (int k = 0; k < n;) {
+        const double tk = tau + k * dt;
+        StepCoef q, q2;
+        double c, delta, omega;
+        if (int rc = coef_at(tk, q, c, delta, omega)) return rc;
         if (int rc = prepare_device(ctx)) return rc;      // SM count and tensor maps, once per configure
-        cudaError_t e = launch_step(ctx, q);
+        int done = 1;
+        cudaError_t e;
+        if (pairs && k + 1 < n) {
+            if (int rc = coef_at(tau + (k + 1) * dt, q2, c, delta, omega)) return rc;
+            TbLattice L{pos_buf(ctx, ctx->cur), pos_buf(ctx, ctx->cur ^ 1), mom_buf_at(ctx, ctx->mcur), mom_buf_at(ctx, ctx->mcur ^ 1),
+                        ctx->V, ctx->N};
+            TbMaps maps;
+            if (ctx->maps_ready) {
+                maps.pos = ctx->pos_halo2[ctx->cur];
+                maps.mom = ctx->mom_halo[ctx->mcur];
+            }
+            e = launch_step_tb(L, q, q2, ctx->stream, ctx->maps_ready ? &maps : nullptr, ctx->sms);
+            ctx->mcur ^= 1;
+            done = 2;
+        } else {
+            e = launch_step(ctx, q);
+        }
         if (e != cudaSuccess) return cuda_fail(ctx, e, "step kernel launch");
         ctx->launches += 1;
         ctx->cur ^= 1;
-        ctx->tau_pos = tk + dt;
+        k += done;
+        ctx->tau_pos = (tau + (k - 1) * dt) + dt;         // start of the last step taken + dtau
         // weights for the diagnostics of the state just produced
         double a1, c1, d1, o1;
         scalars_at(ctx, ctx->tau_pos, era_m, s, a1, c1, d1, o1);
         ctx->a = a1;
         ctx->c = c1;
-        ctx->cG = c * (1.0 + delta) / (1.0 + omega);
+        ctx->cG = c * (1.0 + delta) / (1.0 + omega);      // of the last step taken
         invalidate(ctx);
     }
     return U1U1_OK;
@@ -468,7 +534,7 @@ static int run_sweep(u1u1_ctx *ctx, bool with_codes)
     DiagMaps maps;
     if (ctx->maps_ready) {
         maps.pos = ctx->pos_halo[ctx->cur];
-        maps.mom = ctx->mom_halo;
+        maps.mom = ctx->mom_halo[ctx->mcur];
     }
     int nb = 0;
     cudaError_t e = launch_diag_fused(pos_buf(ctx, ctx->cur), mom_buf(ctx), ctx->V, ctx->N, fused_coef(ctx), cells_buf(ctx),
@@ -747,6 +813,7 @@ extern "C" int u1u1_configure_slab(u1u1_ctx *ctx, int32_t N, int32_t nz_own, int
     ctx->prm = *params;
     ctx->configured = true;
     ctx->cur = 0;
+    ctx->mcur = 0;
     ctx->tau_pos = params->tau_norm;
     ctx->a = ctx->c = ctx->cG = 1.0;
     invalidate(ctx);
@@ -859,7 +926,7 @@ extern "C" int u1u1_slab_diagnostics_partial(u1u1_ctx *ctx, double *raw)
     DiagMaps maps;
     if (ctx->maps_ready) {
         maps.pos = ctx->pos_halo[ctx->cur];
-        maps.mom = ctx->mom_halo;
+        maps.mom = ctx->mom_halo[ctx->mcur];
     }
     int nb = 0;
     cudaError_t e = launch_diag_fused(pos_buf(ctx, ctx->cur), mom_buf(ctx), ctx->V, ctx->N, fused_coef(ctx), ctx->scratch, nullptr, part,

@@ -11,6 +11,20 @@ cudaError_t launch_step_tiled(const Lattice &L, const StepCoef &k, cudaStream_t 
 bool step_tiled_supports(int N);
 bool step_tiled_uses_tma(int N);
 
+// step_tb.cu: TWO fused steps per pass (80 B of HBM traffic per site-update); momenta are read from one buffer and
+// written to another, positions as in the one-step kernel
+struct TbLattice {
+    const float *pos_in;   // positions at tau (read, two-site halo)
+    float *pos_out;        // positions at tau + 2 dtau
+    const float *mom_in;   // momenta before the two kicks (read, one-site halo)
+    float *mom_out;        // momenta after them
+    size_t V;
+    int N;
+};
+struct TbMaps;
+cudaError_t launch_step_tb(const TbLattice &L, StepCoef k1, StepCoef k2, cudaStream_t st, const TbMaps *maps, int sms);
+bool step_tb_supports(int N);
+
 // diag_fused.cu: every in-loop diagnostic from one read of the state.  Partial / result slots:
 enum {
     FR_GAUSS = 0,    // sum g^2, rho^2, div^2 of the p sector, then of the q sector

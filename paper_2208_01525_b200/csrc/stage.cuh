@@ -29,6 +29,12 @@ constexpr int POS_TX_BYTES = NELEM * 32 + ROWS * CCOLS * 8;    // bytes one plan
 constexpr int NITEM = (3 * NELEM + NTHREADS - 1) / NTHREADS;   // cp.async copies per thread per plane (4)
 static_assert(NELEM * 16 <= OFF_B && OFF_B + NELEM * 16 <= OFF_C && OFF_C + ROWS * CCOLS * 8 <= SLOT_BYTES, "slot layout");
 
+// The two-steps-per-pass kernel (step_tb.cu) stages positions with a TWO-site halo: A, B float4[P2_ROWS][P2_COLS], C
+// float2[P2_ROWS][P2_COLS], all from site (x0-2, y0-2) (an even x, so pack C is 16-byte aligned as it is).
+constexpr int P2_COLS = TX + 4, P2_ROWS = TY + 4, P2_ELEM = P2_ROWS * P2_COLS;      // 36 x 12 = 432 sites
+constexpr int P2_OFF_B = P2_ELEM * 16, P2_OFF_C = 2 * P2_ELEM * 16, P2_SLOT_BYTES = P2_OFF_C + P2_ELEM * 8;   // 17 280 B
+static_assert(P2_OFF_B % 128 == 0 && P2_OFF_C % 128 == 0 && P2_SLOT_BYTES % 128 == 0, "TMA destinations");
+
 // Tensor maps of the three packs of one buffer (halo boxes COLS x ROWS, or plain TX x TY tile boxes).
 struct alignas(64) PackMaps {
     CUtensorMap A, B, C;
@@ -43,9 +49,15 @@ struct alignas(64) DiagMaps {
     PackMaps pos, mom;
 };
 
+// Tensor maps of one two-step launch: two-site-halo boxes of the positions being read, one-site-halo boxes of the momenta.
+struct alignas(64) TbMaps {
+    PackMaps pos, mom;
+};
+
 // host (tma_maps.cu): false if cuTensorMapEncodeTiled is unavailable or rejects the layout
 bool encode_halo_maps(PackMaps *m, const float *buf, size_t V, int N, int NZ, int rows = ROWS);
 bool encode_tile_maps(PackMaps *m, const float *buf, size_t V, int N, int NZ);
+bool encode_halo2_maps(PackMaps *m, const float *buf, size_t V, int N, int NZ);
 
 #ifdef __CUDACC__
 __device__ inline unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }

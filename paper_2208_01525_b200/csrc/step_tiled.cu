@@ -18,6 +18,7 @@
 #include "common.cuh"
 #include "kernels.h"
 #include "stage.cuh"
+#include "step_site.cuh"
 
 namespace u1u1 {
 
@@ -59,32 +60,6 @@ __device__ inline void phasor_diff(float th, float &sn, float &c1)
 __device__ inline float plaq(float a, float b, float c, float d)
 {
     return __fsub_rn(__fsub_rn(__fadd_rn(a, b), c), d);
-}
-
-// ---- packed fp32x2 arithmetic (sm_100: FFMA2 / FADD2 / FMUL2, one issue slot for two IEEE fp32 operations) ----
-// A pair holds the SAME quantity of the two sectors (p in .x, q in .y): the two sectors obey the same equations
-// (PAPER.md:79), and the layout of common.cuh puts such pairs in the aligned 64-bit halves of every vector load.
-// Negations fold into the operand modifiers of the packed instructions; scalars broadcast from uniform registers.
-typedef float2 f2;
-__device__ __forceinline__ f2 lo(const float4 &v) { return make_float2(v.x, v.y); }
-__device__ __forceinline__ f2 hi(const float4 &v) { return make_float2(v.z, v.w); }
-__device__ __forceinline__ f2 bc(float a) { return make_float2(a, a); }
-__device__ __forceinline__ f2 neg(f2 a) { return make_float2(-a.x, -a.y); }
-__device__ __forceinline__ f2 add2(f2 a, f2 b) { return __fadd2_rn(a, b); }
-__device__ __forceinline__ f2 sub2(f2 a, f2 b) { return __fadd2_rn(a, neg(b)); }
-__device__ __forceinline__ f2 mul2(f2 a, f2 b) { return __fmul2_rn(a, b); }
-__device__ __forceinline__ f2 fma2(f2 a, f2 b, f2 c) { return __ffma2_rn(a, b, c); }
-__device__ __forceinline__ f2 plaq2(f2 a, f2 b, f2 c, f2 d) { return sub2(sub2(add2(a, b), c), d); }
-// difference-form phasors of both sectors' link: the two MUFU pairs stay scalar, everything around them is packed
-__device__ __forceinline__ void phasor_diff2(f2 th, f2 &sn, f2 &c1)
-{
-    const f2 h = mul2(th, bc(0.5f));
-    f2 sh, ch;
-    __sincosf(h.x, &sh.x, &ch.x);
-    __sincosf(h.y, &sh.y, &ch.y);
-    const f2 sh2 = add2(sh, sh);
-    sn = mul2(sh2, ch);
-    c1 = mul2(sh2, sh);
 }
 
 __device__ inline float ln4(const float4 &v, int i) { return i == 0 ? v.x : i == 1 ? v.y : i == 2 ? v.z : v.w; }
@@ -185,18 +160,13 @@ step_tiled_kernel(Lattice L, StepCoef k, int zchunk, int band, const __grid_cons
     // ---- carried from plane z-1: backward z hop and the two plaquettes that contain theta_z(x - z) ----
     R bzr[2] = {0, 0}, bzi[2] = {0, 0};
     float Pyz_c[2] = {0.f, 0.f}, Pzx_c[2] = {0.f, 0.f};
-    f2 bz2r = bc(0.f), bz2i = bc(0.f), Pyz2_c = bc(0.f), Pzx2_c = bc(0.f);        // the same, packed (PK)
+    PkCarry cy = {bc(0.f), bc(0.f), bc(0.f), bc(0.f)};                              // the same, packed (PK)
     if (PK && active) {
         const char *sc = smem, *sp = smem + SLOT_BYTES;          // planes -1 and 0
-        const float4 Ac = A(sc, 0), Bc = B(sc, 0), Bzp = B(sp, 0), Azp = A(sp, 0);
-        const f2 thz = C(sc, 0), Cxp = C(sc, XP), Cyp = C(sc, CYP);
-        const f2 fr = lo(Ac), fi = hi(Ac);
-        f2 sn, c1;
-        phasor_diff2(thz, sn, c1);
-        bz2r = fma2(neg(sn), fi, fma2(neg(c1), fr, sub2(fr, lo(Azp))));
-        bz2i = fma2(sn, fr, fma2(neg(c1), fi, sub2(fi, hi(Azp))));
-        Pyz2_c = plaq2(hi(Bc), Cyp, hi(Bzp), thz);
-        Pzx2_c = plaq2(thz, lo(Bzp), Cxp, lo(Bc));
+        auto pA = [&](int p, int dx, int dy) { return A(p ? sp : sc, dy * COLS + dx); };
+        auto pB = [&](int p, int dx, int dy) { return B(p ? sp : sc, dy * COLS + dx); };
+        auto pC = [&](int p, int dx, int dy) { return C(p ? sp : sc, dy * CCOLS + dx); };
+        pk_carry_init(cy, pA, pB, pC);
     }
     if (!PK && active) {
         const char *sc = smem, *sp = smem + SLOT_BYTES;          // planes -1 and 0
@@ -272,73 +242,11 @@ step_tiled_kernel(Lattice L, StepCoef k, int zchunk, int band, const __grid_cons
         float2 OC;
 
         if constexpr (PK) {
-            // ---- both sectors at once (the scalar chain below, operation by operation, in packed instructions) ----
-            const f2 fr = lo(Ac), fi = hi(Ac);
-            const f2 thx = lo(Bc), thy = hi(Bc), thz = Cc;
-            const f2 thmx = lo(Bxm), thmy = hi(Bym);                             // theta_i(x - i), i = x, y
-            f2 lap_re = bz2r, lap_im = bz2i, J0, J1, J2, sn, c1, dr, di;
-            // x: forward hop, current, backward hop
-            phasor_diff2(thx, sn, c1);
-            dr = fma2(sn, hi(Axp), fma2(neg(c1), lo(Axp), sub2(lo(Axp), fr)));
-            di = fma2(neg(sn), lo(Axp), fma2(neg(c1), hi(Axp), sub2(hi(Axp), fi)));
-            lap_re = add2(lap_re, dr);
-            lap_im = add2(lap_im, di);
-            J0 = fma2(fr, di, neg(mul2(fi, dr)));
-            phasor_diff2(thmx, sn, c1);
-            lap_re = add2(lap_re, fma2(neg(sn), hi(Axm), fma2(neg(c1), lo(Axm), sub2(lo(Axm), fr))));
-            lap_im = add2(lap_im, fma2(sn, lo(Axm), fma2(neg(c1), hi(Axm), sub2(hi(Axm), fi))));
-            // y
-            phasor_diff2(thy, sn, c1);
-            dr = fma2(sn, hi(Ayp), fma2(neg(c1), lo(Ayp), sub2(lo(Ayp), fr)));
-            di = fma2(neg(sn), lo(Ayp), fma2(neg(c1), hi(Ayp), sub2(hi(Ayp), fi)));
-            lap_re = add2(lap_re, dr);
-            lap_im = add2(lap_im, di);
-            J1 = fma2(fr, di, neg(mul2(fi, dr)));
-            phasor_diff2(thmy, sn, c1);
-            lap_re = add2(lap_re, fma2(neg(sn), hi(Aym), fma2(neg(c1), lo(Aym), sub2(lo(Aym), fr))));
-            lap_im = add2(lap_im, fma2(sn, lo(Aym), fma2(neg(c1), hi(Aym), sub2(hi(Aym), fi))));
-            // z: forward hop, current, and the backward z difference of the NEXT plane
-            phasor_diff2(thz, sn, c1);
-            dr = fma2(sn, hi(Azp), fma2(neg(c1), lo(Azp), sub2(lo(Azp), fr)));
-            di = fma2(neg(sn), lo(Azp), fma2(neg(c1), hi(Azp), sub2(hi(Azp), fi)));
-            lap_re = add2(lap_re, dr);
-            lap_im = add2(lap_im, di);
-            J2 = fma2(fr, di, neg(mul2(fi, dr)));
-            bz2r = fma2(neg(sn), fi, fma2(neg(c1), fr, sub2(fr, lo(Azp))));
-            bz2i = fma2(sn, fr, fma2(neg(c1), fi, sub2(fi, hi(Azp))));
-            // potential force (Eq. 17-18): bracket_s = c lambda_s/2 (|f_s|^2 - sigma_s^2) - c kappa (|f_o|^2 - sigma_o^2)
-            const f2 u = sub2(fma2(fr, fr, mul2(fi, fi)), make_float2(k.sig1sq, k.sig2sq));
-            const f2 ku = mul2(bc(k.kap), u);
-            const f2 bracket = fma2(make_float2(k.lamh1, k.lamh2), u, make_float2(-ku.y, -ku.x));
-            const f2 m0 = lo(MA), m1 = hi(MA);
-            const f2 pr = add2(m0, fma2(bc(k.aSm1), m0, mul2(bc(k.bS), fma2(lap_re, bc(k.inv_dx2), neg(mul2(fr, bracket))))));
-            const f2 pi = add2(m1, fma2(bc(k.aSm1), m1, mul2(bc(k.bS), fma2(lap_im, bc(k.inv_dx2), neg(mul2(fi, bracket))))));
-            MA = make_float4(pr.x, pr.y, pi.x, pi.y);
-            const f2 or_ = fma2(bc(k.dtau), pr, fr), oi_ = fma2(bc(k.dtau), pi, fi);
-            OA = make_float4(or_.x, or_.y, oi_.x, oi_.y);
-            // lattice curl of the plaquettes (Eq. 20-21)
-            const f2 Pxy = plaq2(thx, hi(Bxp), lo(Byp), thy);
-            const f2 Pxy_my = plaq2(lo(Bym), hi(Bxpym), thx, thmy);
-            const f2 Pxy_mx = plaq2(thmx, thy, lo(Bxmyp), hi(Bxm));
-            const f2 Pyz = plaq2(thy, Cyp, hi(Bzp), thz);
-            const f2 Pyz_my = plaq2(thmy, thz, hi(Bymzp), Cym);
-            const f2 Pzx = plaq2(thz, lo(Bzp), Cxp, thx);
-            const f2 Pzx_mx = plaq2(Cxm, lo(Bxmzp), thz, thmx);
-            const f2 cc0 = sub2(sub2(Pxy, Pxy_my), sub2(Pzx, Pzx2_c));
-            const f2 cc1 = sub2(sub2(Pyz, Pyz2_c), sub2(Pxy, Pxy_mx));
-            const f2 cc2 = sub2(sub2(Pzx, Pzx_mx), sub2(Pyz, Pyz_my));
-            Pyz2_c = Pyz;
-            Pzx2_c = Pzx;
-            const f2 cur = make_float2(k.cur1, k.cur2);
-            const f2 g0 = lo(MB), g1 = hi(MB), g2 = MC;
-            const f2 e0 = add2(g0, fma2(bc(k.aGm1), g0, mul2(bc(k.bG), fma2(cur, J0, neg(mul2(cc0, bc(k.inv_dx3)))))));
-            const f2 e1 = add2(g1, fma2(bc(k.aGm1), g1, mul2(bc(k.bG), fma2(cur, J1, neg(mul2(cc1, bc(k.inv_dx3)))))));
-            const f2 e2 = add2(g2, fma2(bc(k.aGm1), g2, mul2(bc(k.bG), fma2(cur, J2, neg(mul2(cc2, bc(k.inv_dx3)))))));
-            MB = make_float4(e0.x, e0.y, e1.x, e1.y);
-            MC = e2;
-            const f2 ox = fma2(bc(k.dtau_dx), e0, thx), oy = fma2(bc(k.dtau_dx), e1, thy);
-            OB = make_float4(ox.x, ox.y, oy.x, oy.y);
-            OC = fma2(bc(k.dtau_dx), e2, thz);
+            // both sectors at once in packed fp32x2 instructions (step_site.cuh)
+            auto pA = [&](int p, int dx, int dy) { return A(p ? sp : sc, dy * COLS + dx); };
+            auto pB = [&](int p, int dx, int dy) { return B(p ? sp : sc, dy * COLS + dx); };
+            auto pC = [&](int p, int dx, int dy) { return C(p ? sp : sc, dy * CCOLS + dx); };
+            pk_site_update(cy, pA, pB, pC, k, MA, MB, MC, OA, OB, OC);
         }
 
         const R m2p = (R)Ac.x * (R)Ac.x + (R)Ac.z * (R)Ac.z;

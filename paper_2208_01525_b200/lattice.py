@@ -11,7 +11,8 @@ from . import binding as B
 
 
 class Lattice:
-    def __init__(self, N: int, device: str = "cuda:0", stream=None):
+    def __init__(self, N: int, device: str = "cuda:0", stream=None, aux: bool = False):
+        """aux=True also allocates the second momentum buffer (u1u1_set_aux): step() then takes two steps per pass."""
         import torch
         if not torch.cuda.is_available():
             raise B.U1U1Error("CUDA device required: libu1u1 has no CPU fallback")
@@ -31,6 +32,21 @@ class Lattice:
                                   self.scratch.data_ptr(), cb, self.stream.cuda_stream)
         if rc:
             raise B.U1U1Error(f"u1u1_create: {self.lib.u1u1_last_error(None).decode()}")
+        self.aux = None
+        if aux:
+            self.set_aux(True)
+
+    def set_aux(self, on: bool):
+        """Attach (allocate) or detach (free) the second momentum buffer."""
+        if on and self.aux is None:
+            ab = self.lib.u1u1_aux_bytes(self.N)
+            with self._torch.cuda.device(self.device):
+                buf = self._torch.empty(ab, dtype=self._torch.uint8, device=self.device)
+            self._check(self.lib.u1u1_set_aux(self._ctx, buf.data_ptr(), ab), "set_aux")
+            self.aux = buf
+        elif not on and self.aux is not None:
+            self._check(self.lib.u1u1_set_aux(self._ctx, None, 0), "set_aux")
+            self.aux = None
 
     # -- helpers ---------------------------------------------------------------------------------
     def _check(self, rc, what):
