@@ -384,7 +384,7 @@ extern "C" int u1u1_step(u1u1_ctx *ctx, int32_t n, double tau, double era_m, dou
             TbMaps maps;
             if (ctx->maps_ready) {
                 maps.pos = ctx->pos_halo2[ctx->cur];
-                maps.mom = ctx->mom_halo[ctx->mcur];
+                maps.mom = ctx->mom_tile[ctx->mcur];
             }
             e = launch_step_tb(L, q, q2, ctx->stream, ctx->maps_ready ? &maps : nullptr, ctx->sms);
             ctx->mcur ^= 1;

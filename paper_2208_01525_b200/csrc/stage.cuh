@@ -49,7 +49,7 @@ struct alignas(64) DiagMaps {
     PackMaps pos, mom;
 };
 
-// Tensor maps of one two-step launch: two-site-halo boxes of the positions being read, one-site-halo boxes of the momenta.
+// Tensor maps of one two-step launch: two-site-halo boxes of the positions being read, tile boxes of the momenta.
 struct alignas(64) TbMaps {
     PackMaps pos, mom;
 };

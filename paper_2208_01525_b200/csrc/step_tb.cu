@@ -3,8 +3,8 @@
 // The one-step kernel (step_tiled.cu) moves every site's 20 words through HBM once per step: 160 B per site-update,
 // which is where it saturates.  Here a CTA advances its 32 x 8 tile by two steps before anything
 // goes back to HBM -- 80 B per site-update:
-//   step 1 is evaluated on the tile AND its one-site halo (34 x 10 sites, from positions staged with a TWO-site halo
-//   and momenta staged with a one-site halo); its new positions go to a shared-memory ring, never to HBM;
+//   step 1 is evaluated on the tile AND its one-site halo (34 x 10 sites, from positions staged with a TWO-site halo);
+//   its new positions go to a shared-memory ring, never to HBM;
 //   step 2 is the one-step kernel's body, reading that ring instead of staged HBM planes.
 // Both steps march through the z planes of a chunk together, step 1 one plane ahead of step 2; everything a site needs
 // from the plane below is carried in registers as in the one-step kernel.  A CTA has 8 "inner" warps (one tile site per
@@ -14,7 +14,11 @@
 // Momenta of halo sites belong to neighbouring tiles, which update them in this same launch: the kernel reads momenta
 // from one buffer and writes them to ANOTHER (the caller's aux buffer, u1u1_set_aux).  Redundant work: step 1 runs on
 // 340 / 256 of the sites and on two extra planes per chunk.
+// Shared memory (114 240 B, 2 CTAs per SM): 3 position slots (the two planes step 1 reads + one in flight), 2 momentum
+// slots (tile only; the halo threads prefetch their site's momenta into registers), 3 slots of step-1 positions (the two
+// planes step 2 reads + the one step 1 writes, so one __syncthreads per plane suffices).
 #include <cstring>
+#include <type_traits>
 
 #include "common.cuh"
 #include "kernels.h"
@@ -28,30 +32,26 @@ namespace {
 constexpr int NIN = NTHREADS;                   // 256 inner threads
 constexpr int NHALO = 2 * COLS + 2 * TY;        // 84 halo sites
 constexpr int TB_THREADS = NIN + 96;            // + 3 halo warps
-constexpr int NP = 3;                           // position ring: the two planes step 1 reads + one in flight
-constexpr int OFF_M = NP * P2_SLOT_BYTES;       // momentum ring (one-site halo, slot layout of stage.cuh): 2 slots
-constexpr int OFF_I = OFF_M + 2 * SLOT_BYTES;   // ring of step-1 positions (same slot layout): 2 slots
-constexpr int OFF_BARS = OFF_I + 2 * SLOT_BYTES;
-constexpr int SMEM_BYTES = OFF_BARS + 64;       // 107 712 B -> 2 CTAs per SM
-constexpr int NCP_P = (3 * P2_ELEM + TB_THREADS - 1) / TB_THREADS;      // cp.async copies per thread and plane (4)
-constexpr int NCP_M = (3 * NELEM + TB_THREADS - 1) / TB_THREADS;        // (3)
+constexpr int NP = 3;                           // position ring
+constexpr int MOFF_B = NIN * 16, MOFF_C = NIN * 32, MSLOT_BYTES = NIN * 40;      // momentum slot: MA | MB | MC of the tile
+constexpr int OFF_M = NP * P2_SLOT_BYTES;
+constexpr int OFF_I = OFF_M + 2 * MSLOT_BYTES;  // ring of step-1 positions (one-site halo, slot layout of stage.cuh): 3 slots
+constexpr int OFF_BARS = OFF_I + 3 * SLOT_BYTES;
+constexpr int SMEM_BYTES = OFF_BARS + 64;       // 114 240 B -> 2 CTAs per SM
+constexpr int NCP_P = (3 * P2_ELEM + TB_THREADS - 1) / TB_THREADS;      // cp.async copies per thread and position plane (4)
 static_assert(OFF_M % 128 == 0 && OFF_I % 128 == 0 && OFF_BARS % 8 == 0, "alignment");
+static_assert(2 * (SMEM_BYTES + 1024) <= 233472, "two CTAs per SM");
 
-__global__ void __launch_bounds__(TB_THREADS, 2)
-step_tb_kernel(TbLattice L, StepCoef k1, StepCoef k2, int zchunk, int band, const __grid_constant__ TbMaps maps)
+// TMA: the tile's two-site halo lies inside the lattice, positions and momenta arrive by TMA boxes; otherwise
+// (boundary / ragged tiles) by per-thread cp.async with the periodic wrap resolved in a per-thread plan.
+template <bool TMA>
+__device__ __forceinline__ void tb_tile(const TbLattice &L, const StepCoef &k1, const StepCoef &k2, const TbMaps &maps, char *smem,
+                                        int x0, int y0, int z0, int wx, int wy, int nz)
 {
-    extern __shared__ __align__(128) char smem[];
     const unsigned sbase = smem_u32(smem), bars = sbase + OFF_BARS;
     const int N = L.N;
     const size_t V = L.V, NN = (size_t)N * N;
     const int tid = threadIdx.x;
-    // (tile, z chunk) of this CTA in band order (step_tiled.cu)
-    const int ntx = (N + TX - 1) / TX, nty = (N + TY - 1) / TY, nzc = (N + zchunk - 1) / zchunk;
-    const int full = ntx * band * nzc, bnd = blockIdx.x / full, rem = blockIdx.x - bnd * full;
-    const int rows = min(band, nty - bnd * band), bzc = rem / (ntx * rows), tl = rem - bzc * (ntx * rows);
-    const int x0 = (tl % ntx) * TX, y0 = (bnd * band + tl / ntx) * TY, z0 = bzc * zchunk;
-    const int wx = min(TX, N - x0), wy = min(TY, N - y0), nz = min(zchunk, N - z0);
-    const bool tma = !(k1.flags & 2) && x0 >= 2 && x0 + TX + 2 <= N && y0 >= 2 && y0 + TY + 2 <= N;     // CTA-uniform
 
     // ---- this thread's step-1 site (c1, r1) relative to the tile origin; inner threads also own it in step 2 ----
     const bool inner = tid < NIN;
@@ -60,7 +60,7 @@ step_tb_kernel(TbLattice L, StepCoef k1, StepCoef k2, int zchunk, int band, cons
     if (inner) {
         c1 = tid & (TX - 1);
         r1 = tid / TX;
-        act = c1 < wx && r1 < wy;
+        act = TMA || (c1 < wx && r1 < wy);
     } else {
         const int h = tid - NIN;
         if (h < COLS) { c1 = h - 1; r1 = -1; act = c1 <= wx; }
@@ -70,30 +70,26 @@ step_tb_kernel(TbLattice L, StepCoef k1, StepCoef k2, int zchunk, int band, cons
     }
     const int eP = (r1 + 2) * P2_COLS + c1 + 2;                        // element index in a position slot (two-site halo)
     const int eI = (r1 + 1) * COLS + c1 + 1, eIC = (r1 + 1) * CCOLS + c1 + 2;      // in a one-site-halo slot (packs A, B / pack C)
-    const size_t gsite = (size_t)(y0 + r1) * N + (size_t)(x0 + c1);   // inner threads only
+    // in-plane site index: the own site of an inner thread (output), the periodic image of a halo thread's site (momenta)
+    const size_t gsite = (size_t)wrapi(y0 + r1, N) * N + (size_t)wrapi(x0 + c1, N);
 
     // ---- staging ----
     // running plane counters: position plane pp = 0 .. nz+3 is relative plane pp - 2, momentum plane mm = 0 .. nz+1 is
     // relative plane mm - 1; ring slot = pp % 3 resp. mm & 1
     const char *posb = reinterpret_cast<const char *>(L.pos_in), *momb = reinterpret_cast<const char *>(L.mom_in);
-    const unsigned long long pol_keep = policy_evict_last();
-    int planP[NCP_P], planM[NCP_M];           // cp.async path: in-plane site of each of this thread's copies (-1: none)
-    if (!tma) {
+    const unsigned long long pol_keep = policy_evict_last(), pol_stream = policy_evict_first();
+    int planP[NCP_P];                         // cp.async path: in-plane site of each of this thread's copies (-1: none)
+    if (!TMA) {
 #pragma unroll
         for (int q = 0; q < NCP_P; q++) {
             const int item = tid + q * TB_THREADS, pack = item / P2_ELEM, e = item - pack * P2_ELEM, r = e / P2_COLS, c = e - r * P2_COLS;
             planP[q] = (pack < 3 && r <= wy + 3 && c <= wx + 3) ? wrapi(y0 - 2 + r, N) * N + wrapi(x0 - 2 + c, N) : -1;
         }
-#pragma unroll
-        for (int q = 0; q < NCP_M; q++) {
-            const int item = tid + q * TB_THREADS, pack = item / NELEM, e = item - pack * NELEM, r = e / COLS, c = e - r * COLS;
-            planM[q] = (pack < 3 && r <= wy + 1 && c <= wx + 1) ? wrapi(y0 - 1 + r, N) * N + wrapi(x0 - 1 + c, N) : -1;
-        }
     }
     auto stage_P = [&](int pp, unsigned slot) {       // TMA: one thread; cp.async: every thread (caller commits)
         const int z = wrapi(z0 + pp - 2, N);
         const unsigned dst = sbase + slot * P2_SLOT_BYTES;
-        if (tma) {
+        if (TMA) {
             const unsigned bar = bars + 8 * slot;
             mbar_expect_tx(bar, P2_SLOT_BYTES);
             tma_load_3d_hint(dst, &maps.pos.A, 4 * (x0 - 2), y0 - 2, z, bar, pol_keep);
@@ -111,24 +107,32 @@ step_tb_kernel(TbLattice L, StepCoef k1, StepCoef k2, int zchunk, int band, cons
             }
         }
     };
-    auto stage_M = [&](int mm) {
+    auto stage_M = [&](int mm) {                      // the tile's momenta of relative plane mm - 1
         const int z = wrapi(z0 + mm - 1, N);
-        const unsigned dst = sbase + OFF_M + (mm & 1) * SLOT_BYTES;
-        if (tma) {
-            stage_plane_tma(maps.mom, x0, y0, z, dst, bars + 8 * (NP + (mm & 1)), pol_keep);
-        } else {
-#pragma unroll
-            for (int q = 0; q < NCP_M; q++) {
-                if (planM[q] < 0) continue;
-                const int item = tid + q * TB_THREADS, pack = item / NELEM, e = item - pack * NELEM;
-                const size_t site = (size_t)z * NN + (size_t)planM[q];
-                if (pack == 0) cp_async16(dst + e * 16, momb + site * 16);
-                else if (pack == 1) cp_async16(dst + OFF_B + e * 16, momb + 16 * V + site * 16);
-                else cp_async8(dst + OFF_C + (e + 2 * (e / COLS) + 1) * 8, momb + 32 * V + site * 8);
-            }
+        const unsigned dst = sbase + OFF_M + (mm & 1) * MSLOT_BYTES;
+        if (TMA) {
+            const unsigned bar = bars + 8 * (NP + (mm & 1));
+            mbar_expect_tx(bar, MSLOT_BYTES);
+            tma_load_3d_hint(dst, &maps.mom.A, 4 * x0, y0, z, bar, pol_keep);
+            tma_load_3d_hint(dst + MOFF_B, &maps.mom.B, 4 * x0, y0, z, bar, pol_keep);
+            tma_load_3d_hint(dst + MOFF_C, &maps.mom.C, 2 * x0, y0, z, bar, pol_keep);
+        } else if (inner && act) {
+            const size_t site = (size_t)z * NN + gsite;
+            cp_async16(dst + tid * 16, momb + site * 16);
+            cp_async16(dst + MOFF_B + tid * 16, momb + 16 * V + site * 16);
+            cp_async8(dst + MOFF_C + tid * 8, momb + 32 * V + site * 8);
         }
     };
-    const bool issuer = !tma || tid == 0;
+    const bool issuer = !TMA || tid == 0;
+    // halo threads: the momenta of their site in relative plane mm - 1, straight into registers one plane ahead
+    float4 MAo = make_float4(0.f, 0.f, 0.f, 0.f), MBo = MAo;        // inner threads: step-1 momenta of the plane step 2 works on next
+    float2 MCo = make_float2(0.f, 0.f);
+    auto prefetch_M = [&](int mm) {
+        const size_t lin = (size_t)wrapi(z0 + mm - 1, N) * NN + gsite;
+        MAo = __ldg(reinterpret_cast<const float4 *>(L.mom_in) + lin);
+        MBo = __ldg(reinterpret_cast<const float4 *>(L.mom_in + 4 * V) + lin);
+        MCo = __ldg(reinterpret_cast<const float2 *>(L.mom_in + 8 * V) + lin);
+    };
 
     // accessors of pk_site_update (A / B / C of the site displaced by (dx, dy) in plane p = 0 or 1): step 1 reads two
     // position slots (two-site halo, pitch P2_COLS), step 2 two slots of step-1 positions (one-site halo, stage.cuh layout)
@@ -142,7 +146,7 @@ step_tb_kernel(TbLattice L, StepCoef k1, StepCoef k2, int zchunk, int band, cons
     auto fC = [&](int p, int dx, int dy) { return *reinterpret_cast<const float2 *>((p ? (P1) : (P0)) + OFF_C + (eIC + dy * CCOLS + dx) * 8); }
 
     // ---- prologue: position planes 0, 1, 2 and momentum planes 0, 1 in flight; step-1 carry from planes 0, 1 ----
-    if (tma) {
+    if (TMA) {
         if (tid == 0) {
 #pragma unroll
             for (int b = 0; b < NP + 2; b++) mbar_init(bars + 8 * b, 1);
@@ -157,7 +161,8 @@ step_tb_kernel(TbLattice L, StepCoef k1, StepCoef k2, int zchunk, int band, cons
         stage_M(0);
         stage_M(1);
     }
-    if (tma) {
+    if (!inner && act) prefetch_M(0);
+    if (TMA) {
         mbar_wait(bars + 0, 0);
         mbar_wait(bars + 8, 0);
     } else {
@@ -172,45 +177,52 @@ step_tb_kernel(TbLattice L, StepCoef k1, StepCoef k2, int zchunk, int band, cons
         pk_carry_init(cy1, fA, fB, fC);
     }
     __syncthreads();                          // everybody is done with position plane 0: its slot takes plane 3
-    if (issuer && 3 <= nz + 3) stage_P(3, 0);
-    if (!tma) cp_async_commit();
+    if (issuer) stage_P(3, 0);
+    if (!TMA) cp_async_commit();
 
-    float4 MAo = make_float4(0.f, 0.f, 0.f, 0.f), MBo = MAo;        // step-1 momenta of the plane step 2 works on next
-    float2 MCo = make_float2(0.f, 0.f);
     unsigned sP = 1;                          // ring slot of position plane t + 1
-    char *iCur = smem + OFF_I, *iPrev = smem + OFF_I + SLOT_BYTES;       // slots of step-1 planes t and t - 1
+    char *iCur = smem + OFF_I, *iPrev = smem + OFF_I + SLOT_BYTES, *iFree = smem + OFF_I + 2 * SLOT_BYTES;   // step-1 planes t, t-1, t-2
     // iteration t: step 1 on relative plane t - 1 (position planes t+1, t+2; momentum plane t), then step 2 on relative
     // plane t - 2 (step-1 planes t-1, t)
     for (int t = 0; t <= nz + 1; t++) {
         const unsigned sP1 = sP == 2u ? 0u : sP + 1u;                // slot of position plane t + 2
-        if (tma) {
+        if (TMA) {
             mbar_wait(bars + 8 * sP1, ((unsigned)(t + 2) / 3u) & 1u);
-            mbar_wait(bars + 8 * (NP + (t & 1)), (unsigned)(t >> 1) & 1u);
+            if (inner) mbar_wait(bars + 8 * (NP + (t & 1)), (unsigned)(t >> 1) & 1u);
         }
         // ---- (a) step 1 of this thread's site in relative plane t - 1 ----
         float4 MA = make_float4(0.f, 0.f, 0.f, 0.f), MB = MA;
         float2 MC = make_float2(0.f, 0.f);
-        char *si = iCur;
         if (act) {
-            const char *ms = smem + OFF_M + (t & 1) * SLOT_BYTES;
-            MA = *reinterpret_cast<const float4 *>(ms + eI * 16);
-            MB = *reinterpret_cast<const float4 *>(ms + OFF_B + eI * 16);
-            MC = *reinterpret_cast<const float2 *>(ms + OFF_C + eIC * 8);
+            if (inner) {
+                const char *ms = smem + OFF_M + (t & 1) * MSLOT_BYTES;
+                MA = *reinterpret_cast<const float4 *>(ms + tid * 16);
+                MB = *reinterpret_cast<const float4 *>(ms + MOFF_B + tid * 16);
+                MC = *reinterpret_cast<const float2 *>(ms + MOFF_C + tid * 8);
+            } else {
+                MA = MAo;
+                MB = MBo;
+                MC = MCo;
+                if (t + 1 <= nz + 1) prefetch_M(t + 1);
+            }
             const char *p0 = smem + sP * P2_SLOT_BYTES, *p1 = smem + sP1 * P2_SLOT_BYTES;
             TB_ACC1(p0, p1);
             float4 OA, OB;
             float2 OC;
             pk_site_update(cy1, fA, fB, fC, k1, MA, MB, MC, OA, OB, OC);
-            *reinterpret_cast<float4 *>(si + eI * 16) = OA;
-            *reinterpret_cast<float4 *>(si + OFF_B + eI * 16) = OB;
-            *reinterpret_cast<float2 *>(si + OFF_C + eIC * 8) = OC;
+            *reinterpret_cast<float4 *>(iCur + eI * 16) = OA;
+            *reinterpret_cast<float4 *>(iCur + OFF_B + eI * 16) = OB;
+            *reinterpret_cast<float2 *>(iCur + OFF_C + eIC * 8) = OC;
         }
-        __syncthreads();                      // step-1 plane t complete; position plane t+1 and momentum plane t are consumed
+        if (!TMA) cp_async_wait<0>();         // the copies issued one iteration ago have landed
+        // the one barrier of the iteration: step-1 plane t is complete; position plane t+1 and momentum plane t are consumed;
+        // everybody is past step 2 of the previous iteration, whose older step-1 plane the NEXT iteration overwrites
+        __syncthreads();
         if (issuer) {
             if (t + 4 <= nz + 3) stage_P(t + 4, sP);
             if (t + 2 <= nz + 1) stage_M(t + 2);
         }
-        if (!tma) cp_async_commit();
+        if (!TMA) cp_async_commit();
 
         // ---- (b) step 2 of the inner sites in relative plane t - 2 ----
         if (inner && act && t >= 1) {
@@ -230,17 +242,38 @@ step_tb_kernel(TbLattice L, StepCoef k1, StepCoef k2, int zchunk, int band, cons
                 __stcs(reinterpret_cast<float2 *>(L.pos_out + 8 * V) + lin, OC);
             }
         }
-        MAo = MA;
-        MBo = MB;
-        MCo = MC;
+        if (inner) {
+            MAo = MA;
+            MBo = MB;
+            MCo = MC;
+        }
         sP = sP1;
-        char *sw = iCur;
-        iCur = iPrev;
-        iPrev = sw;
-        if (!tma) cp_async_wait<1>();         // the copies issued one iteration ago have landed
-        __syncthreads();                      // step-1 plane t-1 is consumed: the next iteration overwrites its slot
+        char *sw = iFree;                     // rotate the step-1 ring: the slot of plane t-2 is written next
+        iFree = iPrev;
+        iPrev = iCur;
+        iCur = sw;
     }
-    if (!tma) cp_async_wait<0>();
+    if (!TMA) cp_async_wait<0>();
+#undef TB_ACC1
+#undef TB_ACC2
+}
+
+__global__ void __launch_bounds__(TB_THREADS, 2)
+step_tb_kernel(TbLattice L, StepCoef k1, StepCoef k2, int zchunk, int band, const __grid_constant__ TbMaps maps)
+{
+    extern __shared__ __align__(128) char smem[];
+    const int N = L.N;
+    // (tile, z chunk) of this CTA in band order (step_tiled.cu)
+    const int ntx = (N + TX - 1) / TX, nty = (N + TY - 1) / TY, nzc = (N + zchunk - 1) / zchunk;
+    const int full = ntx * band * nzc, bnd = blockIdx.x / full, rem = blockIdx.x - bnd * full;
+    const int rows = min(band, nty - bnd * band), bzc = rem / (ntx * rows), tl = rem - bzc * (ntx * rows);
+    const int x0 = (tl % ntx) * TX, y0 = (bnd * band + tl / ntx) * TY, z0 = bzc * zchunk;
+    const int nz = min(zchunk, N - z0);
+    // CTA-uniform choice of the staging path
+    if (!(k1.flags & 2) && x0 >= 2 && x0 + TX + 2 <= N && y0 >= 2 && y0 + TY + 2 <= N)
+        tb_tile<true>(L, k1, k2, maps, smem, x0, y0, z0, TX, TY, nz);
+    else
+        tb_tile<false>(L, k1, k2, maps, smem, x0, y0, z0, min(TX, N - x0), min(TY, N - y0), nz);
 }
 
 }  // namespace
