@@ -43,7 +43,8 @@ def workload_name(n, prephase=PREPHASE_STEPS):
             f"{DIAG_EVERY} steps (BASELINE.json config 5)")
 
 
-TRAFFIC_SOURCES = ("step_tiled.cu", "stage.cuh", "common.cuh")      # what the measured DRAM traffic depends on
+# what the measured DRAM traffic depends on: the sources of the step kernels
+TRAFFIC_SOURCES = ("step_tiled.cu", "step_tb.cu", "step_site.cuh", "stage.cuh", "common.cuh")
 
 
 def csrc_sha():
@@ -56,13 +57,13 @@ def csrc_sha():
     return h.hexdigest()[:16]
 
 
-def measured_traffic(N):
-    """DRAM bytes per launch of the step kernel from profiles/traffic.json, or None if that file was measured on other
-    sources than the ones being timed (the number would be stale)."""
+def measured_traffic(N, two_step):
+    """DRAM bytes per launch of the step kernel (one step, or two steps per pass) from profiles/traffic.json, or None if
+    that file was measured on other sources than the ones being timed (the number would be stale)."""
     try:
         with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
             t = json.load(f)
-        return t.get(f"step_{N}") if t.get("csrc_sha") == csrc_sha() else None
+        return t.get(f"step_tb_{N}" if two_step else f"step_{N}") if t.get("csrc_sha") == csrc_sha() else None
     except Exception:
         return None
 
@@ -209,7 +210,15 @@ def run_ours(args):
     build.build()
     N = args.size
     V = N ** 3
-    lat = Lattice(N, device=f"cuda:{local}", aux=bool(args.tb))
+    lat = Lattice(N, device=f"cuda:{local}")
+    two_step = False
+    if args.tb:
+        # the second momentum buffer (43 GB at 1024^3, 172 + 11 GB in all): u1u1_step then takes two steps per pass
+        try:
+            lat.set_aux(True)
+            two_step = True
+        except Exception as e:          # not enough HBM: the one-step kernel
+            print(f"bench.py: aux buffer not available ({e}); one step per pass", file=sys.stderr)
     prm = Params(tau_norm=256.0, friction=0.5, kernel_variant=args.variant)
     lat.init_fields(replica_seed(rank), DX, prm)
     lat.step(args.prephase, TAU0, ERA, S)                    # damped prephase (config 5: 200 steps)
@@ -255,8 +264,11 @@ def run_ours(args):
     ms_total, ms_steps, ms_diag = max_over_ranks([ms_total, ms_steps, ms_diag], dist, f"cuda:{local}")
     value = whole_job_rate(world, args.steps, V, ms_total)
     kernel_ms = ms_steps / args.steps
+    step_launches = launches - 4 * len(dsegs)                # a diagnostics call is 4 launches (sweep, fold, overlap, fold)
+    steps_per_launch = args.steps / step_launches
     achieved = BYTES_PER_SITE_UPDATE * V / (kernel_ms * 1e-3) / 1e9
     peak, peak_src = measured_peak_gbs()
+    traffic = measured_traffic(N, two_step)
 
     e2e = run_e2e(args, lat, tau, world, dist, local)
 
@@ -275,15 +287,23 @@ def run_ours(args):
         "value_steps_only": whole_job_rate(world, args.steps, V, ms_steps),
         "value_at_config_cadence": whole_job_rate(world, DIAG_EVERY, V, DIAG_EVERY * kernel_ms + ms_diag),
         "diagnostics_ms": ms_diag,
-        "config": {"workload": workload_name(N, args.prephase), "N": N, "state_GB": 120 * V / 1e9,
-                   "l2_policy": "inputs (129 GB state) far larger than the 126 MB L2; no flush needed",
+        "config": {"workload": workload_name(N, args.prephase), "N": N, "state_GB": (160 if two_step else 120) * V / 1e9,
+                   "l2_policy": "inputs (129 GB state + 43 GB second momentum buffer) far larger than the 126 MB L2; no flush needed",
                    "prephase_steps_before_timing": args.prephase, "diag_calls_in_timed_region": len(dsegs),
                    "diag_every": DIAG_EVERY, "diag_every_effective": args.steps / len(dsegs),
-                   "kernel_variant": args.variant, "parallelism": "replicas" if world > 1 else "single"},
+                   "kernel_variant": args.variant, "two_steps_per_pass": two_step,
+                   "parallelism": "replicas" if world > 1 else "single"},
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": measured_traffic(N), "traffic_csrc_sha": csrc_sha(), "peak_source": peak_src,
-                     "kernel": "fused kick+drift step", "kernel_ms": kernel_ms,
-                     "bytes_per_site_update": BYTES_PER_SITE_UPDATE, "frac_of_8TBs_spec": achieved / 8000.0,
+                     "traffic": traffic, "traffic_csrc_sha": csrc_sha(), "peak_source": peak_src,
+                     "kernel": ("two fused kick+drift steps per pass (step_tb_kernel): 80 B of HBM traffic per site-update, "
+                                "so the fraction of the 160 B/site-update roofline can exceed 1") if two_step
+                               else "fused kick+drift step (step_tiled_kernel)",
+                     "kernel_ms": kernel_ms, "launch_ms": kernel_ms * steps_per_launch, "steps_per_launch": steps_per_launch,
+                     "bytes_per_site_update": BYTES_PER_SITE_UPDATE,
+                     "algorithmic_bytes_per_launch": BYTES_PER_SITE_UPDATE * V * steps_per_launch,
+                     "dram_GBs": (traffic / (kernel_ms * steps_per_launch * 1e-3) / 1e9) if traffic else None,
+                     "dram_frac_of_peak": (traffic / (kernel_ms * steps_per_launch * 1e-3) / 1e9 / peak) if traffic else None,
+                     "frac_of_8TBs_spec": achieved / 8000.0,
                      "diagnostics": {"kernel": "fused diagnostics sweep + tolerant overlap", "ms": ms_diag,
                                      "algorithmic_bytes": 80 * V, "achieved": 80 * V / (ms_diag * 1e-3) / 1e9,
                                      "frac": 80 * V / (ms_diag * 1e-3) / 1e9 / peak}},

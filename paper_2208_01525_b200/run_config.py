@@ -29,7 +29,7 @@ KEYS = ("tau", "a", "xi_W", "xi_p", "xi_q", "xi_pq", "xi_L", "v2_L", "v2_pq", "f
 
 
 def run(config: int, size: int | None = None, variant: int = 0, segments: bool = False, device: str = "cuda:0",
-        emit=print):
+        emit=print, aux: bool = True):
     import torch
     c = dict(CONFIGS[config])
     N = size or c["N"]
@@ -39,6 +39,11 @@ def run(config: int, size: int | None = None, variant: int = 0, segments: bool =
     tau_end = TAU0 + total * DTAU
     tau_norm = c["tau_norm"] if c["tau_norm"] is not None else tau_end
     lat = Lattice(N, device=device)
+    if aux:                                          # second momentum buffer: two steps per pass (same bits, faster)
+        try:
+            lat.set_aux(True)
+        except Exception:
+            pass
     prm = Params(init_kind=c["kind"], tau_norm=tau_norm, friction=0.5 if c["pre"] else 1.0, kernel_variant=variant)
     lat.init_fields(config, DX, prm)
     torch.cuda.synchronize()
@@ -78,9 +83,10 @@ def main():
     ap.add_argument("--config", type=int, default=1, choices=sorted(CONFIGS))
     ap.add_argument("--size", type=int, default=None)
     ap.add_argument("--variant", type=int, default=0)
+    ap.add_argument("--no-aux", action="store_true", help="one step per pass (no second momentum buffer)")
     ap.add_argument("--segments", action="store_true", help="also label the pq segments (min 8 cells, one-cell tolerance)")
     a = ap.parse_args()
-    run(a.config, a.size, a.variant, a.segments)
+    run(a.config, a.size, a.variant, a.segments, aux=not a.no_aux)
 
 
 if __name__ == "__main__":
