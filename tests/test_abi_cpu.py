@@ -35,6 +35,9 @@ def test_size_queries(lib):
     assert lib.u1u1_state_bytes(64) == 30 * 64 ** 3 * 4
     assert lib.u1u1_state_bytes(1024) == 30 * 1024 ** 3 * 4          # 128.8 GB: fits 180 GB HBM3e
     assert lib.u1u1_scratch_bytes(64) >= 8 * 64 ** 3
+    assert lib.u1u1_aux_bytes(64) == 10 * 64 ** 3 * 4 and lib.u1u1_aux_bytes(66) == 0
+    # state + second momentum buffer + scratch at 1024^3 fit the 178.4 GiB a B200 reports
+    assert lib.u1u1_state_bytes(1024) + lib.u1u1_aux_bytes(1024) + lib.u1u1_scratch_bytes(1024) < 172 * 2 ** 30
     for bad in (0, 4, 7, 66, 1028, -8):
         assert lib.u1u1_state_bytes(bad) == 0 and lib.u1u1_scratch_bytes(bad) == 0
 
@@ -95,6 +98,9 @@ int main(void)
     p.lambda1 = p.lambda2 = 2.0; p.e1 = p.e2 = 1.0; p.eta1 = p.eta2 = 1.0; p.kappa = 0.9;
     p.dtau = 0.1; p.tau_norm = 1.0; p.friction = 1.0; p.smooth_width = 5.0; p.smooth_trunc = 20;
     if (u1u1_step(ctx, 1, 1.0, 0.5, 1.0) != U1U1_ESTATE) return 7;
+    if (u1u1_aux_bytes(64) != (size_t)10 * 64 * 64 * 64 * 4) return 20;
+    if (u1u1_set_aux(NULL, NULL, 0) != U1U1_EINVAL) return 21;
+    if (u1u1_set_aux(ctx, (void *)0x30001, (size_t)1 << 20) != U1U1_ESIZE) return 22;      /* misaligned */
     if (u1u1_configure(ctx, 16, 0.5, &p) != U1U1_ESIZE) return 8;
     p.kappa = 1.0;
     if (u1u1_configure(ctx, 8, 0.5, &p) != U1U1_EPARAM) return 9;
