@@ -88,8 +88,8 @@ size_t u1u1_scratch_bytes(int32_t N);
  * block evaluates step 1 on its tile plus a one-site halo into shared memory and step 2 from there, so each site's 20
  * words make one HBM round trip per two steps (80 B per site-update instead of 160).  That kernel reads the halo
  * sites' momenta while neighbouring blocks update theirs, hence momenta go from one buffer to the other; the library
- * tracks which one is current.  Results are bit-identical to the one-step kernel's.  Cubic lattices, kernel_variant 0;
- * an odd last step of a call takes the one-step kernel.  May be called before or after u1u1_configure; must hold
+ * tracks which one is current.  Results are bit-identical to the one-step kernel's.  Cubic lattices, kernel_variant 0,
+ * u1u1_step and u1u1_cool; an odd last step of a call takes the one-step kernel.  May be called before or after u1u1_configure; must hold
  * u1u1_aux_bytes(N).  1024^3: 43 GB on top of the 129 GB state (fits the 180 GB of a B200). */
 size_t u1u1_aux_bytes(int32_t N);
 int u1u1_set_aux(u1u1_ctx *ctx, void *aux_dev, size_t aux_bytes);

@@ -313,6 +313,30 @@ static cudaError_t launch_step(u1u1_ctx *ctx, const StepCoef &q)
     return launch_step_tiled(L, q, ctx->stream, tiled_mode(kv), ctx->maps_ready ? &maps : nullptr, ctx->sms);
 }
 
+// Two steps per pass (step_tb.cu) whenever the caller has provided the second momentum buffer (u1u1_set_aux): default
+// kernel variant, cubic lattice; tuning flags 1 (scalar chain) and 256 keep the one-step kernel.
+static bool pairs_enabled(const u1u1_ctx *ctx)
+{
+    const int kv = ctx->prm.kernel_variant;
+    return ctx->aux && !ctx->nz_own && (kv & 15) == 0 && !((kv >> 4) & (1 | 256)) && step_tb_supports(ctx->N);
+}
+
+// one launch, two steps: positions to the other ping-pong buffer, momenta from the current to the other momentum buffer
+static cudaError_t launch_two_steps(u1u1_ctx *ctx, const StepCoef &q1, const StepCoef &q2)
+{
+    TbLattice L{pos_buf(ctx, ctx->cur), pos_buf(ctx, ctx->cur ^ 1), mom_buf_at(ctx, ctx->mcur), mom_buf_at(ctx, ctx->mcur ^ 1),
+                ctx->V, ctx->N};
+    TbMaps maps;
+    if (ctx->maps_ready) {
+        maps.pos = ctx->pos_halo2[ctx->cur];
+        maps.mom = ctx->mom_tile[ctx->mcur];
+    }
+    cudaError_t e = launch_step_tb(L, q1, q2, ctx->stream, ctx->maps_ready ? &maps : nullptr, ctx->sms);
+    ctx->mcur ^= 1;
+    ctx->cur ^= 1;
+    return e;
+}
+
 // calls that read z neighbours through the periodic wrap of a cubic buffer are not available on a z slab
 static int cubic_only(u1u1_ctx *ctx, const char *what)
 {
@@ -365,10 +389,7 @@ extern "C" int u1u1_step(u1u1_ctx *ctx, int32_t n, double tau, double era_m, dou
         q.flags = P.kernel_variant >> 4;
         return U1U1_OK;
     };
-    // Two steps per pass (step_tb.cu) whenever the caller has provided the second momentum buffer (u1u1_set_aux): default
-    // kernel variant, cubic lattice; tuning flag 256 keeps the one-step kernel.  An odd last step takes the one-step kernel.
-    const bool pairs = ctx->aux && !ctx->nz_own && (P.kernel_variant & 15) == 0 && !((P.kernel_variant >> 4) & (1 | 256)) &&
-                       step_tb_supports(ctx->N);
+    const bool pairs = pairs_enabled(ctx);      // an odd last step takes the one-step kernel
     for (int k = 0; k < n;) {
         const double tk = tau + k * dt;
         StepCoef q, q2;
@@ -379,22 +400,14 @@ extern "C" int u1u1_step(u1u1_ctx *ctx, int32_t n, double tau, double era_m, dou
         cudaError_t e;
         if (pairs && k + 1 < n) {
             if (int rc = coef_at(tau + (k + 1) * dt, q2, c, delta, omega)) return rc;
-            TbLattice L{pos_buf(ctx, ctx->cur), pos_buf(ctx, ctx->cur ^ 1), mom_buf_at(ctx, ctx->mcur), mom_buf_at(ctx, ctx->mcur ^ 1),
-                        ctx->V, ctx->N};
-            TbMaps maps;
-            if (ctx->maps_ready) {
-                maps.pos = ctx->pos_halo2[ctx->cur];
-                maps.mom = ctx->mom_tile[ctx->mcur];
-            }
-            e = launch_step_tb(L, q, q2, ctx->stream, ctx->maps_ready ? &maps : nullptr, ctx->sms);
-            ctx->mcur ^= 1;
+            e = launch_two_steps(ctx, q, q2);
             done = 2;
         } else {
             e = launch_step(ctx, q);
+            ctx->cur ^= 1;
         }
         if (e != cudaSuccess) return cuda_fail(ctx, e, "step kernel launch");
         ctx->launches += 1;
-        ctx->cur ^= 1;
         k += done;
         ctx->tau_pos = (tau + (k - 1) * dt) + dt;         // start of the last step taken + dtau
         // weights for the diagnostics of the state just produced
@@ -438,11 +451,19 @@ extern "C" int u1u1_cool(u1u1_ctx *ctx, int32_t n, double dcool)
     q.dtau = (float)dcool;
     q.dtau_dx = (float)(dcool * dx);
     q.flags = P.kernel_variant >> 4;
-    for (int k = 0; k < n; k++) {
-        cudaError_t e = launch_step(ctx, q);
+    const bool pairs = pairs_enabled(ctx);
+    for (int k = 0; k < n;) {
+        cudaError_t e;
+        if (pairs && k + 1 < n) {
+            e = launch_two_steps(ctx, q, q);
+            k += 2;
+        } else {
+            e = launch_step(ctx, q);
+            ctx->cur ^= 1;
+            k += 1;
+        }
         if (e != cudaSuccess) return cuda_fail(ctx, e, "cooling kernel launch");
         ctx->launches += 1;
-        ctx->cur ^= 1;
         invalidate(ctx);
     }
     if (n > 0) {

@@ -77,6 +77,23 @@ def test_aux_attach_detach_keeps_the_state():
     assert np.array_equal(a, lat.export_state().cpu().numpy().astype(np.float64))
 
 
+def test_cooling_two_steps_per_pass_bit_identical():
+    """u1u1_cool (Eq. 27-30 in the same kernels) also takes two steps per pass: the paper's IC pipeline -- random phases,
+    cooling (odd count), damping, evolution -- gives the same bits with and without the aux buffer."""
+    from paper_2208_01525_b200 import Lattice, Params
+    N = 72
+    outs = []
+    for aux in (False, True):
+        lat = Lattice(N, aux=aux)
+        lat.init_fields(3, DX, Params(eta2=1.1, kappa=0.6))
+        lat.cool(11, 1.0 / 30.0)
+        lat.step(6, 1.0, 0.95, 0.0)
+        lat.step(5, 1.6, 0.5, 1.0)
+        outs.append((lat.export_state().cpu().numpy(), lat.diagnostics()["sumW_p"]))
+    assert np.array_equal(outs[0][0], outs[1][0]) and outs[0][1] == outs[1][1]
+    assert np.all(np.isfinite(outs[0][0]))
+
+
 def test_full_size_two_steps_per_pass_tiled_state():
     """1024^3 in the launch configuration bench.py times: a periodic tiling of a 64^3 state evolves as the tiling of the
     64^3 evolution, so every diagnostic count / sum scales by 4096 exactly and sampled blocks are bit-identical."""
