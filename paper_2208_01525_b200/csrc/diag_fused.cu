@@ -22,6 +22,7 @@
 #include "common.cuh"
 #include "kernels.h"
 #include "stage.cuh"
+#include "f32x2.cuh"
 #include "winding.cuh"
 
 namespace u1u1 {
@@ -31,7 +32,7 @@ namespace {
 constexpr int NSLOT = 3;                                   // position ring: planes z, z+1 in use, z+2 in flight
 constexpr int MSLOT_BYTES = 5504;                          // momentum ring slot: pack B (E_x, E_y, H_x, H_y) with halo
 constexpr int OFF_MRING = NSLOT * SLOT_BYTES;
-constexpr int OFF_ALPHA = OFF_MRING + 2 * MSLOT_BYTES;     // float [2 planes][2 sectors][NELEM]
+constexpr int OFF_ALPHA = OFF_MRING + 2 * MSLOT_BYTES;     // float2 [2 planes][NELEM]: the phases (alpha_p, alpha_q) of a site
 constexpr int OFF_XY = OFF_ALPHA + 2 * 2 * NELEM * 4;      // uint2 [2 planes][NELEM]: wrap counts of the x and y links
 constexpr int OFF_Z = OFF_XY + 2 * NELEM * 8;              // uint  [NELEM]: wrap counts of the z links of plane z
 constexpr int OFF_RED = OFF_Z + NELEM * 4;                 // double [FUSED_NRES][NTHREADS / 32]: per-warp accumulators
@@ -51,7 +52,7 @@ diag_fused_kernel(const float *__restrict__ posp, const float *__restrict__ momp
 {
     extern __shared__ __align__(128) char smem[];
     const unsigned sbase = smem_u32(smem), bars = sbase + OFF_BARS;
-    float *alpha = reinterpret_cast<float *>(smem + OFF_ALPHA);
+    float2 *alpha = reinterpret_cast<float2 *>(smem + OFF_ALPHA);
     uint2 *XY = reinterpret_cast<uint2 *>(smem + OFF_XY);
     unsigned *ZW = reinterpret_cast<unsigned *>(smem + OFF_Z);
     double *red = reinterpret_cast<double *>(smem + OFF_RED);
@@ -92,7 +93,8 @@ diag_fused_kernel(const float *__restrict__ posp, const float *__restrict__ momp
         const bool active = tma || (tx < wx && ty < wy);
 
         // this item's partial sums in fp32 (at most zchunk terms each), folded into the per-warp fp64 accumulators at its end
-        float gf[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f}, df[11] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+        f2 gf[3] = {bc(0.f), bc(0.f), bc(0.f)};     // Gauss: sum g^2, rho^2, div^2, (p, q) pairs
+        float df[11] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
         float gmax[2] = {0.f, 0.f}, maxth = 0.f;
         unsigned wsum = 0, csum = 0;          // sum |W| (lanes p: bits 0..15, q: 16..31); pierced cells p, q (same lanes)
         int npq = 0, nnear = 0, maxw = 0;     // cells pierced by both; near-cut plaquettes (p: bits 0..15, q: 16..31)
@@ -150,27 +152,23 @@ diag_fused_kernel(const float *__restrict__ posp, const float *__restrict__ momp
         const int e_row = (TY + 1) * COLS + lane + 1, e_col = (lane + 1) * COLS + TX + 1;
         auto do_alpha = [&](int e, const char *sn, int nxt) {          // phases of one site of plane `sn` into alpha[nxt]
             const float4 a = *reinterpret_cast<const float4 *>(sn + e * 16);
-            alpha[(nxt * 2 + 0) * NELEM + e] = site_phase(a.x, a.z);
-            alpha[(nxt * 2 + 1) * NELEM + e] = site_phase(a.y, a.w);
+            alpha[nxt * NELEM + e] = site_phase2(lo(a), hi(a));
         };
         // wrap counts of the x and y links of one site of plane `sn` (links that leave the extended tile -- x links of
         // the extra column, y links of the extra row -- are evaluated on whatever the neighbouring shared-memory words
         // hold and never read), returns the site's two phases for the z links
-        auto do_links_xy = [&](int e, const char *sn, int nxt, float &a0p, float &a0q) {
+        auto do_links_xy = [&](int e, const char *sn, int nxt, f2 &a0) {
             const float4 Bn = *reinterpret_cast<const float4 *>(sn + OFF_B + e * 16);
-            const float *ap = alpha + (nxt * 2 + 0) * NELEM + e, *aq = alpha + (nxt * 2 + 1) * NELEM + e;
-            a0p = ap[0];
-            a0q = aq[0];
-            const unsigned X = __byte_perm(link_lane(a0p, ap[1], Bn.x), link_lane(a0q, aq[1], Bn.y), 0x5410);
-            const unsigned Y = __byte_perm(link_lane(a0p, ap[COLS], Bn.z), link_lane(a0q, aq[COLS], Bn.w), 0x5410);
-            XY[nxt * NELEM + e] = make_uint2(X, Y);
+            const float2 *ap = alpha + nxt * NELEM + e;
+            a0 = ap[0];
+            XY[nxt * NELEM + e] = make_uint2(link_lane2(a0, ap[1], lo(Bn)), link_lane2(a0, ap[COLS], hi(Bn)));
         };
         auto do_links = [&](int e, const char *sc, const char *sn, int cur) {      // + the z links of plane `sc`
-            float a0p, a0q;
-            do_links_xy(e, sn, cur ^ 1, a0p, a0q);
+            f2 a0;
+            do_links_xy(e, sn, cur ^ 1, a0);
             const int r = e / COLS;
             const float2 Cz = *reinterpret_cast<const float2 *>(sc + OFF_C + (e + 2 * r + 1) * 8);
-            ZW[e] = __byte_perm(link_lane(alpha[(cur * 2 + 0) * NELEM + e], a0p, Cz.x), link_lane(alpha[(cur * 2 + 1) * NELEM + e], a0q, Cz.y), 0x5410);
+            ZW[e] = link_lane2(alpha[cur * NELEM + e], a0, Cz);
         };
         auto wait_plane = [&]() {             // plane iz+1 (slot s_n) has landed
             if (tma) mbar_wait(bars + 8 * s_n, par_n);
@@ -189,9 +187,9 @@ diag_fused_kernel(const float *__restrict__ posp, const float *__restrict__ momp
             if (own_ext) do_alpha(e_own, sn, 0);
             if (xrow || xcol) do_alpha(xrow ? e_row : e_col, sn, 0);
             __syncthreads();
-            float u, v;
-            if (own_ext) do_links_xy(e_own, sn, 0, u, v);
-            if (xrow || xcol) do_links_xy(xrow ? e_row : e_col, sn, 0, u, v);
+            f2 u;
+            if (own_ext) do_links_xy(e_own, sn, 0, u);
+            if (xrow || xcol) do_links_xy(xrow ? e_row : e_col, sn, 0, u);
             __syncthreads();
             if (active) {
                 const uint2 Ln = XY[e_own], Lnx = XY[e_own + 1], Lny = XY[e_own + COLS];
@@ -238,48 +236,47 @@ diag_fused_kernel(const float *__restrict__ posp, const float *__restrict__ momp
                 const float4 Ac = A(sc, 0), Axp = A(sc, 1), Ayp = A(sc, COLS), Azp = A(sn, 0);
                 const float4 Bc = B(sc, 0), Bxp = B(sc, 1), Byp = B(sc, COLS), Bzp = B(sn, 0);
                 const float2 Cc = C(sc, 0), Cxp = C(sc, 1), Cyp = C(sc, CCOLS);
-                float kin = 0.f, grad = 0.f, elec = 0.f, mag = 0.f, m2[2];
+                // both sectors at once: a pair is (p, q) of one quantity, the 64-bit halves of the vector loads (common.cuh)
+                const f2 fr = lo(Ac), fi = hi(Ac), pr = lo(MA), pi = hi(MA);
+                const f2 E[3] = {lo(MB), hi(MB), MC}, Em[3] = {lo(MBxm), hi(MBym), ez_prev};
+                // Gauss (Eq. 9-10): differences and the charge density in fp64 (g is a 1e-6 cancellation), per sector
+                f2 gl, rl, dl;
 #pragma unroll
                 for (int s = 0; s < 2; s++) {
-                    const float fr = pk0(Ac, s), fi = pk1(Ac, s);
-                    const float pr = pk0(MA, s), pi = pk1(MA, s);
-                    // Gauss (Eq. 9-10): differences and the charge density in fp64 (g is a 1e-6 cancellation)
-                    const float E[3] = {pk0(MB, s), pk1(MB, s), pkc(MC, s)};
-                    const float Em[3] = {pk0(MBxm, s), pk1(MBym, s), pkc(ez_prev, s)};
-                    const double div = (((double)E[0] - (double)Em[0]) + ((double)E[1] - (double)Em[1]) + ((double)E[2] - (double)Em[2])) * k.inv_dx;
-                    const double rho = (s ? k.rho2 : k.rho1) * ((double)fr * (double)pi - (double)fi * (double)pr);
-                    const float gl = (float)(div - rho), rl = (float)rho, dl = (float)div;
-                    gf[3 * s + 0] = fmaf(gl, gl, gf[3 * s + 0]);
-                    gf[3 * s + 1] = fmaf(rl, rl, gf[3 * s + 1]);
-                    gf[3 * s + 2] = fmaf(dl, dl, gf[3 * s + 2]);
-                    gmax[s] = fmaxf(gmax[s], fabsf(gl));
-                    // densities (fp32 per-site terms)
-                    kin = fmaf(pr, pr, fmaf(pi, pi, kin));
-                    m2[s] = fmaf(fr, fr, fi * fi);
-                    const float th[3] = {pk0(Bc, s), pk1(Bc, s), pkc(Cc, s)};
-                    const float nr[3] = {pk0(Axp, s), pk0(Ayp, s), pk0(Azp, s)};
-                    const float ni[3] = {pk1(Axp, s), pk1(Ayp, s), pk1(Azp, s)};
-                    float g2 = 0.f, e2 = 0.f;
-#pragma unroll
-                    for (int i = 0; i < 3; i++) {
-                        float sn_, cs_;
-                        __sincosf(th[i], &sn_, &cs_);               // U = exp(-i theta): SFU phasor (abs. error ~5e-7)
-                        const float dr = fmaf(cs_, nr[i], fmaf(sn_, ni[i], -fr)), di = fmaf(cs_, ni[i], fmaf(-sn_, nr[i], -fi));
-                        g2 = fmaf(dr, dr, fmaf(di, di, g2));
-                        e2 = fmaf(E[i], E[i], e2);
-                        maxth = fmaxf(maxth, fabsf(th[i]));
-                    }
-                    // plaquettes (i, j) = (x,y), (x,z), (y,z)
-                    const float ty_x = pk1(Bxp, s), tx_y = pk0(Byp, s);
-                    const float tz_x = pkc(Cxp, s), tx_z = pk0(Bzp, s);
-                    const float tz_y = pkc(Cyp, s), ty_z = pk1(Bzp, s);
-                    const float P0 = th[0] + ty_x - tx_y - th[1], P1 = th[0] + tz_x - tx_z - th[2], P2 = th[1] + tz_y - ty_z - th[2];
-                    grad = fmaf(g2, k.inv_dx2, grad);
-                    elec = fmaf(e2, s ? k.el2 : k.el1, elec);
-                    mag = fmaf(fmaf(P0, P0, fmaf(P1, P1, P2 * P2)), s ? k.mg2 : k.mg1, mag);
+                    const double div = (((double)pkc(E[0], s) - (double)pkc(Em[0], s)) + ((double)pkc(E[1], s) - (double)pkc(Em[1], s)) +
+                                        ((double)pkc(E[2], s) - (double)pkc(Em[2], s))) * k.inv_dx;
+                    const double rho = (s ? k.rho2 : k.rho1) * ((double)pkc(fr, s) * (double)pkc(pi, s) - (double)pkc(fi, s) * (double)pkc(pr, s));
+                    const float g_ = (float)(div - rho), r_ = (float)rho, d_ = (float)div;
+                    if (s) { gl.y = g_; rl.y = r_; dl.y = d_; } else { gl.x = g_; rl.x = r_; dl.x = d_; }
+                    gmax[s] = fmaxf(gmax[s], fabsf(g_));
                 }
+                gf[0] = fma2(gl, gl, gf[0]);
+                gf[1] = fma2(rl, rl, gf[1]);
+                gf[2] = fma2(dl, dl, gf[2]);
+                // densities (fp32 per-site terms, packed fp32x2)
+                const f2 kin2 = fma2(pr, pr, mul2(pi, pi)), m2 = fma2(fr, fr, mul2(fi, fi));
+                const f2 th[3] = {lo(Bc), hi(Bc), Cc};
+                const f2 nr[3] = {lo(Axp), lo(Ayp), lo(Azp)}, ni[3] = {hi(Axp), hi(Ayp), hi(Azp)};
+                f2 g2 = bc(0.f), e2 = bc(0.f);
+#pragma unroll
+                for (int i = 0; i < 3; i++) {
+                    f2 sn_, cs_;
+                    __sincosf(th[i].x, &sn_.x, &cs_.x);             // U = exp(-i theta): SFU phasor (abs. error ~5e-7)
+                    __sincosf(th[i].y, &sn_.y, &cs_.y);
+                    const f2 dr = fma2(cs_, nr[i], fma2(sn_, ni[i], neg(fr))), di = fma2(cs_, ni[i], fma2(neg(sn_), nr[i], neg(fi)));
+                    g2 = fma2(dr, dr, fma2(di, di, g2));
+                    e2 = fma2(E[i], E[i], e2);
+                    maxth = fmaxf(maxth, fmaxf(fabsf(th[i].x), fabsf(th[i].y)));
+                }
+                // plaquettes (i, j) = (x,y), (x,z), (y,z)
+                const f2 P0 = sub2(sub2(add2(th[0], hi(Bxp)), lo(Byp)), th[1]);
+                const f2 P1 = sub2(sub2(add2(th[0], Cxp), lo(Bzp)), th[2]);
+                const f2 P2 = sub2(sub2(add2(th[1], Cyp), hi(Bzp)), th[2]);
+                const f2 gw = mul2(g2, bc(k.inv_dx2)), ew = mul2(e2, make_float2(k.el1, k.el2));
+                const f2 mw = mul2(fma2(P0, P0, fma2(P1, P1, mul2(P2, P2))), make_float2(k.mg1, k.mg2));
+                const float kin = kin2.x + kin2.y, grad = gw.x + gw.y, elec = ew.x + ew.y, mag = mw.x + mw.y;
                 ez_prev = MC;
-                const float a2 = m2[0] - k.sig1sq, b2 = m2[1] - k.sig2sq;
+                const float a2 = m2.x - k.sig1sq, b2 = m2.y - k.sig2sq;
                 const float vint = k.kappa * a2 * b2;
                 const float pot = k.lam1q * a2 * a2 + k.lam2q * b2 * b2 - vint;
                 const float lag = kin - grad + (elec - mag) * k.inv_c - k.c * pot;
@@ -438,7 +435,7 @@ diag_fused_kernel(const float *__restrict__ posp, const float *__restrict__ momp
         auto add = [&](int slot, double v) { if (lane == 0) red[slot * (NTHREADS / 32) + warp] += v; };
         auto amax = [&](int slot, double v) { if (lane == 0) red[slot * (NTHREADS / 32) + warp] = fmax(red[slot * (NTHREADS / 32) + warp], v); };
 #pragma unroll
-        for (int i = 0; i < 6; i++) add(FR_GAUSS + i, warp_sum((double)gf[i]));
+        for (int i = 0; i < 6; i++) add(FR_GAUSS + i, warp_sum((double)pkc(gf[i % 3], i / 3)));
 #pragma unroll
         for (int i = 0; i < 11; i++) add(FR_DENS + i, warp_sum((double)df[i]));
         add(FR_SUMW, (double)__reduce_add_sync(0xffffffffu, wsum & 0xffffu));

@@ -3,23 +3,10 @@
 // (step_tiled.cu) and the two-steps-per-pass kernel (step_tb.cu), so that the two produce the same bits.
 #pragma once
 #include "common.cuh"
+#include "f32x2.cuh"
 
 namespace u1u1 {
 
-// ---- packed fp32x2 arithmetic (sm_100: FFMA2 / FADD2 / FMUL2, one issue slot for two IEEE fp32 operations) ----
-// A pair holds the SAME quantity of the two sectors (p in .x, q in .y): the two sectors obey the same equations
-// (PAPER.md:79), and the layout of common.cuh puts such pairs in the aligned 64-bit halves of every vector load.
-// Negations fold into the operand modifiers of the packed instructions; scalars broadcast from uniform registers.
-typedef float2 f2;
-__device__ __forceinline__ f2 lo(const float4 &v) { return make_float2(v.x, v.y); }
-__device__ __forceinline__ f2 hi(const float4 &v) { return make_float2(v.z, v.w); }
-__device__ __forceinline__ f2 bc(float a) { return make_float2(a, a); }
-__device__ __forceinline__ f2 neg(f2 a) { return make_float2(-a.x, -a.y); }
-__device__ __forceinline__ f2 add2(f2 a, f2 b) { return __fadd2_rn(a, b); }
-__device__ __forceinline__ f2 sub2(f2 a, f2 b) { return __fadd2_rn(a, neg(b)); }
-__device__ __forceinline__ f2 mul2(f2 a, f2 b) { return __fmul2_rn(a, b); }
-__device__ __forceinline__ f2 fma2(f2 a, f2 b, f2 c) { return __ffma2_rn(a, b, c); }
-__device__ __forceinline__ f2 plaq2(f2 a, f2 b, f2 c, f2 d) { return sub2(sub2(add2(a, b), c), d); }
 // difference-form phasors of both sectors' link: the two MUFU pairs stay scalar, everything around them is packed
 __device__ __forceinline__ void phasor_diff2(f2 th, f2 &sn, f2 &c1)
 {
