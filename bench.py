@@ -44,7 +44,7 @@ def workload_name(n, prephase=PREPHASE_STEPS):
 
 
 # what the measured DRAM traffic depends on: the sources of the step kernels
-TRAFFIC_SOURCES = ("step_tiled.cu", "step_tb.cu", "step_site.cuh", "stage.cuh", "common.cuh")
+TRAFFIC_SOURCES = ("step_tiled.cu", "step_tb.cu", "step_site.cuh", "f32x2.cuh", "stage.cuh", "common.cuh")
 
 
 def csrc_sha():
