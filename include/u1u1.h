@@ -72,7 +72,11 @@ typedef struct {
                                 16*1 = variant 0 in scalar instead of packed fp32x2 instructions (same bits);
                                 16*16 / 16*32 = L2 policies, 16*64 / 16*128 = 16 / 32-plane chunks (diagnostics);
                                 16*256 = one-step kernel even with an aux buffer, 16*512 / 16*1024 = 16 / 64-plane
-                                chunks of the two-steps-per-pass kernel.  */
+                                chunks of the two-steps-per-pass kernel;
+                                16*2048 = variant 0 with an explicit range reduction of the link phases in front of the
+                                SFU sine / cosine: phasor error 5e-7 at ANY |theta| instead of 6e-8 |theta| (identical
+                                bits while |theta| < 2 pi, ~4 % slower; for runs whose non-compact phases grow beyond ~10;
+                                u1u1_diagnostics reports max |theta|).  */
 } u1u1_params;
 
 /* Bytes of device memory the caller must provide for an N^3 lattice.

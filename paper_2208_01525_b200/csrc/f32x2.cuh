@@ -19,4 +19,16 @@ __device__ __forceinline__ f2 mul2(f2 a, f2 b) { return __fmul2_rn(a, b); }
 __device__ __forceinline__ f2 fma2(f2 a, f2 b, f2 c) { return __ffma2_rn(a, b, c); }
 __device__ __forceinline__ f2 plaq2(f2 a, f2 b, f2 c, f2 d) { return sub2(sub2(add2(a, b), c), d); }
 
+// Range reduction in front of the SFU sine / cosine (MUFU takes the angle times 1/(2 pi) rounded to fp32, an absolute
+// error of 6e-8 |theta| for the non-compact link phases of reading R-9): r = theta - n 2 pi with n = rint(theta / 2 pi) by
+// the magic-number addition and 2 pi split into its fp32 value and the remainder (Cody-Waite; |theta| < 2^22 * 2 pi).
+// For |theta| < pi (every production run) n = 0 and r is theta itself, bit for bit.
+constexpr float RR_INV_2PI = 0.15915494309189535f, RR_MAGIC = 12582912.f;
+constexpr float RR_2PI_HI = 6.2831854820251465f, RR_2PI_LO = -1.7484555e-07f;       // 2 pi = HI + LO
+__device__ __forceinline__ f2 reduce_2pi2(f2 th)
+{
+    const f2 n = add2(fma2(th, bc(RR_INV_2PI), bc(RR_MAGIC)), bc(-RR_MAGIC));
+    return fma2(n, bc(-RR_2PI_LO), fma2(n, bc(-RR_2PI_HI), th));
+}
+
 }  // namespace u1u1

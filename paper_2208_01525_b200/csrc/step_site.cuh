@@ -8,9 +8,12 @@
 namespace u1u1 {
 
 // difference-form phasors of both sectors' link: the two MUFU pairs stay scalar, everything around them is packed
+// RR: explicit range reduction of the half angle in front of the SFU (f32x2.cuh): keeps the phasor error at 5e-7 for
+// non-compact phases of any size instead of 6e-8 |theta|; the identity, bit for bit, while |theta| < 2 pi.
+template <bool RR>
 __device__ __forceinline__ void phasor_diff2(f2 th, f2 &sn, f2 &c1)
 {
-    const f2 h = mul2(th, bc(0.5f));
+    const f2 h0 = mul2(th, bc(0.5f)), h = RR ? reduce_2pi2(h0) : h0;
     f2 sh, ch;
     __sincosf(h.x, &sh.x, &ch.x);
     __sincosf(h.y, &sh.y, &ch.y);
@@ -29,14 +32,14 @@ struct PkCarry {
 // Accessors: A(p, dx, dy), B(p, dx, dy) return the float4 of pack A / B and C(p, dx, dy) the float2 of pack C of the site
 // displaced by (dx, dy) in plane p (0 = the site's own plane z, 1 = plane z+1); the displacements are literals, so every
 // address is base + immediate.  Operation order = the scalar difference-form chain of step_tiled.cu.
-template <class FA, class FB, class FC>
+template <bool RR, class FA, class FB, class FC>
 __device__ __forceinline__ void pk_carry_init(PkCarry &cy, FA A, FB B, FC C)       // here plane 0 = z-1, plane 1 = z
 {
     const float4 Ac = A(0, 0, 0), Bc = B(0, 0, 0), Bzp = B(1, 0, 0), Azp = A(1, 0, 0);
     const f2 thz = C(0, 0, 0), Cxp = C(0, 1, 0), Cyp = C(0, 0, 1);
     const f2 fr = lo(Ac), fi = hi(Ac);
     f2 sn, c1;
-    phasor_diff2(thz, sn, c1);
+    phasor_diff2<RR>(thz, sn, c1);
     cy.bzr = fma2(neg(sn), fi, fma2(neg(c1), fr, sub2(fr, lo(Azp))));
     cy.bzi = fma2(sn, fr, fma2(neg(c1), fi, sub2(fi, hi(Azp))));
     cy.Pyz = plaq2(hi(Bc), Cyp, hi(Bzp), thz);
@@ -44,7 +47,7 @@ __device__ __forceinline__ void pk_carry_init(PkCarry &cy, FA A, FB B, FC C)    
 }
 
 // MA, MB, MC: the site's momenta, updated in place; OA, OB, OC: its new positions.
-template <class FA, class FB, class FC>
+template <bool RR, class FA, class FB, class FC>
 __device__ __forceinline__ void pk_site_update(PkCarry &cy, FA A, FB B, FC C, const StepCoef &k, float4 &MA, float4 &MB,
                                                float2 &MC, float4 &OA, float4 &OB, float2 &OC)
 {
@@ -57,27 +60,27 @@ __device__ __forceinline__ void pk_site_update(PkCarry &cy, FA A, FB B, FC C, co
     const f2 thmx = lo(Bxm), thmy = hi(Bym);                             // theta_i(x - i), i = x, y
     f2 lap_re = cy.bzr, lap_im = cy.bzi, J0, J1, J2, sn, c1, dr, di;
     // x: forward hop, current, backward hop
-    phasor_diff2(thx, sn, c1);
+    phasor_diff2<RR>(thx, sn, c1);
     dr = fma2(sn, hi(Axp), fma2(neg(c1), lo(Axp), sub2(lo(Axp), fr)));
     di = fma2(neg(sn), lo(Axp), fma2(neg(c1), hi(Axp), sub2(hi(Axp), fi)));
     lap_re = add2(lap_re, dr);
     lap_im = add2(lap_im, di);
     J0 = fma2(fr, di, neg(mul2(fi, dr)));
-    phasor_diff2(thmx, sn, c1);
+    phasor_diff2<RR>(thmx, sn, c1);
     lap_re = add2(lap_re, fma2(neg(sn), hi(Axm), fma2(neg(c1), lo(Axm), sub2(lo(Axm), fr))));
     lap_im = add2(lap_im, fma2(sn, lo(Axm), fma2(neg(c1), hi(Axm), sub2(hi(Axm), fi))));
     // y
-    phasor_diff2(thy, sn, c1);
+    phasor_diff2<RR>(thy, sn, c1);
     dr = fma2(sn, hi(Ayp), fma2(neg(c1), lo(Ayp), sub2(lo(Ayp), fr)));
     di = fma2(neg(sn), lo(Ayp), fma2(neg(c1), hi(Ayp), sub2(hi(Ayp), fi)));
     lap_re = add2(lap_re, dr);
     lap_im = add2(lap_im, di);
     J1 = fma2(fr, di, neg(mul2(fi, dr)));
-    phasor_diff2(thmy, sn, c1);
+    phasor_diff2<RR>(thmy, sn, c1);
     lap_re = add2(lap_re, fma2(neg(sn), hi(Aym), fma2(neg(c1), lo(Aym), sub2(lo(Aym), fr))));
     lap_im = add2(lap_im, fma2(sn, lo(Aym), fma2(neg(c1), hi(Aym), sub2(hi(Aym), fi))));
     // z: forward hop, current, and the backward z difference of the NEXT plane
-    phasor_diff2(thz, sn, c1);
+    phasor_diff2<RR>(thz, sn, c1);
     dr = fma2(sn, hi(Azp), fma2(neg(c1), lo(Azp), sub2(lo(Azp), fr)));
     di = fma2(neg(sn), lo(Azp), fma2(neg(c1), hi(Azp), sub2(hi(Azp), fi)));
     lap_re = add2(lap_re, dr);

@@ -44,7 +44,7 @@ static_assert(2 * (SMEM_BYTES + 1024) <= 233472, "two CTAs per SM");
 
 // TMA: the tile's two-site halo lies inside the lattice, positions and momenta arrive by TMA boxes; otherwise
 // (boundary / ragged tiles) by per-thread cp.async with the periodic wrap resolved in a per-thread plan.
-template <bool TMA>
+template <bool TMA, bool RR>
 __device__ __forceinline__ void tb_tile(const TbLattice &L, const StepCoef &k1, const StepCoef &k2, const TbMaps &maps, char *smem,
                                         int x0, int y0, int z0, int wx, int wy, int nz)
 {
@@ -174,7 +174,7 @@ __device__ __forceinline__ void tb_tile(const TbLattice &L, const StepCoef &k1, 
     if (act) {
         const char *p0 = smem, *p1 = smem + P2_SLOT_BYTES;
         TB_ACC1(p0, p1);
-        pk_carry_init(cy1, fA, fB, fC);
+        pk_carry_init<RR>(cy1, fA, fB, fC);
     }
     __syncthreads();                          // everybody is done with position plane 0: its slot takes plane 3
     if (issuer) stage_P(3, 0);
@@ -209,7 +209,7 @@ __device__ __forceinline__ void tb_tile(const TbLattice &L, const StepCoef &k1, 
             TB_ACC1(p0, p1);
             float4 OA, OB;
             float2 OC;
-            pk_site_update(cy1, fA, fB, fC, k1, MA, MB, MC, OA, OB, OC);
+            pk_site_update<RR>(cy1, fA, fB, fC, k1, MA, MB, MC, OA, OB, OC);
             *reinterpret_cast<float4 *>(iCur + eI * 16) = OA;
             *reinterpret_cast<float4 *>(iCur + OFF_B + eI * 16) = OB;
             *reinterpret_cast<float2 *>(iCur + OFF_C + eIC * 8) = OC;
@@ -228,11 +228,11 @@ __device__ __forceinline__ void tb_tile(const TbLattice &L, const StepCoef &k1, 
         if (inner && act && t >= 1) {
             TB_ACC2(iPrev, iCur);
             if (t == 1) {
-                pk_carry_init(cy2, fA, fB, fC);
+                pk_carry_init<RR>(cy2, fA, fB, fC);
             } else {
                 float4 OA, OB;
                 float2 OC;
-                pk_site_update(cy2, fA, fB, fC, k2, MAo, MBo, MCo, OA, OB, OC);
+                pk_site_update<RR>(cy2, fA, fB, fC, k2, MAo, MBo, MCo, OA, OB, OC);
                 const size_t lin = (size_t)(z0 + t - 2) * NN + gsite;
                 __stcs(reinterpret_cast<float4 *>(L.mom_out) + lin, MAo);
                 __stcs(reinterpret_cast<float4 *>(L.mom_out + 4 * V) + lin, MBo);
@@ -258,6 +258,8 @@ __device__ __forceinline__ void tb_tile(const TbLattice &L, const StepCoef &k1, 
 #undef TB_ACC2
 }
 
+// RR: explicit range reduction of the link phases in front of the SFU (step_site.cuh; tuning flag 2048)
+template <bool RR>
 __global__ void __launch_bounds__(TB_THREADS, 2)
 step_tb_kernel(TbLattice L, StepCoef k1, StepCoef k2, int zchunk, int band, const __grid_constant__ TbMaps maps)
 {
@@ -271,9 +273,9 @@ step_tb_kernel(TbLattice L, StepCoef k1, StepCoef k2, int zchunk, int band, cons
     const int nz = min(zchunk, N - z0);
     // CTA-uniform choice of the staging path
     if (!(k1.flags & 2) && x0 >= 2 && x0 + TX + 2 <= N && y0 >= 2 && y0 + TY + 2 <= N)
-        tb_tile<true>(L, k1, k2, maps, smem, x0, y0, z0, TX, TY, nz);
+        tb_tile<true, RR>(L, k1, k2, maps, smem, x0, y0, z0, TX, TY, nz);
     else
-        tb_tile<false>(L, k1, k2, maps, smem, x0, y0, z0, min(TX, N - x0), min(TY, N - y0), nz);
+        tb_tile<false, RR>(L, k1, k2, maps, smem, x0, y0, z0, min(TX, N - x0), min(TY, N - y0), nz);
 }
 
 }  // namespace
@@ -282,7 +284,8 @@ bool step_tb_supports(int N) { return N >= 8 && (N % 4) == 0; }
 
 cudaError_t launch_step_tb(const TbLattice &L, StepCoef k1, StepCoef k2, cudaStream_t st, const TbMaps *m, int sms)
 {
-    cudaError_t ea = cudaFuncSetAttribute(step_tb_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+    const bool rr = (k1.flags & 2048) != 0;
+    cudaError_t ea = cudaFuncSetAttribute(rr ? step_tb_kernel<true> : step_tb_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
     if (ea != cudaSuccess) return ea;
     TbMaps maps;
     if (!m) {
@@ -300,7 +303,8 @@ cudaError_t launch_step_tb(const TbLattice &L, StepCoef k1, StepCoef k2, cudaStr
     const int nzc = (N + zc - 1) / zc;
     int band = (k1.flags & 8) ? nty : (sms * 2 + ntx - 1) / ntx;
     if (band > nty) band = nty;
-    step_tb_kernel<<<(unsigned)(ntx * nty * nzc), TB_THREADS, SMEM_BYTES, st>>>(L, k1, k2, zc, band, maps);
+    if (rr) step_tb_kernel<true><<<(unsigned)(ntx * nty * nzc), TB_THREADS, SMEM_BYTES, st>>>(L, k1, k2, zc, band, maps);
+    else step_tb_kernel<false><<<(unsigned)(ntx * nty * nzc), TB_THREADS, SMEM_BYTES, st>>>(L, k1, k2, zc, band, maps);
     return cudaGetLastError();
 }
 

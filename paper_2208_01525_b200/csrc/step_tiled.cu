@@ -32,7 +32,8 @@ constexpr int OFF_BARS = OFF_MRING + 2 * MSLOT_BYTES;           // fullP[4], ful
 constexpr int SMEM_BYTES = OFF_BARS + 64;                       // 76 352 B -> 3 CTAs per SM
 
 // exp(-i theta): libm sincosf (1-2 ulp) or, with FAST, the SFU approximations.  MUFU.SIN/COS take the angle
-// in turns and reduce it themselves (one FMUL by 1/(2 pi) + 2 MUFU); error max(5e-7, 6e-8 |theta|).  The
+// in turns and reduce it themselves (one FMUL by 1/(2 pi) + 2 MUFU); error max(5e-7, 6e-8 |theta|) -- 5e-7 at any
+// |theta| in the RR instances, which reduce the angle explicitly first (tuning flag 2048, f32x2.cuh).  The
 // discrete Gauss law holds for ANY complex U used consistently for a link, so this error never enters it
 // (DESIGN.md section 8).
 template <bool FAST>
@@ -78,7 +79,7 @@ __device__ inline void set2(float2 &v, int i, float a) { if (i == 0) v.x = a; el
 // slab's top / bottom output planes are also stored into the neighbouring slabs' halo planes.
 // PK (only with FAST, float, DIFF): both sectors at once in packed fp32x2 instructions; bit-identical to the scalar
 // difference-form chain (same IEEE operations in the same order), which stays available under tuning flag 1.
-template <bool FAST, typename R, bool DIFF, bool SLAB, bool PK>
+template <bool FAST, typename R, bool DIFF, bool SLAB, bool PK, bool RR>
 __global__ void __launch_bounds__(NTHREADS, sizeof(R) == 8 ? 2 : 3)
 step_tiled_kernel(Lattice L, StepCoef k, int zchunk, int band, const __grid_constant__ StepMaps maps)
 {
@@ -166,7 +167,7 @@ step_tiled_kernel(Lattice L, StepCoef k, int zchunk, int band, const __grid_cons
         auto pA = [&](int p, int dx, int dy) { return A(p ? sp : sc, dy * COLS + dx); };
         auto pB = [&](int p, int dx, int dy) { return B(p ? sp : sc, dy * COLS + dx); };
         auto pC = [&](int p, int dx, int dy) { return C(p ? sp : sc, dy * CCOLS + dx); };
-        pk_carry_init(cy, pA, pB, pC);
+        pk_carry_init<RR>(cy, pA, pB, pC);
     }
     if (!PK && active) {
         const char *sc = smem, *sp = smem + SLOT_BYTES;          // planes -1 and 0
@@ -246,7 +247,7 @@ step_tiled_kernel(Lattice L, StepCoef k, int zchunk, int band, const __grid_cons
             auto pA = [&](int p, int dx, int dy) { return A(p ? sp : sc, dy * COLS + dx); };
             auto pB = [&](int p, int dx, int dy) { return B(p ? sp : sc, dy * COLS + dx); };
             auto pC = [&](int p, int dx, int dy) { return C(p ? sp : sc, dy * CCOLS + dx); };
-            pk_site_update(cy, pA, pB, pC, k, MA, MB, MC, OA, OB, OC);
+            pk_site_update<RR>(cy, pA, pB, pC, k, MA, MB, MC, OA, OB, OC);
         }
 
         const R m2p = (R)Ac.x * (R)Ac.x + (R)Ac.z * (R)Ac.z;
@@ -392,11 +393,11 @@ int pick_zchunk(int N, int sms)
     return zc < N ? zc : N;
 }
 
-template <bool FAST, typename R, bool DIFF, bool SLAB = false, bool PK = false>
+template <bool FAST, typename R, bool DIFF, bool SLAB = false, bool PK = false, bool RR = false>
 cudaError_t launch_one(const Lattice &L, StepCoef k, cudaStream_t st, const StepMaps *m, int sms)
 {
     // per device and cheap: set on every launch rather than caching a per-process flag
-    cudaError_t ea = cudaFuncSetAttribute(step_tiled_kernel<FAST, R, DIFF, SLAB, PK>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+    cudaError_t ea = cudaFuncSetAttribute(step_tiled_kernel<FAST, R, DIFF, SLAB, PK, RR>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
     if (ea != cudaSuccess) return ea;
     StepMaps maps;
     if (!m) {
@@ -413,7 +414,7 @@ cudaError_t launch_one(const Lattice &L, StepCoef k, cudaStream_t st, const Step
     int band = (k.flags & 8) ? nty : (sms * per_sm + ntx - 1) / ntx;     // tuning flag 8: the order of a plain 3-d grid
     if (band > nty) band = nty;
     const unsigned grid = (unsigned)ntx * nty * nzc;
-    step_tiled_kernel<FAST, R, DIFF, SLAB, PK><<<grid, NTHREADS, SMEM_BYTES, st>>>(L, k, zc, band, maps);
+    step_tiled_kernel<FAST, R, DIFF, SLAB, PK, RR><<<grid, NTHREADS, SMEM_BYTES, st>>>(L, k, zc, band, maps);
     return cudaGetLastError();
 }
 
@@ -433,8 +434,10 @@ cudaError_t launch_step_tiled(const Lattice &L, const StepCoef &k, cudaStream_t 
         case 3: return launch_one<true, float, false>(L, k, st, maps, sms);
         case 4: return launch_one<false, float, true>(L, k, st, maps, sms);
         default:            // the production instance: packed fp32x2 chain (tuning flag 1: the same chain in scalar instructions)
+            // (tuning flag 2048: the packed chain with explicit range reduction of the link phases)
             return (k.flags & 1) ? launch_one<true, float, true>(L, k, st, maps, sms)
-                                 : launch_one<true, float, true, false, true>(L, k, st, maps, sms);
+                 : (k.flags & 2048) ? launch_one<true, float, true, false, true, true>(L, k, st, maps, sms)
+                                    : launch_one<true, float, true, false, true>(L, k, st, maps, sms);
     }
 }
 

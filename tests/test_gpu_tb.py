@@ -30,9 +30,10 @@ def run(state64, N, params, calls, aux):
     return lat.export_state().cpu().numpy().astype(np.float64), lat
 
 
+# flags 2048: the instances with explicit range reduction of the link phases (same bits while |theta| < 2 pi);
 # 132: interior (TMA), boundary and ragged tiles, two z chunks with a ragged one; 64: no interior tile in x (cp.async
 # only); 8 / 12: the lattice is smaller than a tile and the two-site halo wraps onto the tile itself; 40: ragged in x
-@pytest.mark.parametrize("N,flags", [(132, 0), (132, 2), (132, 512), (64, 0), (40, 0), (12, 0), (8, 0), (96, 1024)])
+@pytest.mark.parametrize("N,flags", [(132, 0), (132, 2), (132, 512), (64, 0), (40, 0), (12, 0), (8, 0), (96, 1024), (68, 2048)])
 def test_two_steps_per_pass_bit_identical(N, flags):
     from paper_2208_01525_b200 import Params
     s0 = inputs.to_f32_exact(inputs.random_state((N, N, N), seed=41 + N))
