@@ -181,7 +181,9 @@ __device__ __forceinline__ void tb_tile(const TbLattice &L, const StepCoef &k1, 
     if (!TMA) cp_async_commit();
 
     unsigned sP = 1;                          // ring slot of position plane t + 1
-    char *iCur = smem + OFF_I, *iPrev = smem + OFF_I + SLOT_BYTES, *iFree = smem + OFF_I + 2 * SLOT_BYTES;   // step-1 planes t, t-1, t-2
+    // slots of the step-1 planes t, t-1, t-2 as explicit pointers rotated at the end of every iteration (computing them from
+    // the parity of t was miscompiled in the peeled iteration t = 1: DESIGN.md section 12)
+    char *iCur = smem + OFF_I, *iPrev = smem + OFF_I + SLOT_BYTES, *iFree = smem + OFF_I + 2 * SLOT_BYTES;
     // iteration t: step 1 on relative plane t - 1 (position planes t+1, t+2; momentum plane t), then step 2 on relative
     // plane t - 2 (step-1 planes t-1, t)
     for (int t = 0; t <= nz + 1; t++) {
