@@ -41,6 +41,7 @@ struct u1u1_ctx {
     int sms = 0;
     bool maps_ready = false;
     PackMaps pos_halo[2], mom_halo[2], mom_tile[2];     // momenta: [0] the buffer inside `state`, [1] the aux buffer
+    PackMaps mom_tile_tb[2];                             // tile boxes of the two-steps-per-pass kernel's tile
     PackMaps pos_halo2[2];                               // two-site-halo boxes of the positions (two-steps-per-pass kernel)
     // optional second momentum buffer (u1u1_set_aux): enables the two-steps-per-pass kernel, which reads the momenta
     // from one buffer and writes them to the other
@@ -192,6 +193,8 @@ static int prepare_device(u1u1_ctx *ctx)
         if (ok && ctx->aux)
             ok = encode_halo_maps(&ctx->mom_halo[1], ctx->aux, ctx->V, ctx->N, NZ) &&
                  encode_tile_maps(&ctx->mom_tile[1], ctx->aux, ctx->V, ctx->N, NZ) &&
+                 encode_tb_tile_maps(&ctx->mom_tile_tb[0], mom_buf_at(ctx, 0), ctx->V, ctx->N, NZ) &&
+                 encode_tb_tile_maps(&ctx->mom_tile_tb[1], ctx->aux, ctx->V, ctx->N, NZ) &&
                  encode_halo2_maps(&ctx->pos_halo2[0], pos_buf(ctx, 0), ctx->V, ctx->N, NZ) &&
                  encode_halo2_maps(&ctx->pos_halo2[1], pos_buf(ctx, 1), ctx->V, ctx->N, NZ);
         if (!ok) return fail(ctx, U1U1_ECUDA, "cuTensorMapEncodeTiled unavailable or rejected the layout (TMA is required)");
@@ -329,7 +332,7 @@ static cudaError_t launch_two_steps(u1u1_ctx *ctx, const StepCoef &q1, const Ste
     TbMaps maps;
     if (ctx->maps_ready) {
         maps.pos = ctx->pos_halo2[ctx->cur];
-        maps.mom = ctx->mom_tile[ctx->mcur];
+        maps.mom = ctx->mom_tile_tb[ctx->mcur];
     }
     cudaError_t e = launch_step_tb(L, q1, q2, ctx->stream, ctx->maps_ready ? &maps : nullptr, ctx->sms);
     ctx->mcur ^= 1;

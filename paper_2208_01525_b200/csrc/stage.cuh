@@ -31,8 +31,12 @@ static_assert(NELEM * 16 <= OFF_B && OFF_B + NELEM * 16 <= OFF_C && OFF_C + ROWS
 
 // The two-steps-per-pass kernel (step_tb.cu) stages positions with a TWO-site halo: A, B float4[P2_ROWS][P2_COLS], C
 // float2[P2_ROWS][P2_COLS], all from site (x0-2, y0-2) (an even x, so pack C is 16-byte aligned as it is).
-constexpr int P2_COLS = TX + 4, P2_ROWS = TY + 4, P2_ELEM = P2_ROWS * P2_COLS;      // 36 x 12 = 432 sites
-constexpr int P2_OFF_B = P2_ELEM * 16, P2_OFF_C = 2 * P2_ELEM * 16, P2_SLOT_BYTES = P2_OFF_C + P2_ELEM * 8;   // 17 280 B
+#ifndef TB_TY
+#define TB_TY 16         // 8: 352 threads, 2 CTAs/SM, 80 registers; 16: 640 threads, 1 CTA/SM, 96 registers (faster)
+#endif
+constexpr int TBY = TB_TY;          // tile height of the two-steps-per-pass kernel
+constexpr int P2_COLS = TX + 4, P2_ROWS = TBY + 4, P2_ELEM = P2_ROWS * P2_COLS;      // 36 x 20 = 720 sites
+constexpr int P2_OFF_B = P2_ELEM * 16, P2_OFF_C = 2 * P2_ELEM * 16, P2_SLOT_BYTES = P2_OFF_C + P2_ELEM * 8;   // 28 800 B
 static_assert(P2_OFF_B % 128 == 0 && P2_OFF_C % 128 == 0 && P2_SLOT_BYTES % 128 == 0, "TMA destinations");
 
 // Tensor maps of the three packs of one buffer (halo boxes COLS x ROWS, or plain TX x TY tile boxes).
@@ -58,6 +62,7 @@ struct alignas(64) TbMaps {
 bool encode_halo_maps(PackMaps *m, const float *buf, size_t V, int N, int NZ, int rows = ROWS);
 bool encode_tile_maps(PackMaps *m, const float *buf, size_t V, int N, int NZ);
 bool encode_halo2_maps(PackMaps *m, const float *buf, size_t V, int N, int NZ);
+bool encode_tb_tile_maps(PackMaps *m, const float *buf, size_t V, int N, int NZ);
 
 #ifdef __CUDACC__
 __device__ inline unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }

@@ -27,12 +27,13 @@ __device__ __forceinline__ void phasor_diff2(f2 th, f2 &sn, f2 &c1)
 // conj(U_z(x-z)) f(x-z) - f(x) and the two plaquettes that contain theta_z(x-z) (bit-identical to the neighbour's own).
 struct PkCarry {
     f2 bzr, bzi, Pyz, Pzx;
+    float4 Ac, Bc;          // OWN: the site's own packs A and B, loaded one plane earlier as its z+1 neighbour's
 };
 
 // Accessors: A(p, dx, dy), B(p, dx, dy) return the float4 of pack A / B and C(p, dx, dy) the float2 of pack C of the site
 // displaced by (dx, dy) in plane p (0 = the site's own plane z, 1 = plane z+1); the displacements are literals, so every
 // address is base + immediate.  Operation order = the scalar difference-form chain of step_tiled.cu.
-template <bool RR, class FA, class FB, class FC>
+template <bool RR, bool OWN = false, class FA, class FB, class FC>
 __device__ __forceinline__ void pk_carry_init(PkCarry &cy, FA A, FB B, FC C)       // here plane 0 = z-1, plane 1 = z
 {
     const float4 Ac = A(0, 0, 0), Bc = B(0, 0, 0), Bzp = B(1, 0, 0), Azp = A(1, 0, 0);
@@ -44,15 +45,21 @@ __device__ __forceinline__ void pk_carry_init(PkCarry &cy, FA A, FB B, FC C)    
     cy.bzi = fma2(sn, fr, fma2(neg(c1), fi, sub2(fi, hi(Azp))));
     cy.Pyz = plaq2(hi(Bc), Cyp, hi(Bzp), thz);
     cy.Pzx = plaq2(thz, lo(Bzp), Cxp, lo(Bc));
+    if (OWN) {
+        cy.Ac = Azp;
+        cy.Bc = Bzp;
+    }
 }
 
 // MA, MB, MC: the site's momenta, updated in place; OA, OB, OC: its new positions.
-template <bool RR, class FA, class FB, class FC>
+// OWN: the site's own packs A and B of plane z come from the carry (two fewer 128-bit shared-memory reads, eight more
+// carried registers).
+template <bool RR, bool OWN = false, class FA, class FB, class FC>
 __device__ __forceinline__ void pk_site_update(PkCarry &cy, FA A, FB B, FC C, const StepCoef &k, float4 &MA, float4 &MB,
                                                float2 &MC, float4 &OA, float4 &OB, float2 &OC)
 {
-    const float4 Ac = A(0, 0, 0), Axp = A(0, 1, 0), Axm = A(0, -1, 0), Ayp = A(0, 0, 1), Aym = A(0, 0, -1), Azp = A(1, 0, 0);
-    const float4 Bc = B(0, 0, 0), Bxp = B(0, 1, 0), Bxm = B(0, -1, 0), Byp = B(0, 0, 1), Bym = B(0, 0, -1);
+    const float4 Ac = OWN ? cy.Ac : A(0, 0, 0), Axp = A(0, 1, 0), Axm = A(0, -1, 0), Ayp = A(0, 0, 1), Aym = A(0, 0, -1), Azp = A(1, 0, 0);
+    const float4 Bc = OWN ? cy.Bc : B(0, 0, 0), Bxp = B(0, 1, 0), Bxm = B(0, -1, 0), Byp = B(0, 0, 1), Bym = B(0, 0, -1);
     const float4 Bxmyp = B(0, -1, 1), Bxpym = B(0, 1, -1), Bzp = B(1, 0, 0), Bxmzp = B(1, -1, 0), Bymzp = B(1, 0, -1);
     const f2 Cc = C(0, 0, 0), Cxp = C(0, 1, 0), Cxm = C(0, -1, 0), Cyp = C(0, 0, 1), Cym = C(0, 0, -1);
     const f2 fr = lo(Ac), fi = hi(Ac);
@@ -111,6 +118,10 @@ __device__ __forceinline__ void pk_site_update(PkCarry &cy, FA A, FB B, FC C, co
     const f2 cc2 = sub2(sub2(Pzx, Pzx_mx), sub2(Pyz, Pyz_my));
     cy.Pyz = Pyz;
     cy.Pzx = Pzx;
+    if (OWN) {
+        cy.Ac = Azp;
+        cy.Bc = Bzp;
+    }
     const f2 cur = make_float2(k.cur1, k.cur2);
     const f2 g0 = lo(MB), g1 = hi(MB), g2 = MC;
     const f2 e0 = add2(g0, fma2(bc(k.aGm1), g0, mul2(bc(k.bG), fma2(cur, J0, neg(mul2(cc0, bc(k.inv_dx3)))))));

@@ -1,22 +1,23 @@
 // step_tb.cu -- TWO fused kick+drift steps per pass over the lattice (temporal blocking; Eq. 17-26).
 //
 // The one-step kernel (step_tiled.cu) moves every site's 20 words through HBM once per step: 160 B per site-update,
-// which is where it saturates.  Here a CTA advances its 32 x 8 tile by two steps before anything
-// goes back to HBM -- 80 B per site-update:
-//   step 1 is evaluated on the tile AND its one-site halo (34 x 10 sites, from positions staged with a TWO-site halo);
+// which is where it saturates.  Here a CTA advances its 32 x 16 tile (TX x TBY, stage.cuh) by two
+// steps before anything goes back to HBM -- 80 B per site-update:
+//   step 1 is evaluated on the tile AND its one-site halo (34 x 18 sites, from positions staged with a TWO-site halo);
 //   its new positions go to a shared-memory ring, never to HBM;
 //   step 2 is the one-step kernel's body, reading that ring instead of staged HBM planes.
 // Both steps march through the z planes of a chunk together, step 1 one plane ahead of step 2; everything a site needs
-// from the plane below is carried in registers as in the one-step kernel.  A CTA has 8 "inner" warps (one tile site per
-// thread: step 1 and step 2) and 3 "halo" warps (the 84 sites around the tile: step 1 only), so every thread owns exactly
-// one step-1 site.  The arithmetic per site is pk_site_update() of step_site.cuh for both steps: the result is
+// from the plane below is carried in registers as in the one-step kernel.  A CTA has 16 "inner" warps (one tile site per
+// thread: step 1 and step 2) and 4 "halo" warps (the 100 sites around the tile: step 1 only), so every thread owns
+// exactly one step-1 site.  The arithmetic per site is pk_site_update() of step_site.cuh for both steps: the result is
 // bit-identical to two launches of the one-step kernel.
 // Momenta of halo sites belong to neighbouring tiles, which update them in this same launch: the kernel reads momenta
 // from one buffer and writes them to ANOTHER (the caller's aux buffer, u1u1_set_aux).  Redundant work: step 1 runs on
-// 340 / 256 of the sites and on two extra planes per chunk.
-// Shared memory (114 240 B, 2 CTAs per SM): 3 position slots (the two planes step 1 reads + one in flight), 2 momentum
-// slots (tile only; the halo threads prefetch their site's momenta into registers), 3 slots of step-1 positions (the two
-// planes step 2 reads + the one step 1 writes, so one __syncthreads per plane suffices).
+// 612 / 512 of the sites and on two extra planes per chunk of 128.
+// Shared memory (202 304 B, one CTA of 640 threads per SM, 96 registers): 3 position slots (the two planes step 1 reads
+// + one in flight), 2 momentum slots (tile only; the halo threads prefetch their site's momenta into registers), 3 slots
+// of step-1 positions (the two planes step 2 reads + the one step 1 writes, so one __syncthreads per plane suffices).
+// (TB_TY = 8 builds the first version of the round: 32 x 8 tiles, 352 threads, 2 CTAs per SM at 80 registers; 5 % slower.)
 #include <cstring>
 #include <type_traits>
 
@@ -29,18 +30,25 @@ namespace u1u1 {
 
 namespace {
 
-constexpr int NIN = NTHREADS;                   // 256 inner threads
-constexpr int NHALO = 2 * COLS + 2 * TY;        // 84 halo sites
-constexpr int TB_THREADS = NIN + 96;            // + 3 halo warps
+// step 1 carries the site's own packs A and B from plane to plane in registers (step_site.cuh, OWN): at 96 registers that
+// fits without spills and saves two 128-bit shared-memory reads per step-1 site; in step 2 as well it would spill
+constexpr bool OWN1 = TBY == 16, OWN2 = false;
+constexpr int NIN = TX * TBY;                   // inner threads (512)
+constexpr int NHALO = 2 * COLS + 2 * TBY;       // halo sites (100)
+constexpr int TB_THREADS = NIN + 32 * ((NHALO + 31) / 32);        // + halo warps (4): 640
+constexpr int TB_CTAS = TBY == 8 ? 2 : 1;       // CTAs per SM
+// a slot of step-1 positions: A, B float4[TBY + 2][COLS], C float2[TBY + 2][CCOLS] (stage.cuh's slot layout for TBY = 8)
+constexpr int I_OFF_B = (((TBY + 2) * COLS * 16 + 127) / 128) * 128, I_OFF_C = 2 * I_OFF_B;
+constexpr int I_SLOT = I_OFF_C + (((TBY + 2) * CCOLS * 8 + 127) / 128) * 128;
 constexpr int NP = 3;                           // position ring
 constexpr int MOFF_B = NIN * 16, MOFF_C = NIN * 32, MSLOT_BYTES = NIN * 40;      // momentum slot: MA | MB | MC of the tile
 constexpr int OFF_M = NP * P2_SLOT_BYTES;
 constexpr int OFF_I = OFF_M + 2 * MSLOT_BYTES;  // ring of step-1 positions (one-site halo, slot layout of stage.cuh): 3 slots
-constexpr int OFF_BARS = OFF_I + 3 * SLOT_BYTES;
-constexpr int SMEM_BYTES = OFF_BARS + 64;       // 114 240 B -> 2 CTAs per SM
+constexpr int OFF_BARS = OFF_I + 3 * I_SLOT;
+constexpr int SMEM_BYTES = OFF_BARS + 64;       // 202 304 B (TBY = 16), one CTA per SM
 constexpr int NCP_P = (3 * P2_ELEM + TB_THREADS - 1) / TB_THREADS;      // cp.async copies per thread and position plane (4)
 static_assert(OFF_M % 128 == 0 && OFF_I % 128 == 0 && OFF_BARS % 8 == 0, "alignment");
-static_assert(2 * (SMEM_BYTES + 1024) <= 233472, "two CTAs per SM");
+static_assert(TB_CTAS * (SMEM_BYTES + 1024) <= 233472, "CTAs per SM");
 
 // TMA: the tile's two-site halo lies inside the lattice, positions and momenta arrive by TMA boxes; otherwise
 // (boundary / ragged tiles) by per-thread cp.async with the periodic wrap resolved in a per-thread plan.
@@ -65,8 +73,8 @@ __device__ __forceinline__ void tb_tile(const TbLattice &L, const StepCoef &k1, 
         const int h = tid - NIN;
         if (h < COLS) { c1 = h - 1; r1 = -1; act = c1 <= wx; }
         else if (h < 2 * COLS) { c1 = h - COLS - 1; r1 = wy; act = c1 <= wx; }
-        else if (h < 2 * COLS + TY) { c1 = -1; r1 = h - 2 * COLS; act = r1 < wy; }
-        else { c1 = wx; r1 = h - 2 * COLS - TY; act = h < NHALO && r1 < wy; }
+        else if (h < 2 * COLS + TBY) { c1 = -1; r1 = h - 2 * COLS; act = r1 < wy; }
+        else { c1 = wx; r1 = h - 2 * COLS - TBY; act = h < NHALO && r1 < wy; }
     }
     const int eP = (r1 + 2) * P2_COLS + c1 + 2;                        // element index in a position slot (two-site halo)
     const int eI = (r1 + 1) * COLS + c1 + 1, eIC = (r1 + 1) * CCOLS + c1 + 2;      // in a one-site-halo slot (packs A, B / pack C)
@@ -142,8 +150,8 @@ __device__ __forceinline__ void tb_tile(const TbLattice &L, const StepCoef &k1, 
     auto fC = [&](int p, int dx, int dy) { return *reinterpret_cast<const float2 *>((p ? (P1) : (P0)) + P2_OFF_C + (eP + dy * P2_COLS + dx) * 8); }
 #define TB_ACC2(P0, P1)                                                                                                      \
     auto fA = [&](int p, int dx, int dy) { return *reinterpret_cast<const float4 *>((p ? (P1) : (P0)) + (eI + dy * COLS + dx) * 16); };         \
-    auto fB = [&](int p, int dx, int dy) { return *reinterpret_cast<const float4 *>((p ? (P1) : (P0)) + OFF_B + (eI + dy * COLS + dx) * 16); }; \
-    auto fC = [&](int p, int dx, int dy) { return *reinterpret_cast<const float2 *>((p ? (P1) : (P0)) + OFF_C + (eIC + dy * CCOLS + dx) * 8); }
+    auto fB = [&](int p, int dx, int dy) { return *reinterpret_cast<const float4 *>((p ? (P1) : (P0)) + I_OFF_B + (eI + dy * COLS + dx) * 16); }; \
+    auto fC = [&](int p, int dx, int dy) { return *reinterpret_cast<const float2 *>((p ? (P1) : (P0)) + I_OFF_C + (eIC + dy * CCOLS + dx) * 8); }
 
     // ---- prologue: position planes 0, 1, 2 and momentum planes 0, 1 in flight; step-1 carry from planes 0, 1 ----
     if (TMA) {
@@ -170,11 +178,11 @@ __device__ __forceinline__ void tb_tile(const TbLattice &L, const StepCoef &k1, 
         cp_async_wait<0>();
         __syncthreads();
     }
-    PkCarry cy1 = {bc(0.f), bc(0.f), bc(0.f), bc(0.f)}, cy2 = cy1;
+    PkCarry cy1 = {bc(0.f), bc(0.f), bc(0.f), bc(0.f), make_float4(0.f, 0.f, 0.f, 0.f), make_float4(0.f, 0.f, 0.f, 0.f)}, cy2 = cy1;
     if (act) {
         const char *p0 = smem, *p1 = smem + P2_SLOT_BYTES;
         TB_ACC1(p0, p1);
-        pk_carry_init<RR>(cy1, fA, fB, fC);
+        pk_carry_init<RR, OWN1>(cy1, fA, fB, fC);
     }
     __syncthreads();                          // everybody is done with position plane 0: its slot takes plane 3
     if (issuer) stage_P(3, 0);
@@ -183,7 +191,7 @@ __device__ __forceinline__ void tb_tile(const TbLattice &L, const StepCoef &k1, 
     unsigned sP = 1;                          // ring slot of position plane t + 1
     // slots of the step-1 planes t, t-1, t-2 as explicit pointers rotated at the end of every iteration (computing them from
     // the parity of t was miscompiled in the peeled iteration t = 1: DESIGN.md section 12)
-    char *iCur = smem + OFF_I, *iPrev = smem + OFF_I + SLOT_BYTES, *iFree = smem + OFF_I + 2 * SLOT_BYTES;
+    char *iCur = smem + OFF_I, *iPrev = smem + OFF_I + I_SLOT, *iFree = smem + OFF_I + 2 * I_SLOT;
     // iteration t: step 1 on relative plane t - 1 (position planes t+1, t+2; momentum plane t), then step 2 on relative
     // plane t - 2 (step-1 planes t-1, t)
     for (int t = 0; t <= nz + 1; t++) {
@@ -211,10 +219,10 @@ __device__ __forceinline__ void tb_tile(const TbLattice &L, const StepCoef &k1, 
             TB_ACC1(p0, p1);
             float4 OA, OB;
             float2 OC;
-            pk_site_update<RR>(cy1, fA, fB, fC, k1, MA, MB, MC, OA, OB, OC);
+            pk_site_update<RR, OWN1>(cy1, fA, fB, fC, k1, MA, MB, MC, OA, OB, OC);
             *reinterpret_cast<float4 *>(iCur + eI * 16) = OA;
-            *reinterpret_cast<float4 *>(iCur + OFF_B + eI * 16) = OB;
-            *reinterpret_cast<float2 *>(iCur + OFF_C + eIC * 8) = OC;
+            *reinterpret_cast<float4 *>(iCur + I_OFF_B + eI * 16) = OB;
+            *reinterpret_cast<float2 *>(iCur + I_OFF_C + eIC * 8) = OC;
         }
         if (!TMA) cp_async_wait<0>();         // the copies issued one iteration ago have landed
         // the one barrier of the iteration: step-1 plane t is complete; position plane t+1 and momentum plane t are consumed;
@@ -230,11 +238,11 @@ __device__ __forceinline__ void tb_tile(const TbLattice &L, const StepCoef &k1, 
         if (inner && act && t >= 1) {
             TB_ACC2(iPrev, iCur);
             if (t == 1) {
-                pk_carry_init<RR>(cy2, fA, fB, fC);
+                pk_carry_init<RR, OWN2>(cy2, fA, fB, fC);
             } else {
                 float4 OA, OB;
                 float2 OC;
-                pk_site_update<RR>(cy2, fA, fB, fC, k2, MAo, MBo, MCo, OA, OB, OC);
+                pk_site_update<RR, OWN2>(cy2, fA, fB, fC, k2, MAo, MBo, MCo, OA, OB, OC);
                 const size_t lin = (size_t)(z0 + t - 2) * NN + gsite;
                 __stcs(reinterpret_cast<float4 *>(L.mom_out) + lin, MAo);
                 __stcs(reinterpret_cast<float4 *>(L.mom_out + 4 * V) + lin, MBo);
@@ -262,22 +270,22 @@ __device__ __forceinline__ void tb_tile(const TbLattice &L, const StepCoef &k1, 
 
 // RR: explicit range reduction of the link phases in front of the SFU (step_site.cuh; tuning flag 2048)
 template <bool RR>
-__global__ void __launch_bounds__(TB_THREADS, 2)
+__global__ void __launch_bounds__(TB_THREADS, TB_CTAS)
 step_tb_kernel(TbLattice L, StepCoef k1, StepCoef k2, int zchunk, int band, const __grid_constant__ TbMaps maps)
 {
     extern __shared__ __align__(128) char smem[];
     const int N = L.N;
     // (tile, z chunk) of this CTA in band order (step_tiled.cu)
-    const int ntx = (N + TX - 1) / TX, nty = (N + TY - 1) / TY, nzc = (N + zchunk - 1) / zchunk;
+    const int ntx = (N + TX - 1) / TX, nty = (N + TBY - 1) / TBY, nzc = (N + zchunk - 1) / zchunk;
     const int full = ntx * band * nzc, bnd = blockIdx.x / full, rem = blockIdx.x - bnd * full;
     const int rows = min(band, nty - bnd * band), bzc = rem / (ntx * rows), tl = rem - bzc * (ntx * rows);
-    const int x0 = (tl % ntx) * TX, y0 = (bnd * band + tl / ntx) * TY, z0 = bzc * zchunk;
+    const int x0 = (tl % ntx) * TX, y0 = (bnd * band + tl / ntx) * TBY, z0 = bzc * zchunk;
     const int nz = min(zchunk, N - z0);
     // CTA-uniform choice of the staging path
-    if (!(k1.flags & 2) && x0 >= 2 && x0 + TX + 2 <= N && y0 >= 2 && y0 + TY + 2 <= N)
-        tb_tile<true, RR>(L, k1, k2, maps, smem, x0, y0, z0, TX, TY, nz);
+    if (!(k1.flags & 2) && x0 >= 2 && x0 + TX + 2 <= N && y0 >= 2 && y0 + TBY + 2 <= N)
+        tb_tile<true, RR>(L, k1, k2, maps, smem, x0, y0, z0, TX, TBY, nz);
     else
-        tb_tile<false, RR>(L, k1, k2, maps, smem, x0, y0, z0, min(TX, N - x0), min(TY, N - y0), nz);
+        tb_tile<false, RR>(L, k1, k2, maps, smem, x0, y0, z0, min(TX, N - x0), min(TBY, N - y0), nz);
 }
 
 }  // namespace
@@ -296,14 +304,15 @@ cudaError_t launch_step_tb(const TbLattice &L, StepCoef k1, StepCoef k2, cudaStr
     } else {
         maps = *m;
     }
-    // z chunk: the two extra step-1 planes per chunk want long chunks, L2 reuse of the halos and enough CTAs want short ones
-    int zc = (k1.flags & 512) ? 16 : (k1.flags & 1024) ? 64 : 32;
+    // z chunk: the two extra step-1 planes and the prologue per chunk want long chunks, L2 reuse of the halos and enough CTAs
+    // want short ones (measured at 1024^3 with the 32 x 16 tile: 16 planes 23.1 ms, 32: 22.3, 64: 21.9, 128: 21.6, 256: 21.7)
+    int zc = (k1.flags & 512) ? 16 : (k1.flags & 1024) ? 64 : 128;
     const int N = L.N;
-    const int ntx = (N + TX - 1) / TX, nty = (N + TY - 1) / TY;
-    while (zc > 8 && (long)ntx * nty * ((N + zc - 1) / zc) < (long)sms * 2 * 4) zc >>= 1;
+    const int ntx = (N + TX - 1) / TX, nty = (N + TBY - 1) / TBY;
+    while (zc > 8 && (long)ntx * nty * ((N + zc - 1) / zc) < (long)sms * TB_CTAS * 4) zc >>= 1;
     if (zc > N) zc = N;
     const int nzc = (N + zc - 1) / zc;
-    int band = (k1.flags & 8) ? nty : (sms * 2 + ntx - 1) / ntx;
+    int band = (k1.flags & 8) ? nty : (sms * TB_CTAS + ntx - 1) / ntx;
     if (band > nty) band = nty;
     if (rr) step_tb_kernel<true><<<(unsigned)(ntx * nty * nzc), TB_THREADS, SMEM_BYTES, st>>>(L, k1, k2, zc, band, maps);
     else step_tb_kernel<false><<<(unsigned)(ntx * nty * nzc), TB_THREADS, SMEM_BYTES, st>>>(L, k1, k2, zc, band, maps);

@@ -161,7 +161,7 @@ step_tiled_kernel(Lattice L, StepCoef k, int zchunk, int band, const __grid_cons
     // ---- carried from plane z-1: backward z hop and the two plaquettes that contain theta_z(x - z) ----
     R bzr[2] = {0, 0}, bzi[2] = {0, 0};
     float Pyz_c[2] = {0.f, 0.f}, Pzx_c[2] = {0.f, 0.f};
-    PkCarry cy = {bc(0.f), bc(0.f), bc(0.f), bc(0.f)};                              // the same, packed (PK)
+    PkCarry cy = {bc(0.f), bc(0.f), bc(0.f), bc(0.f), make_float4(0.f, 0.f, 0.f, 0.f), make_float4(0.f, 0.f, 0.f, 0.f)};                              // the same, packed (PK)
     if (PK && active) {
         const char *sc = smem, *sp = smem + SLOT_BYTES;          // planes -1 and 0
         auto pA = [&](int p, int dx, int dy) { return A(p ? sp : sc, dy * COLS + dx); };

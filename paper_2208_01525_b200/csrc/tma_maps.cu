@@ -58,6 +58,12 @@ bool encode_halo2_maps(PackMaps *m, const float *buf, size_t V, int N, int NZ)
            encode_pack(&m->C, buf + 8 * V, 2, N, NZ, P2_COLS, P2_ROWS);
 }
 
+bool encode_tb_tile_maps(PackMaps *m, const float *buf, size_t V, int N, int NZ)
+{
+    return encode_pack(&m->A, buf, 4, N, NZ, TX, TBY) && encode_pack(&m->B, buf + 4 * V, 4, N, NZ, TX, TBY) &&
+           encode_pack(&m->C, buf + 8 * V, 2, N, NZ, TX, TBY);
+}
+
 bool encode_tile_maps(PackMaps *m, const float *buf, size_t V, int N, int NZ)
 {
     return encode_pack(&m->A, buf, 4, N, NZ, TX, TY) && encode_pack(&m->B, buf + 4 * V, 4, N, NZ, TX, TY) &&
