@@ -1,6 +1,8 @@
 """Build libu1u1.so in-tree with nvcc for sm_100a (cross-compiles without a GPU).
 
     python -m paper_2208_01525_b200.build [--force] [--verbose]
+
+U1U1_NVCC_EXTRA (environment): extra nvcc flags, e.g. "-DTB_TY=8" for the 32 x 8-tile version of the two-step kernel.
 """
 from __future__ import annotations
 
