@@ -14,7 +14,7 @@
 // Momenta of halo sites belong to neighbouring tiles, which update them in this same launch: the kernel reads momenta
 // from one buffer and writes them to ANOTHER (the caller's aux buffer, u1u1_set_aux).  Redundant work: step 1 runs on
 // 612 / 512 of the sites and on two extra planes per chunk of 128.
-// Shared memory (202 304 B, one CTA of 640 threads per SM, 96 registers): 3 position slots (the two planes step 1 reads
+// Shared memory (201 152 B, one CTA of 640 threads per SM, 96 registers): 3 position slots (the two planes step 1 reads
 // + one in flight), 2 momentum slots (tile only; the halo threads prefetch their site's momenta into registers), 3 slots
 // of step-1 positions (the two planes step 2 reads + the one step 1 writes, so one __syncthreads per plane suffices).
 // (TB_TY = 8 builds the first version of the round: 32 x 8 tiles, 352 threads, 2 CTAs per SM at 80 registers; 5 % slower.)
@@ -37,15 +37,18 @@ constexpr int NIN = TX * TBY;                   // inner threads (512)
 constexpr int NHALO = 2 * COLS + 2 * TBY;       // halo sites (100)
 constexpr int TB_THREADS = NIN + 32 * ((NHALO + 31) / 32);        // + halo warps (4): 640
 constexpr int TB_CTAS = TBY == 8 ? 2 : 1;       // CTAs per SM
-// a slot of step-1 positions: A, B float4[TBY + 2][COLS], C float2[TBY + 2][CCOLS] (stage.cuh's slot layout for TBY = 8)
-constexpr int I_OFF_B = (((TBY + 2) * COLS * 16 + 127) / 128) * 128, I_OFF_C = 2 * I_OFF_B;
-constexpr int I_SLOT = I_OFF_C + (((TBY + 2) * CCOLS * 8 + 127) / 128) * 128;
+// a slot of step-1 positions: A float4[TBY + 2][COLS], then the x, y and z links as three float2[TBY + 2][COLS] arrays of
+// (p, q) pairs.  Splitting pack B makes the stencil reads that need only the x or only the y links (6 of step 2's 21)
+// contiguous 64-bit reads: two shared-memory wavefronts per warp instead of the four a 64-bit read at a 16-byte pitch
+// takes (two-way bank conflict per half-warp) -- the layout of THIS ring is free, the staged HBM planes' is not.
+constexpr int I_OFF_X = (TBY + 2) * COLS * 16, I_OFF_Y = I_OFF_X + (TBY + 2) * COLS * 8, I_OFF_C = I_OFF_Y + (TBY + 2) * COLS * 8;
+constexpr int I_SLOT = ((I_OFF_C + (TBY + 2) * COLS * 8 + 127) / 128) * 128;
 constexpr int NP = 3;                           // position ring
 constexpr int MOFF_B = NIN * 16, MOFF_C = NIN * 32, MSLOT_BYTES = NIN * 40;      // momentum slot: MA | MB | MC of the tile
 constexpr int OFF_M = NP * P2_SLOT_BYTES;
 constexpr int OFF_I = OFF_M + 2 * MSLOT_BYTES;  // ring of step-1 positions (one-site halo, slot layout of stage.cuh): 3 slots
 constexpr int OFF_BARS = OFF_I + 3 * I_SLOT;
-constexpr int SMEM_BYTES = OFF_BARS + 64;       // 202 304 B (TBY = 16), one CTA per SM
+constexpr int SMEM_BYTES = OFF_BARS + 64;       // 201 152 B (TBY = 16), one CTA per SM
 constexpr int NCP_P = (3 * P2_ELEM + TB_THREADS - 1) / TB_THREADS;      // cp.async copies per thread and position plane (4)
 static_assert(OFF_M % 128 == 0 && OFF_I % 128 == 0 && OFF_BARS % 8 == 0, "alignment");
 static_assert(TB_CTAS * (SMEM_BYTES + 1024) <= 233472, "CTAs per SM");
@@ -77,7 +80,7 @@ __device__ __forceinline__ void tb_tile(const TbLattice &L, const StepCoef &k1, 
         else { c1 = wx; r1 = h - 2 * COLS - TBY; act = h < NHALO && r1 < wy; }
     }
     const int eP = (r1 + 2) * P2_COLS + c1 + 2;                        // element index in a position slot (two-site halo)
-    const int eI = (r1 + 1) * COLS + c1 + 1, eIC = (r1 + 1) * CCOLS + c1 + 2;      // in a one-site-halo slot (packs A, B / pack C)
+    const int eI = (r1 + 1) * COLS + c1 + 1;                           // in a slot of step-1 positions (one-site halo)
     // in-plane site index: the own site of an inner thread (output), the periodic image of a halo thread's site (momenta)
     const size_t gsite = (size_t)wrapi(y0 + r1, N) * N + (size_t)wrapi(x0 + c1, N);
 
@@ -150,8 +153,12 @@ __device__ __forceinline__ void tb_tile(const TbLattice &L, const StepCoef &k1, 
     auto fC = [&](int p, int dx, int dy) { return *reinterpret_cast<const float2 *>((p ? (P1) : (P0)) + P2_OFF_C + (eP + dy * P2_COLS + dx) * 8); }
 #define TB_ACC2(P0, P1)                                                                                                      \
     auto fA = [&](int p, int dx, int dy) { return *reinterpret_cast<const float4 *>((p ? (P1) : (P0)) + (eI + dy * COLS + dx) * 16); };         \
-    auto fB = [&](int p, int dx, int dy) { return *reinterpret_cast<const float4 *>((p ? (P1) : (P0)) + I_OFF_B + (eI + dy * COLS + dx) * 16); }; \
-    auto fC = [&](int p, int dx, int dy) { return *reinterpret_cast<const float2 *>((p ? (P1) : (P0)) + I_OFF_C + (eIC + dy * CCOLS + dx) * 8); }
+    auto fB = [&](int p, int dx, int dy) {                                                                                      \
+        const float2 bx = *reinterpret_cast<const float2 *>((p ? (P1) : (P0)) + I_OFF_X + (eI + dy * COLS + dx) * 8);          \
+        const float2 by = *reinterpret_cast<const float2 *>((p ? (P1) : (P0)) + I_OFF_Y + (eI + dy * COLS + dx) * 8);          \
+        return make_float4(bx.x, bx.y, by.x, by.y);         /* the half a caller does not use is never loaded */            \
+    };                                                                                                                          \
+    auto fC = [&](int p, int dx, int dy) { return *reinterpret_cast<const float2 *>((p ? (P1) : (P0)) + I_OFF_C + (eI + dy * COLS + dx) * 8); }
 
     // ---- prologue: position planes 0, 1, 2 and momentum planes 0, 1 in flight; step-1 carry from planes 0, 1 ----
     if (TMA) {
@@ -221,8 +228,9 @@ __device__ __forceinline__ void tb_tile(const TbLattice &L, const StepCoef &k1, 
             float2 OC;
             pk_site_update<RR, OWN1>(cy1, fA, fB, fC, k1, MA, MB, MC, OA, OB, OC);
             *reinterpret_cast<float4 *>(iCur + eI * 16) = OA;
-            *reinterpret_cast<float4 *>(iCur + I_OFF_B + eI * 16) = OB;
-            *reinterpret_cast<float2 *>(iCur + I_OFF_C + eIC * 8) = OC;
+            *reinterpret_cast<float2 *>(iCur + I_OFF_X + eI * 8) = make_float2(OB.x, OB.y);
+            *reinterpret_cast<float2 *>(iCur + I_OFF_Y + eI * 8) = make_float2(OB.z, OB.w);
+            *reinterpret_cast<float2 *>(iCur + I_OFF_C + eI * 8) = OC;
         }
         if (!TMA) cp_async_wait<0>();         // the copies issued one iteration ago have landed
         // the one barrier of the iteration: step-1 plane t is complete; position plane t+1 and momentum plane t are consumed;
