@@ -153,6 +153,34 @@ int u1u1_diagnostics(u1u1_ctx *ctx, double *out_host);
  * cG = c (1+delta)/(1+omega) of the last completed step.  Synchronises the stream. */
 int u1u1_gauss_violation(u1u1_ctx *ctx, double *out_host);
 
+/* gauss_violation_static: the same eight numbers (PAPER.md:73-77 Eq. 9-10, :272) for a caller that cannot allocate
+ * device memory -- no context, no scratch buffer, and no cudaMalloc / cudaFree (or any allocating routine) inside.
+ * Who that is: code living inside a host application whose own pool already holds all of HBM (a 1024^3 run with the
+ * second momentum buffer leaves ~8 of 178 GiB), a monitor called from a loop that must not stall (cudaMalloc and
+ * cudaFree synchronise the whole device), a tool that holds nothing but a checkpoint.  Such a caller cannot supply the
+ * 10 B/site scratch buffer that u1u1_create wants, so this call reduces through a 256 KiB array built into the
+ * library image instead (every GPU that loads libu1u1.so carries it until the process exits).
+ *   state_canonical_dev  DEVICE, read only: float32 [20][N][N][N] in the canonical layout above (4-byte aligned)
+ *   N                    multiple of 4, 8 <= N <= U1U1_STATIC_MAX_N; a larger N returns U1U1_ESIZE (the built-in array
+ *                        holds 4 N partial rows and cannot grow)
+ *   dx, e1, e2           lattice spacing and the a = 1 gauge couplings e_p0, e_q0, all > 0
+ *   cG                   Gauss-law coefficient c (1+delta)/(1+omega) of the step that produced the state (what the
+ *                        context tracks for u1u1_gauss_violation); a^{2s} for a state at rest, 1 in flat space
+ *   out_dev              DEVICE, 8 doubles (8-byte aligned), layout as u1u1_gauss_violation; written by the last of the
+ *                        two kernels this call enqueues on `cuda_stream`.  The call does NOT synchronise: read `out_dev`
+ *                        after the stream has reached that point.
+ *   err_host, err_len    optional HOST buffer that receives a message when the call fails (may be NULL / 0)
+ * Returns 0 or a U1U1_E* code; nothing is enqueued on failure of the argument checks.
+ * First call on a device: looks up the device address of the built-in array (cudaGetSymbolAddress, once per device,
+ * with the current device).  Make that first call on each GPU during set-up, before any stream capture is begun.
+ * Shared state: ALL calls in the process on the same GPU use the same array and find the previous call's partial
+ * sums in it.  Every call overwrites the rows it reads, so nothing needs clearing and calls on ONE stream may follow
+ * each other freely; two calls that can overlap on the GPU (different streams, different host threads without
+ * ordering) race on the array and both results are garbage -- order them with an event. */
+#define U1U1_STATIC_MAX_N 1024
+int u1u1_gauss_violation_static(const void *state_canonical_dev, int32_t N, double dx, double e1, double e2, double cG,
+                                double *out_dev, void *cuda_stream, char *err_host, size_t err_len);
+
 /* Canonical-layout copies, DEVICE<->DEVICE (float32 [20][N][N][N]) and HOST<->DEVICE variants
  * (the host variants copy through the same stream and synchronise it). */
 int u1u1_export_state(u1u1_ctx *ctx, void *dst_dev);

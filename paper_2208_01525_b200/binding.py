@@ -14,6 +14,7 @@ LIB_PATH = os.path.join(HERE, "libu1u1.so")
 
 DIAG_LEN = 48
 GAUSS_LEN = 8
+STATIC_MAX_N = 1024        # U1U1_STATIC_MAX_N
 SEG_LEN = 8
 SEG_SLOTS = ["N_pq", "L_pq", "l_pq", "cells_kept", "segments_all", "cells_all", "largest"]
 DIAG_SLOTS = ["tau", "a", "c", "sumW_p", "sumW_q", "cells_p", "cells_q", "cells_pq", "near_p", "near_q",
@@ -50,7 +51,7 @@ class U1U1Error(RuntimeError):
 _lib = None
 SYMBOLS = ["u1u1_state_bytes", "u1u1_scratch_bytes", "u1u1_aux_bytes", "u1u1_set_aux", "u1u1_create", "u1u1_destroy", "u1u1_last_error",
            "u1u1_configure", "u1u1_init_fields", "u1u1_set_params", "u1u1_set_time", "u1u1_step", "u1u1_cool",
-           "u1u1_diagnostics", "u1u1_gauss_violation", "u1u1_export_state", "u1u1_import_state",
+           "u1u1_diagnostics", "u1u1_gauss_violation", "u1u1_gauss_violation_static", "u1u1_export_state", "u1u1_import_state",
            "u1u1_export_state_host", "u1u1_import_state_host", "u1u1_export_windings", "u1u1_export_block", "u1u1_launch_count", "u1u1_pq_segments", "u1u1_export_labels", "u1u1_import_state_tiled",
            "u1u1_slab_state_bytes", "u1u1_configure_slab", "u1u1_set_slab_peers", "u1u1_init_slab", "u1u1_export_slab",
            "u1u1_import_slab", "u1u1_push_halos", "u1u1_slab_scratch_bytes", "u1u1_push_diag_halos",
@@ -84,6 +85,7 @@ def load():
     L.u1u1_cool.argtypes = [vp, i32, d]
     L.u1u1_diagnostics.argtypes = [vp, dp]
     L.u1u1_gauss_violation.argtypes = [vp, dp]
+    L.u1u1_gauss_violation_static.argtypes = [vp, i32, d, d, d, d, vp, vp, ctypes.c_char_p, ctypes.c_size_t]
     L.u1u1_export_state.argtypes = [vp, vp]
     L.u1u1_import_state.argtypes = [vp, vp]
     L.u1u1_export_state_host.argtypes = [vp, vp]

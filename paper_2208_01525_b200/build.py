@@ -13,7 +13,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libu1u1.so")
-SOURCES = ["api.cu", "tma_maps.cu", "step_ref.cu", "step_tiled.cu", "step_tb.cu", "diag_fused.cu", "diag.cu", "segments.cu", "init.cu"]
+SOURCES = ["api.cu", "tma_maps.cu", "step_ref.cu", "step_tiled.cu", "step_tb.cu", "diag_fused.cu", "diag.cu", "gauss_static.cu", "segments.cu", "init.cu"]
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
          "-Xcompiler", "-fPIC", "--shared", "-cudart", "static"]
 

@@ -223,3 +223,27 @@ class Slab:
         assert tuple(t.shape) == (20, self.nz_own, self.N, self.N), t.shape
         self._check(self.lib.u1u1_import_slab(self._ctx, t.data_ptr()), "import_slab")
         self.stream.synchronize()
+
+
+def gauss_violation_static(state, dx: float, e1: float, e2: float, cG: float, out=None, stream=None):
+    """u1u1_gauss_violation_static: the Gauss-law norms of a canonical float32 [20, N, N, N] device tensor, for callers
+    that cannot hand the library a scratch buffer (their framework's pool owns the whole GPU, or they run where a
+    cudaMalloc would stall the device).  No context is involved and the library allocates nothing: the partial sums go
+    through a fixed array inside libu1u1.so, shared by every call on that GPU -- so keep calls on one stream, or order
+    them.  `out` (8 float64 on the same device) is filled asynchronously on `stream` and returned; pass your own to keep
+    this wrapper allocation-free as well.  Raises U1U1Error with the library's message, e.g. for N > STATIC_MAX_N."""
+    import torch
+    lib = B.load()
+    if state.dtype != torch.float32 or not state.is_cuda or not state.is_contiguous() or state.dim() != 4 \
+            or state.shape[0] != 20 or not (state.shape[1] == state.shape[2] == state.shape[3]):
+        raise B.U1U1Error("gauss_violation_static: need a contiguous float32 CUDA tensor [20, N, N, N]")
+    with torch.cuda.device(state.device):
+        if out is None:
+            out = torch.empty(B.GAUSS_LEN, dtype=torch.float64, device=state.device)
+        st = stream if stream is not None else torch.cuda.current_stream(state.device)
+        err = ctypes.create_string_buffer(256)
+        rc = lib.u1u1_gauss_violation_static(state.data_ptr(), int(state.shape[1]), dx, e1, e2, cG, out.data_ptr(),
+                                             st.cuda_stream, err, len(err))
+    if rc:
+        raise B.U1U1Error(f"{B.ERRORS.get(rc, rc)}: {err.value.decode()}")
+    return out
