@@ -133,3 +133,98 @@ def test_full_size_two_steps_per_pass_tiled_state():
     assert abs(dbig["sum_L"] - 4096 * dsmall["sum_L"]) <= 1e-9 * 4096 * abs(dsmall["sum_grad"])
     del big
     torch.cuda.empty_cache()
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# The two-step kernel against the ORACLE directly (Eq. 17-26), at the tight tolerance and at the size
+# and launch configuration bench.py times -- not through bit-identity with the one-step kernel.
+# ------------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("N,m,s,f", [(24, 2 / 3, 1.0, 1.0), (40, 0.5, -1.0, 0.5), (8, 0.0, 1.0, 1.0),
+                                      (36, 0.9, 0.0, 1.0), (132, 0.5, 0.0, 1.0)])
+def test_two_steps_per_pass_generic_state_against_oracle(N, m, s, f):
+    """The five generic cases of test_gpu_step.test_generic_state_every_term (all 20 components non-trivial, unequal
+    couplings, friction, ragged sizes, minimum size, every era, s in {1, 0, -1}) as ONE launch of the two-step kernel
+    against two oracle steps: R-16 error below 2e-5 (twice the one-step bar)."""
+    from paper_2208_01525_b200 import Params
+    K = O.Couplings(lambda1=2.0, lambda2=1.7, e1=1.0, e2=0.9, eta1=1.0, eta2=1.2, kappa=0.8)
+    prm = Params(lambda1=2.0, lambda2=1.7, e1=1.0, e2=0.9, eta1=1.0, eta2=1.2, kappa=0.8, tau_norm=1.5, friction=f)
+    s0 = inputs.to_f32_exact(inputs.random_state((N, N, N), seed=N))
+    ref = s0.copy()
+    O.step(ref, DX, K, 2.0, m, s, DTAU, tau_norm=1.5, friction=f, n=2)
+    gpu, lat = run(s0, N, prm, [(2, 2.0, m, s)], aux=True)
+    assert lat.step_launches == 1
+    err = group_errors(gpu, ref)
+    assert max(err.values()) < 2e-5, err
+
+
+@pytest.mark.parametrize("N", [40, 132])
+def test_cooling_two_steps_per_pass_against_oracle(N):
+    """u1u1_cool through the two-step kernel (one launch for two Euler steps of Eq. 27-30) against the oracle."""
+    import torch
+    from paper_2208_01525_b200 import Lattice, Params
+    K = O.Couplings(lambda1=2.0, lambda2=1.7, e1=1.0, e2=0.9, eta1=1.0, eta2=1.2, kappa=0.8)
+    prm = Params(lambda1=2.0, lambda2=1.7, e1=1.0, e2=0.9, eta1=1.0, eta2=1.2, kappa=0.8)
+    s0 = inputs.to_f32_exact(inputs.random_state((N, N, N), seed=N + 1))
+    ref = s0.copy()
+    O.cool(ref, DX, K, 1.0 / 30.0, n=2)
+    lat = Lattice(N, aux=True)
+    lat.configure(DX, prm)
+    lat.import_state(torch.from_numpy(s0.astype(np.float32)))
+    l0 = lat.launch_count()
+    lat.cool(2, 1.0 / 30.0)
+    assert lat.launch_count() - l0 == 1              # the two Euler steps were one pass of the two-step kernel
+    gpu = lat.export_state().cpu().numpy().astype(np.float64)
+    assert not gpu[inputs.MOM].any()
+    for name in ("phi", "psi", "thetaA", "thetaB"):
+        comps = inputs.GROUPS[name]
+        err = np.max(np.abs(gpu[comps] - ref[comps])) / np.max(np.abs(ref[comps]))
+        assert err < 2e-5, (name, err)
+
+
+def test_sampled_sites_full_size_two_steps_per_pass():
+    """1024^3 with the aux buffer -- the kernel and launch configuration bench.py times: 5^3 neighbourhoods are exported,
+    the lattice takes ONE two-step pass, and the oracle steps each block twice as a tiny periodic lattice.  The centre's
+    two-step cone of dependence is +-2 sites (diagonals included), so the centre is free of wrap pollution.  Sites sit on
+    the tile seams (x = 31 | 32, y = 15 | 16), the z-chunk seams (z = 127 | 128), the periodic wrap, and at random."""
+    import gc
+    import torch
+    from paper_2208_01525_b200 import Lattice, Params, state_bytes, scratch_bytes
+    N = 1024
+    gc.collect(); torch.cuda.empty_cache()
+    free, _ = torch.cuda.mem_get_info()
+    need = state_bytes(N) * 4 // 3 + scratch_bytes(N) + (1 << 30)
+    if free < need:
+        pytest.skip(f"needs {need / 2**30:.0f} GiB of free HBM, have {free / 2**30:.0f}")
+    lat = Lattice(N, aux=True)
+    prm = Params(tau_norm=256.0, friction=0.5)
+    lat.init_fields(5, DX, prm)
+    lat.step(6, 1.0, 0.5, 1.0)                       # damped prephase steps: links and momenta switch on
+    prm.friction = 1.0
+    lat.set_params(prm)
+    lat.step(2, 1.6, 0.5, 1.0)
+    tau = 1.8
+    rng = np.random.default_rng(2048)
+    sites = [(0, 0, 0), (N - 1, N - 1, N - 1), (N - 1, 0, 517), (1, N - 2, N - 1), (0, 1023, 1),
+             (31, 15, 127), (32, 16, 128), (31, 16, 128), (32, 15, 127), (63, 31, 255), (64, 32, 256),
+             (991, 1007, 895), (992, 1008, 896), (30, 14, 126), (33, 17, 129), (511, 511, 511), (512, 512, 512)]
+    sites += [tuple(int(v) for v in rng.integers(0, N, 3)) for _ in range(19)]
+    assert len(sites) >= 32
+    before = [lat.export_block(x - 2, y - 2, z - 2, 5, 5, 5).cpu().numpy().astype(np.float64) for (x, y, z) in sites]
+    l0 = lat.launch_count()
+    lat.step(2, tau, 0.5, 1.0)
+    assert lat.launch_count() - l0 == 1              # one pass of step_tb_kernel
+    after = [lat.export_block(x, y, z, 1, 1, 1).cpu().numpy().astype(np.float64).reshape(20) for (x, y, z) in sites]
+    K = O.Couplings()
+    worst = {}
+    for b, a in zip(before, after):
+        ref = b.copy()
+        O.step(ref, DX, K, tau, 0.5, 1.0, DTAU, tau_norm=256.0, n=2)
+        for name, comps in inputs.GROUPS.items():
+            scale = max(np.max(np.abs(ref[comps])), 1e-3)
+            err = np.max(np.abs(a[comps] - ref[comps, 2, 2, 2])) / scale
+            worst[name] = max(worst.get(name, 0.0), err)
+    assert max(worst.values()) < 2e-5, worst
+    g = lat.gauss_violation()
+    assert g[3] < 1e-5 and g[7] < 1e-5, g
+    del lat
+    torch.cuda.empty_cache()
