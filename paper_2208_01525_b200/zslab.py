@@ -10,6 +10,10 @@ Not the default path: the benchmark workload (1024^3) fits one GPU and runs ther
 independent replicas.  Nothing in this environment has more than one GPU, so the multi-process path is exercised with
 two ranks on ONE GPU (their kernels never wait on one another: the barrier is on the host) and the kernel path by R slab
 contexts in one process (`SlabRing`), both bit-identical to the single-lattice run.
+
+UNVERIFIED ON MORE THAN ONE GPU: the NCCL stream-ordered barrier and the peer stores across NVLink have never run on
+real multi-GPU hardware (no node with several GPUs was available in any round).  The handle exchange relies on the private
+torch calls `_share_cuda_` / `_new_shared_cuda`.
 """
 from __future__ import annotations
 
@@ -144,6 +148,7 @@ def run(size: int, steps: int, seed: int = 5, nz_global: int | None = None, chec
     slab.configure_slab(DX, prm)
     peers = open_peer_states(slab.state, dist, rank, world, up, dn)
     slab.set_slab_peers(peers[0].data_ptr(), peers[1].data_ptr())
+    slab._peers = peers                             # the context holds raw pointers into these mappings: they live as long as the slab
     token = torch.zeros(1, device=f"cuda:{dev}")
 
     def barrier():
