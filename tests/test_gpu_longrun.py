@@ -4,8 +4,9 @@ the smaller box) on a 128^3 lattice, monitored every 10 steps, for the default f
 0) and the fp64 chain (variant 4), which sits at the fp32 STORAGE floor.
 
 Recorded per run: max over the run of ||g||_2 / max(||rho||_2, ||div E||_2) per sector (reading R-17) and the largest
-non-compact link phase |theta| reached (reading R-9: the SFU phasor's error grows with |theta|).  The numbers are
-written to gpurun_out/gauss_longrun.json; the committed copy is profiles/gauss_longrun.json.
+non-compact link phase |theta| reached (reading R-9: the SFU phasor's error grows with |theta|).  The summary table
+is profiles/gauss_longrun.md; set U1U1_LONGRUN_JSON=<path> to have this test write the numbers (with the per-100-step
+series) to a file -- by default it writes nothing.
 """
 import json
 import os
@@ -64,9 +65,10 @@ def longrun(config, variant, aux=False):
     if aux:
         return out
     _results[key] = out
-    os.makedirs(os.path.join(ROOT, "gpurun_out"), exist_ok=True)
-    with open(os.path.join(ROOT, "gpurun_out", "gauss_longrun.json"), "w") as f:
-        json.dump(sorted(_results.values(), key=lambda r: (r["config"], r["variant"])), f, indent=1)
+    path = os.environ.get("U1U1_LONGRUN_JSON")
+    if path:
+        with open(path, "w") as f:
+            json.dump(sorted(_results.values(), key=lambda r: (r["config"], r["variant"])), f, indent=1)
     return out
 
 
@@ -93,7 +95,7 @@ def test_config5_default_chain_sits_at_the_storage_floor():
     has decayed with them.  The bar the arithmetic can meet is therefore "at the storage floor": the default fp32
     chain within 1.2x of the fp64 chain at every monitored step's maximum (measured: 6.77e-5 vs 6.75e-5), both under
     the measured ceiling 1e-4; up to the half light-crossing time of the box (step 310) the same 1.2x holds (the
-    values are in profiles/gauss_longrun.json)."""
+    values are in profiles/gauss_longrun.md)."""
     r0, r4 = longrun(5, 0), longrun(5, 4)
     assert r0["gauss_rel_max_after_prephase"] <= 1.2 * r4["gauss_rel_max_after_prephase"], (r0, r4)
     assert r0["gauss_rel_max_after_prephase"] < 1e-4 and r4["gauss_rel_max_after_prephase"] < 1e-4, (r0, r4)
