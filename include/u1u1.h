@@ -215,7 +215,9 @@ int u1u1_export_windings(u1u1_ctx *ctx, int32_t sector, void *w_dev, void *near_
  *   [1] L_pq     dx * sum over those segments of (N_cells - 1)             (off-by-one corrected)
  *   [2] l_pq     L_pq / N_pq (0 if there is none)                           (Eq. 38)
  *   [3] cells in those segments   [4] number of all segments   [5] number of all pq cells
- *   [6] cells of the largest segment   [7] 0
+ *   [6] cells of the largest segment
+ *   [7] plain number of cells of the region mask (all regions): equals [5] for exact overlap; with tolerance it counts a
+ *       one-cell-displaced pair twice, which is the reading R-21b replaced -- reported so both can be compared
  * The paper's production threshold is N_cells > 41 (min_cells = 42, L_pq > 20), Fig. 1 uses l_pq >= 3.5 (min_cells = 8).
  * A region's cell count is (its cells pierced by p + its cells pierced by q) / 2 (reading R-21b): the number of cells
  * for exact overlap, and the same length for a one-cell-displaced pair of lines as for a coincident pair.
@@ -311,7 +313,12 @@ enum {
     U1U1_D_MAX_THETA,    /* largest |theta| of any link (non-compact phases drift in temporal gauge; the winding
                             sweep needs |theta| < 180 and u1u1_diagnostics fails with U1U1_ESTATE beyond)  */
     U1U1_D_GAUSS,        /* 8 slots: the u1u1_gauss_violation array of the same sweep (no second pass needed) */
-    U1U1_D_USED = U1U1_D_GAUSS + 8 /* number of slots in use; the rest of the 48 are zero        */
+    U1U1_D_V2_VALID = U1U1_D_GAUSS + 8, /* 1 * [V2_L usable] + 2 * [V2_PQ usable].  Eq. 36-37 is a velocity only
+                            if the weight localises on strings: usable means R is finite with 0 <= R <= 1, i.e. 0 <= <v^2> <= 1.
+                            When the weighted sums of |Pi|^2 and |D+ phi|^2 have opposite signs, or radiation dominates them
+                            (e.g. config 5's early times, strings hundreds of lattice spacings wide), the bit is 0 and the
+                            V2 slot -- still the raw 2R/(1+R) -- must not be read as a velocity.                        */
+    U1U1_D_USED          /* number of slots in use (= U1U1_DIAG_LEN)                                */
 };
 
 #ifdef __cplusplus

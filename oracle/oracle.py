@@ -263,7 +263,8 @@ def pq_segments(Cp, Cq, dx, min_cells=1, tolerant=False):
     pierced by q) / 2 (reading R-21b): the number of its cells for exact overlap, and for one cell of tolerance the
     SAME length for a coincident and for a one-cell-displaced pair of lines (as L_pq^tol of R-13b; the plain cell count
     of the union mask would double for the displaced pair).  N_pq = regions with N >= min_cells, L_pq = dx sum (N - 1)
-    over them (:248), l_pq = L_pq / N_pq (Eq. 38).  Returns (dict, sorted list of all region counts N)."""
+    over them (:248), l_pq = L_pq / N_pq (Eq. 38).  `cells_mask` is the plain cell count of the union mask, the reading
+    R-21b replaced.  Returns (dict, sorted list of all region counts N)."""
     mask = pq_mask(Cp, Cq, tolerant)
     nz, ny, nx = mask.shape
     seen = np.zeros(mask.shape, dtype=bool)
@@ -287,7 +288,10 @@ def pq_segments(Cp, Cq, dx, min_cells=1, tolerant=False):
     kept = [n for n in sizes if n >= min_cells]
     L = dx * sum(n - 1 for n in kept)
     out = {"N_pq": len(kept), "L_pq": L, "l_pq": L / len(kept) if kept else 0.0, "cells_kept": sum(kept),
-           "segments_all": len(sizes), "cells_all": sum(sizes), "largest": max(sizes) if sizes else 0}
+           "segments_all": len(sizes), "cells_all": sum(sizes), "largest": max(sizes) if sizes else 0,
+           # the OTHER reading of a tolerant region's size, for comparison with the paper's Fig. 1: the plain number of cells
+           # of the union mask (equal to cells_all for exact overlap, about twice it for displaced pairs)
+           "cells_mask": int(np.sum(mask))}
     return out, sorted(sizes)
 
 
@@ -365,4 +369,6 @@ def derived(s, shape, dx, K):
         "f_total": L_pq / tot if tot > 0 else 0.0,
         "f_p": L_pq / L_p if L_p > 0 else 0.0,
         "v2_L": 2 * R_L / (1 + R_L), "v2_pq": 2 * R_V / (1 + R_V),
+        # Eq. 36 is a velocity only for 0 <= R <= 1 (0 <= <v^2> <= 1): bit 0 for W = L, bit 1 for W = V_int
+        "v2_valid": (1 if 0.0 <= R_L <= 1.0 else 0) + (2 if 0.0 <= R_V <= 1.0 else 0),
     }

@@ -16,13 +16,13 @@ DIAG_LEN = 48
 GAUSS_LEN = 8
 STATIC_MAX_N = 1024        # U1U1_STATIC_MAX_N
 SEG_LEN = 8
-SEG_SLOTS = ["N_pq", "L_pq", "l_pq", "cells_kept", "segments_all", "cells_all", "largest"]
+SEG_SLOTS = ["N_pq", "L_pq", "l_pq", "cells_kept", "segments_all", "cells_all", "largest", "cells_mask"]
 DIAG_SLOTS = ["tau", "a", "c", "sumW_p", "sumW_q", "cells_p", "cells_q", "cells_pq", "near_p", "near_q",
               "maxW", "sum_L", "sum_kin_L", "sum_grad_L", "sum_kin_V", "sum_grad_V", "sum_vint", "sum_kin",
               "sum_grad", "sum_elec", "sum_mag", "sum_pot", "L_p", "L_q", "L_pq", "xi_p", "xi_q", "xi_pq",
               "xi_W", "xi_L", "f_total", "f_p", "v2_L", "v2_pq", "energy", "cells_pq_tol_p", "cells_pq_tol_q", "L_pq_tol",
               "max_theta", "gauss_l2_p", "gauss_rho_p", "gauss_max_p", "gauss_rel_p", "gauss_l2_q", "gauss_rho_q",
-              "gauss_max_q", "gauss_rel_q"]
+              "gauss_max_q", "gauss_rel_q", "v2_valid"]
 ERRORS = {-1: "EINVAL", -2: "ESIZE", -3: "EPARAM", -4: "ESTATE", -5: "ECUDA", -6: "EUNSTABLE"}
 
 

@@ -610,6 +610,8 @@ static void derive_diagnostics(const u1u1_ctx *ctx, const double *r, double site
     const double RL = dn[2] != 0 ? dn[1] / dn[2] : NAN, RV = dn[4] != 0 ? dn[3] / dn[4] : NAN;
     out[U1U1_D_V2_L] = 2.0 * RL / (1.0 + RL);
     out[U1U1_D_V2_PQ] = 2.0 * RV / (1.0 + RV);
+    // a velocity only while the weight localises on strings: R finite, 0 <= R <= 1 (NaN fails both comparisons)
+    out[U1U1_D_V2_VALID] = (RL >= 0.0 && RL <= 1.0 ? 1.0 : 0.0) + (RV >= 0.0 && RV <= 1.0 ? 2.0 : 0.0);
     out[U1U1_D_ENERGY] = dx * dx * dx * (dn[6] + dn[7] + dn[8] + dn[9] + dn[10]);
     out[U1U1_D_CELLS_PQ_TOL_P] = r[32];
     out[U1U1_D_CELLS_PQ_TOL_Q] = r[33];
@@ -767,8 +769,8 @@ extern "C" int u1u1_pq_segments(u1u1_ctx *ctx, int32_t min_cells, int32_t tolera
     ctx->labels_valid = false;
     if (e != cudaSuccess) return cuda_fail(ctx, e, "pq_segments kernel launch");
     ctx->launches += 5;
-    double r[6];
-    if (int rc = fetch(ctx, r, 6)) return rc;
+    double r[7];
+    if (int rc = fetch(ctx, r, 7)) return rc;
     ctx->labels_valid = true;
     memset(out, 0, U1U1_SEG_LEN * sizeof(double));
     out[0] = r[0];
@@ -777,7 +779,8 @@ extern "C" int u1u1_pq_segments(u1u1_ctx *ctx, int32_t min_cells, int32_t tolera
     out[3] = r[2];
     out[4] = r[3];
     out[5] = r[4];
-    out[6] = r[5];
+    out[6] = r[6];
+    out[7] = r[5];
     return U1U1_OK;
 }
 

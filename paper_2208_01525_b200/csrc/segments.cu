@@ -101,26 +101,28 @@ __global__ void seg_flatten_count_kernel(int *label, int *size, const uint8_t *c
     }
 }
 
-// Partials: [segments with n >= min_cells, sum (n - 1) over them, cells n in them, all segments, all pq cells | largest n],
-// n = size / 2 (may be a half-integer for tolerant regions)
+// Partials: [segments with n >= min_cells, sum (n - 1) over them, cells n in them, all segments, all pq cells,
+// cells of the union mask | largest n], n = size / 2 (may be a half-integer for tolerant regions)
 __global__ void __launch_bounds__(RED_BLOCK) seg_reduce_kernel(const int *label, const int *size, size_t V,
                                                                int min_cells, double *partials)
 {
-    double acc[6] = {0, 0, 0, 0, 0, 0};
+    double acc[7] = {0, 0, 0, 0, 0, 0, 0};
     for (size_t lin = (size_t)blockIdx.x * blockDim.x + threadIdx.x; lin < V; lin += (size_t)gridDim.x * blockDim.x) {
-        if (label[lin] != (int)lin) continue;        // roots only
+        const int lab = label[lin];
+        if (lab >= 0) acc[5] += 1.0;                 // plain cell count of the mask (the reading R-21b replaced)
+        if (lab != (int)lin) continue;               // roots only
         const int n2 = size[lin];
         const double n = 0.5 * (double)n2;
         acc[3] += 1.0;
         acc[4] += n;
-        acc[5] = fmax(acc[5], n);
+        acc[6] = fmax(acc[6], n);
         if (n2 >= 2 * min_cells) {
             acc[0] += 1.0;
             acc[1] += n - 1.0;
             acc[2] += n;
         }
     }
-    block_reduce_store<6>(acc, 5, partials);
+    block_reduce_store<7>(acc, 6, partials);
 }
 
 }  // namespace
@@ -136,7 +138,7 @@ cudaError_t launch_segments(const uint8_t *cells, size_t V, int N, int tolerant,
     seg_merge_kernel<<<nb, RED_BLOCK, 0, st>>>(label, V, N);
     seg_flatten_count_kernel<<<nb, RED_BLOCK, 0, st>>>(label, size, cells, V);
     seg_reduce_kernel<<<nb, RED_BLOCK, 0, st>>>(label, size, V, min_cells, partials);
-    e = launch_fold(partials, nb, 6, 5, result, st);
+    e = launch_fold(partials, nb, 7, 6, result, st);
     return e != cudaSuccess ? e : cudaGetLastError();
 }
 

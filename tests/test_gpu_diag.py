@@ -238,6 +238,9 @@ def test_diagnostics_match_oracle(N, nsteps, kind):
             assert np.isclose(d[k], ref[k], rtol=1e-12), k
     for k in ("xi_L", "v2_L", "v2_pq"):
         assert np.isclose(d[k], ref[k], rtol=1e-4), (k, d[k], ref[k])
+    # the validity bits of Eq. 36 (0 <= R <= 1, i.e. 0 <= v2 <= 1), unless a v2 sits on a threshold
+    if all(min(abs(ref[k]), abs(ref[k] - 1.0)) > 1e-3 for k in ("v2_L", "v2_pq")):
+        assert d["v2_valid"] == ref["v2_valid"], (d["v2_valid"], ref["v2_valid"], ref["v2_L"], ref["v2_pq"])
 
 
 def test_known_vortex_lines_on_gpu():

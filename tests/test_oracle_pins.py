@@ -548,6 +548,13 @@ def test_derived_scalars_definitions():
     assert np.isclose(d["xi_L"], np.sqrt(2 * np.pi * vol / (0.125 * 50)))  # Eq. 33, mu = 2 pi
     assert np.isclose(d["v2_L"], 2 * (1 / 3) / (1 + 1 / 3))                # Eq. 36
     assert np.isclose(d["v2_pq"], 2 * 0.25 / 1.25)
+    assert d["v2_valid"] == 3
+    # the estimator is a velocity only for 0 <= R <= 1: opposite signs of the weighted sums (R < 0), R > 1 (<v^2> > 1)
+    # and an empty denominator (NaN) clear the bit of that weight and leave the other one alone
+    for kin_L, grad_L, kin_V, grad_V, want in [(3.0, -9.0, 1.0, 4.0, 2), (-3.0, -9.0, -1.0, 4.0, 1), (-9.5, -9.0, 1.0, 4.0, 2),
+                                                (-3.0, -9.0, 4.5, 4.0, 1), (-3.0, 0.0, 1.0, 0.0, 0), (0.0, -9.0, 4.0, 4.0, 3)]:
+        s2 = dict(s, sum_kin_L=kin_L, sum_grad_L=grad_L, sum_kin_V=kin_V, sum_grad_V=grad_V)
+        assert O.derived(s2, (8, 8, 8), 0.5, K0)["v2_valid"] == want, (kin_L, grad_L, kin_V, grad_V)
 
 
 def test_tolerant_overlap_count():
@@ -667,6 +674,7 @@ def test_pq_segments_on_hand_built_regions():
     out, sizes = O.pq_segments(Cp, Cq, 0.5)
     assert sizes == [3, 4, 7] and out["N_pq"] == 3 and out["L_pq"] == 0.5 * (2 + 3 + 6)
     assert np.isclose(out["l_pq"], 0.5 * 11 / 3) and out["largest"] == 7 and out["cells_all"] == 14
+    assert out["cells_mask"] == 14             # exact overlap: the union mask IS the set of pq cells
     out, _ = O.pq_segments(Cp, Cq, 0.5, min_cells=4)
     assert out["N_pq"] == 2 and out["L_pq"] == 0.5 * (3 + 6) and out["cells_kept"] == 11 and out["segments_all"] == 3
     # one cell of tolerance: q displaced by one cell from a p line -> both lines' cells form ONE region
@@ -676,6 +684,7 @@ def test_pq_segments_on_hand_built_regions():
     assert O.pq_segments(Cp, Cq, 0.5)[1] == []
     out, sizes = O.pq_segments(Cp, Cq, 0.5, tolerant=True)
     assert sizes == [7] and out["N_pq"] == 1 and out["cells_all"] == 7
+    assert out["cells_mask"] == 14             # the plain mask count doubles for the displaced pair (what R-21b avoids)
     # reading R-21b: the displaced 7-cell pair has the SAME length and the same threshold behaviour as the coincident one
     Cq2 = np.zeros_like(Cq)
     Cq2[2:9, 3, 3] = 2
@@ -697,6 +706,7 @@ def test_pq_segments_on_hand_built_regions():
     out4, sizes4 = O.pq_segments(Cp, Cq4, 0.5, tolerant=True)
     assert sizes4 == [7.5] and out4["L_pq"] == 0.5 * 6.5
     assert 0.5 * sum(O.cells_pq_tolerant(Cp, Cq4)) == out4["cells_all"] == 7.5
+    assert out4["cells_mask"] == 15 and out3["cells_mask"] == 3 + 2 * 4
 
 
 def test_pq_segments_against_library_labelling():
