@@ -60,23 +60,21 @@ typedef struct {
                                 (damping prephase of BASELINE.json configs 2 and 5)              */
     double smooth_width;     /* init_kind 1: Gaussian width in lattice units                     */
     int32_t smooth_trunc;    /* init_kind 1: kernel truncated at |d| <= smooth_trunc (<= 32)     */
-    int32_t kernel_variant;  /* step kernel (DESIGN.md sections 7-8):
+    int32_t kernel_variant;  /* step kernel arithmetic (DESIGN.md sections 7-8), 0 .. 7:
                                 0 = tiled, fp32 chain in DIFFERENCE FORM, SFU phasor (default: fp32 speed, Gauss
                                     residual within ~1-3x of the fp32 storage floor);
                                 2 = tiled, plain fp32 chain, SFU phasor (Gauss residual ~30x the floor);
                                 4 = tiled, fp64 kick chain, SFU phasor (Gauss residual AT the storage floor);
                                 5 / 6 / 7 = 2 / 4 / 0 with libm sincosf instead of the SFU phasor;
                                 1 / 3 = reference one-thread-per-site kernel in fp32 / fp64.
-                                Bits 4.. are tuning switches (0 in production): 16*2 = cp.async staging everywhere
-                                (no TMA), 16*4 = momenta by ld.global.cs, 16*8 = plain grid order (step kernel);
-                                16*1 = variant 0 in scalar instead of packed fp32x2 instructions (same bits);
-                                16*16 / 16*32 = L2 policies, 16*64 / 16*128 = 16 / 32-plane chunks (diagnostics);
-                                16*256 = one-step kernel even with an aux buffer, 16*512 / 16*1024 = 16 / 64-plane
-                                chunks of the two-steps-per-pass kernel;
-                                16*2048 = variant 0 with an explicit range reduction of the link phases in front of the
-                                SFU sine / cosine: phasor error 5e-7 at ANY |theta| instead of 6e-8 |theta| (identical
-                                bits while |theta| < 2 pi, ~4 % slower; for runs whose non-compact phases grow beyond ~10;
-                                u1u1_diagnostics reports max |theta|).  */
+                                (The experimental switches that used to ride in the upper bits are no longer part of
+                                this struct: include/u1u1_tuning.h.)                                  */
+    int32_t range_reduce;    /* variant 0 only: explicit range reduction of the non-compact link phases in front of the
+                                SFU sine / cosine -- phasor error 5e-7 at ANY |theta| instead of 6e-8 |theta| (identical
+                                bits while |theta| < 2 pi, ~4 % slower).  0 = off (default), 1 = on,
+                                2 = automatic: on from the first u1u1_diagnostics sweep that reports max |theta| > 10
+                                (U1U1_D_MAX_THETA) until the next configure / init_fields.                */
+    int32_t reserved;        /* 0 */
 } u1u1_params;
 
 /* Bytes of device memory the caller must provide for an N^3 lattice.

@@ -35,12 +35,21 @@ class Params(ctypes.Structure):
                 ("kappa", ctypes.c_double), ("dtau", ctypes.c_double),
                 ("tau_norm", ctypes.c_double), ("friction", ctypes.c_double),
                 ("smooth_width", ctypes.c_double), ("smooth_trunc", ctypes.c_int32),
-                ("kernel_variant", ctypes.c_int32)]
+                ("kernel_variant", ctypes.c_int32), ("range_reduce", ctypes.c_int32), ("reserved", ctypes.c_int32)]
 
     def __init__(self, **kw):
+        """kernel_variant = 0..7 (include/u1u1.h).  For the tests' convenience a value of variant + 16 * switches is split
+        here: the switches (include/u1u1_tuning.h) go to `self.tuning`, which Lattice hands to u1u1_set_tuning, and the old
+        switch 2048 becomes the named field range_reduce = 1.  The C struct never sees more than 0..7."""
         d = dict(init_kind=0, lambda1=2.0, lambda2=2.0, e1=1.0, e2=1.0, eta1=1.0, eta2=1.0, kappa=0.9,
-                 dtau=0.1, tau_norm=1.0, friction=1.0, smooth_width=5.0, smooth_trunc=20, kernel_variant=0)
+                 dtau=0.1, tau_norm=1.0, friction=1.0, smooth_width=5.0, smooth_trunc=20, kernel_variant=0,
+                 range_reduce=0, reserved=0)
         d.update(kw)
+        kv = int(d["kernel_variant"])
+        self.tuning = (kv >> 4) & 2047
+        if (kv >> 4) & 2048:
+            d["range_reduce"] = 1
+        d["kernel_variant"] = kv & 15
         super().__init__(struct_size=ctypes.sizeof(Params), **d)
 
 
@@ -56,6 +65,7 @@ SYMBOLS = ["u1u1_state_bytes", "u1u1_scratch_bytes", "u1u1_aux_bytes", "u1u1_set
            "u1u1_slab_state_bytes", "u1u1_configure_slab", "u1u1_set_slab_peers", "u1u1_init_slab", "u1u1_export_slab",
            "u1u1_import_slab", "u1u1_push_halos", "u1u1_slab_scratch_bytes", "u1u1_push_diag_halos",
            "u1u1_slab_diagnostics_partial", "u1u1_slab_diagnostics_finish"]
+TUNING_SYMBOLS = ["u1u1_set_tuning"]          # include/u1u1_tuning.h: experimental switches, outside the supported boundary
 SLAB_NRAW, SLAB_NSUM = 28, 24
 
 
@@ -80,6 +90,7 @@ def load():
     L.u1u1_configure.argtypes = [vp, i32, d, pp]
     L.u1u1_init_fields.argtypes = [vp, u64, i32, d, pp]
     L.u1u1_set_params.argtypes = [vp, pp]
+    L.u1u1_set_tuning.argtypes = [vp, ctypes.c_uint32]
     L.u1u1_set_time.argtypes = [vp, d, d, d]
     L.u1u1_step.argtypes = [vp, i32, d, d, d]
     L.u1u1_cool.argtypes = [vp, i32, d]

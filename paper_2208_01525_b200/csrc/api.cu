@@ -8,6 +8,7 @@
 #include <string>
 
 #include "../../include/u1u1.h"
+#include "../../include/u1u1_tuning.h"
 #include "common.cuh"
 #include "kernels.h"
 #include "stage.cuh"
@@ -37,6 +38,8 @@ struct u1u1_ctx {
     bool codes_valid = false;    // scratch holds the winding codes of the current state
     bool labels_valid = false;   // scratch holds segment labels of the current state
     uint64_t launches = 0;
+    uint32_t tuning = 0;         // experimental switches (u1u1_set_tuning, include/u1u1_tuning.h)
+    double last_max_theta = 0.0; // of the last diagnostics sweep since configure (range_reduce = 2)
     // device properties and TMA tensor maps, set up on the first launch (nothing here needs a GPU before that)
     int sms = 0;
     bool maps_ready = false;
@@ -161,8 +164,25 @@ static int check_params(u1u1_ctx *ctx, const u1u1_params *p)
     if (p->init_kind != 0 && p->init_kind != 1) return fail(ctx, U1U1_EINVAL, "init_kind must be 0 or 1");
     if (p->init_kind == 1 && (!(p->smooth_width > 0) || p->smooth_trunc < 1 || p->smooth_trunc > 32))
         return fail(ctx, U1U1_EINVAL, "init_kind 1 needs smooth_width > 0 and 1 <= smooth_trunc <= 32");
-    if (p->kernel_variant < 0 || (p->kernel_variant & 15) > 7 || p->kernel_variant > 65535)
-        return fail(ctx, U1U1_EINVAL, "kernel_variant must be 0..7 (+16*tuning flags)");
+    if (p->kernel_variant < 0 || p->kernel_variant > 7) return fail(ctx, U1U1_EINVAL, "kernel_variant must be 0..7");
+    if (p->range_reduce < 0 || p->range_reduce > 2 || p->reserved != 0)
+        return fail(ctx, U1U1_EINVAL, "range_reduce must be 0 (off), 1 (on) or 2 (automatic), reserved 0");
+    return U1U1_OK;
+}
+
+// switches handed to the kernels: the experimental mask + 2048 when the range reduction of the link phases is on
+static int kernel_flags(const u1u1_ctx *ctx)
+{
+    const int rr = ctx->prm.range_reduce;
+    const bool reduce = rr == 1 || (rr == 2 && ctx->last_max_theta > 10.0);
+    return (int)ctx->tuning | (reduce ? 2048 : 0);
+}
+
+extern "C" int u1u1_set_tuning(u1u1_ctx *ctx, uint32_t flags)
+{
+    if (!ctx) return U1U1_EINVAL;
+    if (flags & ~U1U1_TUNE_ALL) return fail(ctx, U1U1_EINVAL, "set_tuning: unknown switch (see include/u1u1_tuning.h)");
+    ctx->tuning = flags;
     return U1U1_OK;
 }
 
@@ -226,6 +246,7 @@ extern "C" int u1u1_configure(u1u1_ctx *ctx, int32_t N, double dx, const u1u1_pa
     ctx->a = ctx->c = ctx->cG = 1.0;
     ctx->diag_valid = ctx->codes_valid = ctx->labels_valid = false;
     ctx->maps_ready = false;
+    ctx->last_max_theta = 0.0;
     return U1U1_OK;
 }
 
@@ -320,8 +341,7 @@ static cudaError_t launch_step(u1u1_ctx *ctx, const StepCoef &q)
 // kernel variant, cubic lattice; tuning flags 1 (scalar chain) and 256 keep the one-step kernel.
 static bool pairs_enabled(const u1u1_ctx *ctx)
 {
-    const int kv = ctx->prm.kernel_variant;
-    return ctx->aux && !ctx->nz_own && (kv & 15) == 0 && !((kv >> 4) & (1 | 256)) && step_tb_supports(ctx->N);
+    return ctx->aux && !ctx->nz_own && ctx->prm.kernel_variant == 0 && !(ctx->tuning & (1 | 256)) && step_tb_supports(ctx->N);
 }
 
 // one launch, two steps: positions to the other ping-pong buffer, momenta from the current to the other momentum buffer
@@ -389,7 +409,7 @@ extern "C" int u1u1_step(u1u1_ctx *ctx, int32_t n, double tau, double era_m, dou
         q.dtau_dx = (float)(dt * dx);
         q.aSm1 = (float)(f * (1.0 - delta) / (1.0 + delta) - 1.0);
         q.aGm1 = (float)(f * (1.0 - omega) / (1.0 + omega) - 1.0);
-        q.flags = P.kernel_variant >> 4;
+        q.flags = kernel_flags(ctx);
         return U1U1_OK;
     };
     const bool pairs = pairs_enabled(ctx);      // an odd last step takes the one-step kernel
@@ -453,7 +473,7 @@ extern "C" int u1u1_cool(u1u1_ctx *ctx, int32_t n, double dcool)
     q.inv_dx3 = (float)(1.0 / (dx * dx * dx));
     q.dtau = (float)dcool;
     q.dtau_dx = (float)(dcool * dx);
-    q.flags = P.kernel_variant >> 4;
+    q.flags = kernel_flags(ctx);
     const bool pairs = pairs_enabled(ctx);
     for (int k = 0; k < n;) {
         cudaError_t e;
@@ -510,7 +530,7 @@ static FusedCoef fused_coef(const u1u1_ctx *ctx)
     k.sig2sq = (float)(P.eta2 * P.eta2);
     k.c = (float)ctx->c;
     k.inv_c = (float)(1.0 / ctx->c);
-    k.flags = P.kernel_variant >> 4;
+    k.flags = kernel_flags(ctx);
     k.nz_own = ctx->nz_own;
     return k;
 }
@@ -629,6 +649,7 @@ extern "C" int u1u1_diagnostics(u1u1_ctx *ctx, double *out)
     double r[34];
     if (int rc = fetch(ctx, r, 34)) return rc;
     // the byte lanes of the winding sweep hold wrap counts |n| <= 31: fail loudly beyond (non-compact links, reading R-9)
+    ctx->last_max_theta = std::fmax(ctx->last_max_theta, r[FR_MAXTH]);
     if (r[FR_MAXTH] > 180.0) {
         ctx->diag_valid = false;
         return fail(ctx, U1U1_ESTATE, "diagnostics: a link phase exceeds |theta| = 180, beyond the range of the winding sweep");

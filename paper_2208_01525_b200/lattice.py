@@ -66,13 +66,20 @@ class Lattice:
             pass
 
     # -- the C ABI, same names ---------------------------------------------------------------------
+    def set_tuning(self, flags: int):
+        """Experimental switches (include/u1u1_tuning.h); 0 in production."""
+        self._check(self.lib.u1u1_set_tuning(self._ctx, int(flags)), "set_tuning")
+
     def configure(self, dx: float, params: B.Params):
+        self.set_tuning(getattr(params, "tuning", 0))
         self._check(self.lib.u1u1_configure(self._ctx, self.N, dx, ctypes.byref(params)), "configure")
 
     def init_fields(self, seed: int, dx: float, params: B.Params):
+        self.set_tuning(getattr(params, "tuning", 0))
         self._check(self.lib.u1u1_init_fields(self._ctx, seed, self.N, dx, ctypes.byref(params)), "init_fields")
 
     def set_params(self, params: B.Params):
+        self.set_tuning(getattr(params, "tuning", 0))
         self._check(self.lib.u1u1_set_params(self._ctx, ctypes.byref(params)), "set_params")
 
     def set_time(self, tau: float, era_m: float, s: float):
@@ -185,7 +192,10 @@ class Slab:
     step = Lattice.step
     launch_count = Lattice.launch_count
 
+    set_tuning = Lattice.set_tuning
+
     def configure_slab(self, dx: float, params: B.Params):
+        self.set_tuning(getattr(params, "tuning", 0))
         self._check(self.lib.u1u1_configure_slab(self._ctx, self.N, self.nz_own, self.z_first, dx, ctypes.byref(params)),
                     "configure_slab")
 

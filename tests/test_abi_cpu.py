@@ -29,6 +29,12 @@ def test_every_declared_symbol_is_exported(lib):
     for n in names:
         assert hasattr(lib, n), f"{n} declared in include/u1u1.h but not exported"
     assert sorted(binding.SYMBOLS) == names
+    # the experimental switches live in a header of their own, outside the supported boundary
+    tuning = re.sub(r"/\*.*?\*/", "", open(os.path.join(ROOT, "include", "u1u1_tuning.h")).read(), flags=re.S)
+    tnames = sorted(set(re.findall(r"\b(u1u1_[a-z_]+)\s*\(", tuning)))
+    assert tnames == sorted(binding.TUNING_SYMBOLS) and all(hasattr(lib, n) for n in tnames)
+    main = open(os.path.join(ROOT, "include", "u1u1.h")).read()
+    assert "16*" not in main and "set_tuning" not in main
 
 
 def test_size_queries(lib):
@@ -45,8 +51,14 @@ def test_size_queries(lib):
 def test_params_struct_matches_header(lib):
     from paper_2208_01525_b200 import Params
     p = Params()
-    assert p.struct_size == ctypes.sizeof(Params) == 104
+    assert p.struct_size == ctypes.sizeof(Params) == 112
     assert (p.lambda1, p.e1, p.eta1, p.kappa, p.dtau) == (2.0, 1.0, 1.0, 0.9, 0.1)
+    assert (p.kernel_variant, p.range_reduce, p.reserved, p.tuning) == (0, 0, 0, 0)
+    # the binding splits the tests' shorthand variant + 16 * switches; the C struct only ever holds 0..7
+    q = Params(kernel_variant=4 + 16 * (2 | 512))
+    assert (q.kernel_variant, q.tuning, q.range_reduce) == (4, 2 | 512, 0)
+    q = Params(kernel_variant=16 * 2048)
+    assert (q.kernel_variant, q.tuning, q.range_reduce) == (0, 0, 1)
 
 
 def test_create_validates_without_gpu(lib):
@@ -66,6 +78,12 @@ def test_create_validates_without_gpu(lib):
     assert b"kappa" in lib.u1u1_last_error(ctx)
     bad = Params(); bad.struct_size = 8
     assert lib.u1u1_configure(ctx, 8, 0.5, ctypes.byref(bad)) == -1
+    bad = Params(); bad.kernel_variant = 16                                            # switches are not part of the struct any more
+    assert lib.u1u1_configure(ctx, 8, 0.5, ctypes.byref(bad)) == -1
+    bad = Params(range_reduce=3)
+    assert lib.u1u1_configure(ctx, 8, 0.5, ctypes.byref(bad)) == -1 and b"range_reduce" in lib.u1u1_last_error(ctx)
+    assert lib.u1u1_set_tuning(ctx, 4096) == -1 and lib.u1u1_set_tuning(ctx, 2 | 512) == 0 and lib.u1u1_set_tuning(ctx, 0) == 0
+    assert lib.u1u1_configure(ctx, 8, 0.5, ctypes.byref(Params(range_reduce=2))) == 0
     assert lib.u1u1_configure(ctx, 8, 0.5, ctypes.byref(p)) == 0
     assert lib.u1u1_step(ctx, 0, 1.0, 0.5, 1.0) == 0                                   # n = 0: no launch
     assert lib.u1u1_step(ctx, 1, 1.0, 1.5, 1.0) == -1                                  # era out of range

@@ -256,3 +256,27 @@ def test_large_link_phases(variant, tol):
     gpu, _ = run_gpu(s0, N, Params(kernel_variant=variant), [(1, 1.0, 0.5, 1.0)])
     err = group_errors(gpu, ref)
     assert max(err.values()) < tol, err
+
+
+def test_range_reduce_automatic():
+    """u1u1_params.range_reduce = 2: off until a diagnostics sweep reports max |theta| > 10, on from then until the next
+    configure.  Before the sweep the step equals range_reduce = 0 bit for bit, after it range_reduce = 1."""
+    import torch
+    from paper_2208_01525_b200 import Lattice, Params
+    N = 24
+    s0 = inputs.to_f32_exact(inputs.random_state((N, N, N), seed=3, amp_theta=12.0)).astype(np.float32)
+
+    def one_step(range_reduce, sweep_first):
+        lat = Lattice(N)
+        lat.configure(DX, Params(range_reduce=range_reduce))
+        lat.import_state(torch.from_numpy(s0))
+        if sweep_first:
+            assert lat.diagnostics()["max_theta"] > 30
+        lat.step(1, 1.0, 0.5, 1.0)
+        return lat.export_state().cpu().numpy()
+
+    off, on = one_step(0, False), one_step(1, False)
+    assert not np.array_equal(off, on)                      # at |theta| ~ 40 the two phasors differ
+    assert np.array_equal(one_step(2, False), off)
+    assert np.array_equal(one_step(2, True), on)
+    assert np.array_equal(one_step(0, True), off)           # the sweep alone changes nothing
