@@ -88,7 +88,9 @@ __device__ __forceinline__ void tb_tile(const TbLattice &L, const StepCoef &k1, 
     // running plane counters: position plane pp = 0 .. nz+3 is relative plane pp - 2, momentum plane mm = 0 .. nz+1 is
     // relative plane mm - 1; ring slot = pp % 3 resp. mm & 1
     const char *posb = reinterpret_cast<const char *>(L.pos_in), *momb = reinterpret_cast<const char *>(L.mom_in);
-    const unsigned long long pol_keep = policy_evict_last(), pol_stream = policy_evict_first();
+    // evict-last on both the position and the momentum boxes: the neighbouring tiles re-read the position halo and the
+    // halo threads re-read the momentum lines; evict-first on the momenta was measured and made no difference
+    const unsigned long long pol_keep = policy_evict_last();
     int planP[NCP_P];                         // cp.async path: in-plane site of each of this thread's copies (-1: none)
     if (!TMA) {
 #pragma unroll
