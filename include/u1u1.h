@@ -158,7 +158,7 @@ int u1u1_gauss_violation(u1u1_ctx *ctx, double *out_host);
  * cudaFree synchronise the whole device), a tool that holds nothing but a checkpoint.  Such a caller cannot supply the
  * 10 B/site scratch buffer that u1u1_create wants, so this call reduces through a 256 KiB array built into the
  * library image instead (every GPU that loads libu1u1.so carries it until the process exits).
- *   state_canonical_dev  DEVICE, read only: float32 [20][N][N][N] in the canonical layout above (4-byte aligned)
+ *   state_canonical_dev  DEVICE, read only: float32 [20][N][N][N] in the canonical layout above (16-byte aligned)
  *   N                    multiple of 4, 8 <= N <= U1U1_STATIC_MAX_N; a larger N returns U1U1_ESIZE (the built-in array
  *                        holds 4 N partial rows and cannot grow)
  *   dx, e1, e2           lattice spacing and the a = 1 gauge couplings e_p0, e_q0, all > 0

@@ -66,36 +66,47 @@ struct GaussArgs {
     double rho_p, rho_q;     // 2 e_p0^2 cG, 2 e_q0^2 cG
 };
 
-// One block per (z, quarter of the rows).  Row of partials: [sum g_p^2, rho_p^2, div_p^2, sum g_q^2, rho_q^2, div_q^2,
-// max|g_p|, max|g_q|].  Every block writes its whole row, so no part of the scratch has to be cleared beforehand.
+// One block per (z, quarter of the rows); a thread takes four consecutive x sites at a time, so every component plane
+// is read with 128-bit loads (N is a multiple of 4 and the state 16-byte aligned: every group of four is aligned).
+// Row of partials: [sum g_p^2, rho_p^2, div_p^2, sum g_q^2, rho_q^2, div_q^2, max|g_p|, max|g_q|].  Every block writes
+// its whole row, so no part of the scratch has to be cleared beforehand.
+__device__ inline float4 ld4(const float *p) { return *reinterpret_cast<const float4 *>(p); }
+__device__ inline float at4(const float4 &v, int j) { return j == 0 ? v.x : j == 1 ? v.y : j == 2 ? v.z : v.w; }
+
 __global__ void __launch_bounds__(RED_BLOCK) gauss_canonical_kernel(GaussArgs a, double *rows)
 {
-    const int N = a.N, z = blockIdx.x / YSPLIT, y0 = (blockIdx.x % YSPLIT) * (N / YSPLIT);
+    const int N = a.N, nq = N / 4, z = blockIdx.x / YSPLIT, y0 = (blockIdx.x % YSPLIT) * (N / YSPLIT);
     const int zm = z == 0 ? N - 1 : z - 1;
     const size_t V = a.V, NN = (size_t)N * N;
     const float *f = a.canon;
     double acc[ROW] = {0, 0, 0, 0, 0, 0, 0, 0};
-    for (int i = threadIdx.x; i < (N / YSPLIT) * N; i += RED_BLOCK) {
-        const int y = y0 + i / N, x = i % N;
+    for (int i = threadIdx.x; i < (N / YSPLIT) * nq; i += RED_BLOCK) {
+        const int y = y0 + i / nq, x = 4 * (i % nq);
         const int xm = x == 0 ? N - 1 : x - 1, ym = y == 0 ? N - 1 : y - 1;
-        const size_t lin = (size_t)x + (size_t)N * y + NN * z;
-        const size_t lx = (size_t)xm + (size_t)N * y + NN * z, ly = (size_t)x + (size_t)N * ym + NN * z,
-                     lz = (size_t)x + (size_t)N * y + NN * zm;
+        const size_t row = (size_t)N * y + NN * z, lin = row + x;
+        const size_t lx = row + xm, ly = (size_t)N * ym + NN * z + x, lz = (size_t)N * y + NN * zm + x;
 #pragma unroll
         for (int s = 0; s < 2; s++) {
             const float *fld = f + (size_t)(4 * s) * V;             // phi_re, phi_im, Pi_re, Pi_im | psi ..., Psi ...
             const float *el = f + (size_t)(11 + 6 * s) * V;         // E_xyz | H_xyz
-            double div = 0.0;
-            div += ((double)el[lin] - (double)el[lx]) * a.inv_dx;
-            div += ((double)el[V + lin] - (double)el[V + ly]) * a.inv_dx;
-            div += ((double)el[2 * V + lin] - (double)el[2 * V + lz]) * a.inv_dx;
-            const double fr = fld[lin], fi = fld[V + lin], pr = fld[2 * V + lin], pi = fld[3 * V + lin];
-            const double rho = (s ? a.rho_q : a.rho_p) * (fr * pi - fi * pr);
-            const double g = div - rho;
-            acc[3 * s + 0] += g * g;
-            acc[3 * s + 1] += rho * rho;
-            acc[3 * s + 2] += div * div;
-            acc[6 + s] = fmax(acc[6 + s], fabs(g));
+            const float4 fr = ld4(fld + lin), fi = ld4(fld + V + lin), pr = ld4(fld + 2 * V + lin), pi = ld4(fld + 3 * V + lin);
+            const float4 ex = ld4(el + lin), ey = ld4(el + V + lin), ez = ld4(el + 2 * V + lin);
+            const float4 eym = ld4(el + V + ly), ezm = ld4(el + 2 * V + lz);
+            const float exm[4] = {el[lx], ex.x, ex.y, ex.z};        // E_x of the site one to the left
+            const double coef = s ? a.rho_q : a.rho_p;
+#pragma unroll
+            for (int j = 0; j < 4; j++) {
+                double div = 0.0;
+                div += ((double)at4(ex, j) - (double)exm[j]) * a.inv_dx;
+                div += ((double)at4(ey, j) - (double)at4(eym, j)) * a.inv_dx;
+                div += ((double)at4(ez, j) - (double)at4(ezm, j)) * a.inv_dx;
+                const double rho = coef * ((double)at4(fr, j) * (double)at4(pi, j) - (double)at4(fi, j) * (double)at4(pr, j));
+                const double g = div - rho;
+                acc[3 * s + 0] += g * g;
+                acc[3 * s + 1] += rho * rho;
+                acc[3 * s + 2] += div * div;
+                acc[6 + s] = fmax(acc[6 + s], fabs(g));
+            }
         }
     }
     __shared__ double sm[ROW][RED_BLOCK / 32];
@@ -179,8 +190,8 @@ extern "C" int u1u1_gauss_violation_static(const void *state_canonical_dev, int3
     if (N < 8 || (N % 4) != 0) return refuse(err_host, err_len, U1U1_ESIZE, "N must be a multiple of 4, at least 8");
     if (!(dx > 0) || !(e1 > 0) || !(e2 > 0) || !std::isfinite(cG))
         return refuse(err_host, err_len, U1U1_EPARAM, "need dx > 0, e1 > 0, e2 > 0 and a finite cG");
-    if (((uintptr_t)state_canonical_dev & 3) || ((uintptr_t)out_dev & 7))
-        return refuse(err_host, err_len, U1U1_EINVAL, "state must be 4-byte aligned and out 8-byte aligned");
+    if (((uintptr_t)state_canonical_dev & 15) || ((uintptr_t)out_dev & 7))
+        return refuse(err_host, err_len, U1U1_EINVAL, "state must be 16-byte aligned and out 8-byte aligned");
     if (!gpu_can_reach(state_canonical_dev) || !gpu_can_reach(out_dev))
         return refuse(err_host, err_len, U1U1_EINVAL, "state and out must be memory the GPU can address (DEVICE pointers)");
 
